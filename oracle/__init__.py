@@ -1,0 +1,9 @@
+"""CPU oracle of the projection step -- TEST INFRASTRUCTURE, NOT PRODUCT (see oracle.h).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
+import this package.  It imports nothing from the CUDA package.
+"""
+from .oracle import (  # noqa: F401
+    BC_Z_PERIODIC, BC_Z_WALL, rhs, poisson, projection_step, projection_step_paper,
+    dft_axis, divergence, laplacian, threads,
+)

@@ -1,0 +1,463 @@
+/*
+ * oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT.  See oracle.h for the contract, the
+ * passages of the paper each function follows, and who may load this library.
+ *
+ * Deliberately plain: every discrete operator is written out index by index, the
+ * Fourier expansions are naive O(n^2) sums against a table of roots of unity, the
+ * tridiagonal systems are solved by the textbook Thomas recurrences.  Nothing here is
+ * blocked, fused or reordered beyond "which thread gets which independent line".
+ *
+ * build: gcc -O3 -fopenmp -fPIC -shared (no -ffast-math, no -march flags) -- see build.py
+ */
+#include "oracle.h"
+
+#include <math.h>
+#include <omp.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* ------------------------------------------------------------------ helpers */
+
+typedef struct {
+    int nx, ny, nz, wall;
+    double dx, dy, dz;
+    double rho1, rho2, rho0, dt;
+} grid_t;
+
+static int grid_init(grid_t *g, int nx, int ny, int nz, double lx, double ly, double lz,
+                     int bc_z, double rho1, double rho2, double dt) {
+    if (nx < 1 || ny < 1 || nz < 1) return 1;
+    if (!(lx > 0.0) || !(ly > 0.0) || !(lz > 0.0)) return 1;
+    if (bc_z != ORACLE_BC_Z_PERIODIC && bc_z != ORACLE_BC_Z_WALL) return 1;
+    if (bc_z == ORACLE_BC_Z_WALL && nz < 2) return 1;
+    g->nx = nx; g->ny = ny; g->nz = nz; g->wall = (bc_z == ORACLE_BC_Z_WALL);
+    g->dx = lx / nx; g->dy = ly / ny; g->dz = lz / nz;         /* uniform spacing */
+    g->rho1 = rho1; g->rho2 = rho2;
+    g->rho0 = rho1 < rho2 ? rho1 : rho2;                        /* rho0 = min density, PAPER.md:161 (R3) */
+    g->dt = dt;
+    return 0;
+}
+
+static inline size_t at(const grid_t *g, int i, int j, int k) {
+    return (size_t)i + (size_t)g->nx * ((size_t)j + (size_t)g->ny * (size_t)k);
+}
+static inline int wrap(int i, int n) { return i < 0 ? i + n : (i >= n ? i - n : i); }
+
+static void set_threads(int nthreads) {
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+    else omp_set_num_threads(omp_get_num_procs());
+}
+int oracle_threads(int nthreads) { return nthreads > 0 ? nthreads : omp_get_num_procs(); }
+
+/* cell density, eq. (2): rho = rho1*phi + rho2*(1-phi) (phi = 1 is phase 1, R11) */
+static inline double rho_c(const grid_t *g, const double *phi, int i, int j, int k) {
+    double f = phi[at(g, i, j, k)];
+    return g->rho1 * f + g->rho2 * (1.0 - f);
+}
+/* time-extrapolated pressure for constant dt: p_hat = 2 p^n - p^(n-1) (R4) */
+static inline double p_hat(const grid_t *g, const double *p, const double *p_old, int i, int j, int k) {
+    size_t q = at(g, i, j, k);
+    return 2.0 * p[q] - p_old[q];
+}
+
+/* gradient of a centred field f on the east / north / top face of cell (i,j,k) */
+static inline double grad_x(const grid_t *g, const double *f, int i, int j, int k) {
+    return (f[at(g, wrap(i + 1, g->nx), j, k)] - f[at(g, i, j, k)]) / g->dx;
+}
+static inline double grad_y(const grid_t *g, const double *f, int i, int j, int k) {
+    return (f[at(g, i, wrap(j + 1, g->ny), k)] - f[at(g, i, j, k)]) / g->dy;
+}
+static inline double grad_z(const grid_t *g, const double *f, int i, int j, int k) {
+    if (g->wall && k == g->nz - 1) return 0.0;    /* top wall face: normal gradient is 0 (R8) */
+    return (f[at(g, i, j, wrap(k + 1, g->nz))] - f[at(g, i, j, k)]) / g->dz;
+}
+
+/* the same three gradients for p_hat */
+static inline double gph_x(const grid_t *g, const double *p, const double *po, int i, int j, int k) {
+    return (p_hat(g, p, po, wrap(i + 1, g->nx), j, k) - p_hat(g, p, po, i, j, k)) / g->dx;
+}
+static inline double gph_y(const grid_t *g, const double *p, const double *po, int i, int j, int k) {
+    return (p_hat(g, p, po, i, wrap(j + 1, g->ny), k) - p_hat(g, p, po, i, j, k)) / g->dy;
+}
+static inline double gph_z(const grid_t *g, const double *p, const double *po, int i, int j, int k) {
+    if (g->wall && k == g->nz - 1) return 0.0;
+    return (p_hat(g, p, po, i, j, wrap(k + 1, g->nz)) - p_hat(g, p, po, i, j, k)) / g->dz;
+}
+
+/* face densities: arithmetic mean of the two adjacent cells (R2) */
+static inline double rho_fx(const grid_t *g, const double *phi, int i, int j, int k) {
+    return 0.5 * (rho_c(g, phi, i, j, k) + rho_c(g, phi, wrap(i + 1, g->nx), j, k));
+}
+static inline double rho_fy(const grid_t *g, const double *phi, int i, int j, int k) {
+    return 0.5 * (rho_c(g, phi, i, j, k) + rho_c(g, phi, i, wrap(j + 1, g->ny), k));
+}
+static inline double rho_fz(const grid_t *g, const double *phi, int i, int j, int k) {
+    /* at the top wall face the value is never used with a non-zero gradient; use the cell value */
+    if (g->wall && k == g->nz - 1) return rho_c(g, phi, i, j, k);
+    return 0.5 * (rho_c(g, phi, i, j, k) + rho_c(g, phi, i, j, wrap(k + 1, g->nz)));
+}
+
+/* splitting flux F = (1 - rho0/rho_f) grad p_hat on the three faces of cell (i,j,k) */
+static inline double flux_x(const grid_t *g, const double *phi, const double *p, const double *po, int i, int j, int k) {
+    return (1.0 - g->rho0 / rho_fx(g, phi, i, j, k)) * gph_x(g, p, po, i, j, k);
+}
+static inline double flux_y(const grid_t *g, const double *phi, const double *p, const double *po, int i, int j, int k) {
+    return (1.0 - g->rho0 / rho_fy(g, phi, i, j, k)) * gph_y(g, p, po, i, j, k);
+}
+static inline double flux_z(const grid_t *g, const double *phi, const double *p, const double *po, int i, int j, int k) {
+    return (1.0 - g->rho0 / rho_fz(g, phi, i, j, k)) * gph_z(g, p, po, i, j, k);
+}
+
+/* divergence of a face field at cell (i,j,k); the bottom wall face (k = -1) is 0 and not stored */
+static inline double div_at(const grid_t *g, const double *a, const double *b, const double *c, int i, int j, int k) {
+    double am = a[at(g, wrap(i - 1, g->nx), j, k)];
+    double bm = b[at(g, i, wrap(j - 1, g->ny), k)];
+    double cm = (g->wall && k == 0) ? 0.0 : c[at(g, i, j, wrap(k - 1, g->nz))];
+    size_t q = at(g, i, j, k);
+    return (a[q] - am) / g->dx + (b[q] - bm) / g->dy + (c[q] - cm) / g->dz;
+}
+
+/* ------------------------------------------------------- discrete operators */
+
+int oracle_divergence(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                      const double *u, const double *v, const double *w, double *div_out, int nthreads) {
+    grid_t g;
+    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, 1.0, 1.0, 1.0)) return 1;
+    set_threads(nthreads);
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) div_out[at(&g, i, j, k)] = div_at(&g, u, v, w, i, j, k);
+    return 0;
+}
+
+/* L p = div(grad p): (Gx p[i] - Gx p[i-1])/dx + ... with the wall faces carrying 0 */
+int oracle_laplacian(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                     const double *p, double *lap_out, int nthreads) {
+    grid_t g;
+    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, 1.0, 1.0, 1.0)) return 1;
+    set_threads(nthreads);
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                double gxp = grad_x(&g, p, i, j, k), gxm = grad_x(&g, p, wrap(i - 1, nx), j, k);
+                double gyp = grad_y(&g, p, i, j, k), gym = grad_y(&g, p, i, wrap(j - 1, ny), k);
+                double gzp = grad_z(&g, p, i, j, k);
+                double gzm = (g.wall && k == 0) ? 0.0 : grad_z(&g, p, i, j, wrap(k - 1, nz));
+                lap_out[at(&g, i, j, k)] = (gxp - gxm) / g.dx + (gyp - gym) / g.dy + (gzp - gzm) / g.dz;
+            }
+    return 0;
+}
+
+/* ------------------------------------------------------------ splitting RHS */
+
+int oracle_rhs(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+               double rho1, double rho2, double dt,
+               const double *u, const double *v, const double *w, const double *phi,
+               const double *p, const double *p_old, double *rhs_out, int nthreads) {
+    grid_t g;
+    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt)) return 1;
+    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0)) return 1;
+    set_threads(nthreads);
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                /* rho0/dt * div(u*)   -- eq. (17) */
+                double d_u = div_at(&g, u, v, w, i, j, k);
+                /* div[(1 - rho0/rho) grad p_hat]  -- splitting term of eq. (16) moved to the RHS (R1) */
+                double fxp = flux_x(&g, phi, p, p_old, i, j, k);
+                double fxm = flux_x(&g, phi, p, p_old, wrap(i - 1, nx), j, k);
+                double fyp = flux_y(&g, phi, p, p_old, i, j, k);
+                double fym = flux_y(&g, phi, p, p_old, i, wrap(j - 1, ny), k);
+                double fzp = flux_z(&g, phi, p, p_old, i, j, k);
+                double fzm = (g.wall && k == 0) ? 0.0 : flux_z(&g, phi, p, p_old, i, j, wrap(k - 1, nz));
+                double d_f = (fxp - fxm) / g.dx + (fyp - fym) / g.dy + (fzp - fzm) / g.dz;
+                rhs_out[at(&g, i, j, k)] = g.rho0 / g.dt * d_u + d_f;
+            }
+    return 0;
+}
+
+/* ------------------------------------------------------------- naive DFT */
+
+/* table of roots of unity e^{sign*2*pi*i*m/n}, m = 0..n-1, evaluated in long double */
+static int root_table(int n, int sign, double **tr, double **ti) {
+    *tr = (double *)malloc(sizeof(double) * (size_t)n);
+    *ti = (double *)malloc(sizeof(double) * (size_t)n);
+    if (!*tr || !*ti) { free(*tr); free(*ti); return 1; }
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int m = 0; m < n; ++m) {
+        long double a = two_pi * (long double)m / (long double)n;
+        (*tr)[m] = (double)cosl(a);
+        (*ti)[m] = (double)((long double)sign * sinl(a));
+    }
+    return 0;
+}
+
+#define LINE_BATCH 128  /* independent lines handed to one thread at a time; not a blocking of the sum */
+
+int oracle_dft_axis(long n_outer, int n, long n_inner, int sign,
+                    const double *in_re, const double *in_im,
+                    double *out_re, double *out_im, int nthreads) {
+    if (n_outer < 1 || n < 1 || n_inner < 1 || (sign != 1 && sign != -1)) return 1;
+    double *tr, *ti;
+    if (root_table(n, sign, &tr, &ti)) return 2;
+    set_threads(nthreads);
+    long n_batch = (n_inner + LINE_BATCH - 1) / LINE_BATCH;
+#pragma omp parallel for collapse(2) schedule(dynamic, 1)
+    for (long o = 0; o < n_outer; ++o)
+        for (long b = 0; b < n_batch; ++b) {
+            long q0 = b * LINE_BATCH;
+            int len = (int)((n_inner - q0) < LINE_BATCH ? (n_inner - q0) : LINE_BATCH);
+            double acc_re[LINE_BATCH], acc_im[LINE_BATCH];
+            for (int k = 0; k < n; ++k) {            /* output index */
+                for (int q = 0; q < len; ++q) { acc_re[q] = 0.0; acc_im[q] = 0.0; }
+                int m = 0;                           /* m = (k*j) mod n, kept exactly in integers */
+                for (int j = 0; j < n; ++j) {        /* the O(n) sum, in increasing j */
+                    double wr = tr[m], wi = ti[m];
+                    const double *xr = in_re + ((size_t)o * n + j) * (size_t)n_inner + q0;
+                    const double *xi = in_im + ((size_t)o * n + j) * (size_t)n_inner + q0;
+                    for (int q = 0; q < len; ++q) {
+                        acc_re[q] += wr * xr[q] - wi * xi[q];
+                        acc_im[q] += wr * xi[q] + wi * xr[q];
+                    }
+                    m += k; if (m >= n) m -= n;
+                }
+                double *yr = out_re + ((size_t)o * n + k) * (size_t)n_inner + q0;
+                double *yi = out_im + ((size_t)o * n + k) * (size_t)n_inner + q0;
+                for (int q = 0; q < len; ++q) { yr[q] = acc_re[q]; yi[q] = acc_im[q]; }
+            }
+        }
+    free(tr); free(ti);
+    return 0;
+}
+
+/* eigenvalues of the periodic second-difference operator (R6):
+ * lambda[m] = -2 (1 - cos(2 pi m / n)) / d^2 */
+static double *eigenvalues(int n, double d) {
+    double *lam = (double *)malloc(sizeof(double) * (size_t)n);
+    if (!lam) return NULL;
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int m = 0; m < n; ++m)
+        lam[m] = (double)(-2.0L * (1.0L - cosl(two_pi * (long double)m / (long double)n))) / (d * d);
+    return lam;
+}
+
+/* ------------------------------------------------------ tridiagonal in z */
+
+/* textbook Thomas for one (kx,ky): a x_{k-1} + b_k x_k + c x_{k+1} = d_k, a = c = 1/dz^2,
+ * b_k = -2/dz^2 + lam_xy inside, -1/dz^2 + lam_xy in the first/last row (Neumann, R7).
+ * d is complex (dr, di), the coefficients are real.  stride = distance between k and k+1.
+ * singular != 0 (the (0,0) column, lam_xy = 0): eliminate rows 0..nz-2, pin x_{nz-1} = 0,
+ * back-substitute, then remove the mean over k (R5). cp, dpr, dpi: scratch of length nz. */
+static void thomas_column(int nz, double dz, double lam_xy, int singular,
+                          double *dr, double *di, size_t stride,
+                          double *cp, double *dpr, double *dpi) {
+    const double a = 1.0 / (dz * dz), c = a;
+    const double b_end = -1.0 / (dz * dz) + lam_xy, b_in = -2.0 / (dz * dz) + lam_xy;
+    cp[0] = c / b_end;
+    dpr[0] = dr[0] / b_end;
+    dpi[0] = di[0] / b_end;
+    int last = singular ? nz - 2 : nz - 1;           /* last row that is eliminated */
+    for (int k = 1; k <= last; ++k) {
+        double b = (k == nz - 1) ? b_end : b_in;
+        double m = b - a * cp[k - 1];
+        cp[k] = c / m;
+        dpr[k] = (dr[k * stride] - a * dpr[k - 1]) / m;
+        dpi[k] = (di[k * stride] - a * dpi[k - 1]) / m;
+    }
+    if (singular) { dr[(nz - 1) * stride] = 0.0; di[(nz - 1) * stride] = 0.0; }
+    else { dr[(nz - 1) * stride] = dpr[nz - 1]; di[(nz - 1) * stride] = dpi[nz - 1]; }
+    for (int k = nz - 2; k >= 0; --k) {
+        dr[k * stride] = dpr[k] - cp[k] * dr[(k + 1) * stride];
+        di[k * stride] = dpi[k] - cp[k] * di[(k + 1) * stride];
+    }
+    if (singular) {
+        double mr = 0.0, mi = 0.0;
+        for (int k = 0; k < nz; ++k) { mr += dr[k * stride]; mi += di[k * stride]; }
+        mr /= nz; mi /= nz;
+        for (int k = 0; k < nz; ++k) { dr[k * stride] -= mr; di[k * stride] -= mi; }
+    }
+}
+
+/* --------------------------------------------------------- Poisson solve */
+
+int oracle_poisson(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                   const double *rhs, double *p_out, double *imag_residue_out, int nthreads) {
+    grid_t g;
+    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, 1.0, 1.0, 1.0)) return 1;
+    set_threads(nthreads);
+    const size_t n = (size_t)nx * ny * nz;
+    double *ar = (double *)malloc(sizeof(double) * n), *ai = (double *)calloc(n, sizeof(double));
+    double *br = (double *)malloc(sizeof(double) * n), *bi = (double *)malloc(sizeof(double) * n);
+    double *lamx = eigenvalues(nx, g.dx), *lamy = eigenvalues(ny, g.dy), *lamz = eigenvalues(nz, g.dz);
+    int rc = 0;
+    if (!ar || !ai || !br || !bi || !lamx || !lamy || !lamz) { rc = 2; goto done; }
+    memcpy(ar, rhs, sizeof(double) * n);
+
+    /* step 1: forward transform along x;  a -> b */
+    if (oracle_dft_axis((long)ny * nz, nx, 1, -1, ar, ai, br, bi, nthreads)) { rc = 2; goto done; }
+    /* step 3: forward transform along y;  b -> a   (steps 2,4,6,8 are transposes: no-ops here) */
+    if (oracle_dft_axis(nz, ny, nx, -1, br, bi, ar, ai, nthreads)) { rc = 2; goto done; }
+
+    if (!g.wall) {
+        /* triply periodic: expand along z as well, divide by the eigenvalue sum, (0,0,0) mode -> 0 */
+        if (oracle_dft_axis(1, nz, (long)nx * ny, -1, ar, ai, br, bi, nthreads)) { rc = 2; goto done; }
+#pragma omp parallel for collapse(2) schedule(static)
+        for (int kz = 0; kz < nz; ++kz)
+            for (int ky = 0; ky < ny; ++ky)
+                for (int kx = 0; kx < nx; ++kx) {
+                    size_t q = at(&g, kx, ky, kz);
+                    if (kx == 0 && ky == 0 && kz == 0) { br[q] = 0.0; bi[q] = 0.0; }
+                    else {
+                        double lam = lamx[kx] + lamy[ky] + lamz[kz];
+                        br[q] = br[q] / lam;
+                        bi[q] = bi[q] / lam;
+                    }
+                }
+        if (oracle_dft_axis(1, nz, (long)nx * ny, +1, br, bi, ar, ai, nthreads)) { rc = 2; goto done; }
+    } else {
+        /* step 5: Gauss elimination along z for every (kx,ky) */
+        int fail = 0;
+#pragma omp parallel
+        {
+            double *cp = (double *)malloc(sizeof(double) * (size_t)nz);
+            double *dpr = (double *)malloc(sizeof(double) * (size_t)nz);
+            double *dpi = (double *)malloc(sizeof(double) * (size_t)nz);
+            if (!cp || !dpr || !dpi) {
+#pragma omp atomic write
+                fail = 1;
+            } else {
+#pragma omp for collapse(2) schedule(static)
+                for (int ky = 0; ky < ny; ++ky)
+                    for (int kx = 0; kx < nx; ++kx) {
+                        size_t q = at(&g, kx, ky, 0);
+                        thomas_column(nz, g.dz, lamx[kx] + lamy[ky], (kx == 0 && ky == 0),
+                                      ar + q, ai + q, (size_t)nx * ny, cp, dpr, dpi);
+                    }
+            }
+            free(cp); free(dpr); free(dpi);
+        }
+        if (fail) { rc = 2; goto done; }
+    }
+
+    /* step 7: backward transform along y;  a -> b */
+    if (oracle_dft_axis(nz, ny, nx, +1, ar, ai, br, bi, nthreads)) { rc = 2; goto done; }
+    /* step 9: backward transform along x;  b -> a */
+    if (oracle_dft_axis((long)ny * nz, nx, 1, +1, br, bi, ar, ai, nthreads)) { rc = 2; goto done; }
+
+    {
+        /* normalisation of the unnormalised forward/backward pair (R9); real part */
+        const double norm = g.wall ? (double)nx * (double)ny : (double)nx * (double)ny * (double)nz;
+        double max_re = 0.0, max_im = 0.0;
+#pragma omp parallel for reduction(max : max_re, max_im) schedule(static)
+        for (size_t q = 0; q < n; ++q) {
+            double re = ar[q] / norm, im = ai[q] / norm;
+            p_out[q] = re;
+            if (fabs(re) > max_re) max_re = fabs(re);
+            if (fabs(im) > max_im) max_im = fabs(im);
+        }
+        if (imag_residue_out) *imag_residue_out = (max_re > 0.0) ? max_im / max_re : max_im;
+    }
+done:
+    free(ar); free(ai); free(br); free(bi); free(lamx); free(lamy); free(lamz);
+    return rc;
+}
+
+/* ------------------------------------------------------------- full step */
+
+/* u = u* - dt [ (1/rho0) grad p_new + (1/rho_f - 1/rho0) grad p_hat ]  on every stored face;
+ * at the top wall face both gradients are 0, so w keeps its entry value (R8). */
+static void correct_velocity(const grid_t *g, double *u, double *v, double *w, const double *phi,
+                             const double *p_new, const double *p, const double *p_old) {
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i) {
+                size_t q = at(g, i, j, k);
+                double rx = rho_fx(g, phi, i, j, k), ry = rho_fy(g, phi, i, j, k), rz = rho_fz(g, phi, i, j, k);
+                u[q] = u[q] - g->dt * (grad_x(g, p_new, i, j, k) / g->rho0 +
+                                       (1.0 / rx - 1.0 / g->rho0) * gph_x(g, p, p_old, i, j, k));
+                v[q] = v[q] - g->dt * (grad_y(g, p_new, i, j, k) / g->rho0 +
+                                       (1.0 / ry - 1.0 / g->rho0) * gph_y(g, p, p_old, i, j, k));
+                w[q] = w[q] - g->dt * (grad_z(g, p_new, i, j, k) / g->rho0 +
+                                       (1.0 / rz - 1.0 / g->rho0) * gph_z(g, p, p_old, i, j, k));
+            }
+}
+
+int oracle_projection_step(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                           double rho1, double rho2, double dt,
+                           double *u, double *v, double *w, const double *phi,
+                           double *p, const double *p_old, double *rhs_out, int nthreads) {
+    grid_t g;
+    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt)) return 1;
+    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0)) return 1;
+    const size_t n = (size_t)nx * ny * nz;
+    double *rhs = (double *)malloc(sizeof(double) * n), *p_new = (double *)malloc(sizeof(double) * n);
+    int rc = 0;
+    if (!rhs || !p_new) { rc = 2; goto done; }
+    if ((rc = oracle_rhs(nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt, u, v, w, phi, p, p_old, rhs, nthreads))) goto done;
+    if (rhs_out) memcpy(rhs_out, rhs, sizeof(double) * n);
+    if ((rc = oracle_poisson(nx, ny, nz, lx, ly, lz, bc_z, rhs, p_new, NULL, nthreads))) goto done;
+    set_threads(nthreads);
+    correct_velocity(&g, u, v, w, phi, p_new, p, p_old);
+    memcpy(p, p_new, sizeof(double) * n);                       /* p <- p^(n+1), zero mean */
+done:
+    free(rhs); free(p_new);
+    return rc;
+}
+
+/* the paper's incremental grouping, eqs. (16)-(19), with the sign of R1 */
+int oracle_projection_step_paper(int nx, int ny, int nz, double lx, double ly, double lz,
+                                 int bc_z, double rho1, double rho2, double dt,
+                                 double *u, double *v, double *w, const double *phi,
+                                 double *p, const double *p_old, int nthreads) {
+    grid_t g;
+    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt)) return 1;
+    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0)) return 1;
+    const size_t n = (size_t)nx * ny * nz;
+    double *us = (double *)malloc(sizeof(double) * n), *vs = (double *)malloc(sizeof(double) * n);
+    double *ws = (double *)malloc(sizeof(double) * n), *rhs = (double *)malloc(sizeof(double) * n);
+    double *psi = (double *)malloc(sizeof(double) * n);
+    int rc = 0;
+    if (!us || !vs || !ws || !rhs || !psi) { rc = 2; goto done; }
+    set_threads(nthreads);
+    /* eq. (16): u*_paper = u** - dt/rho0 [ grad p^n - (1 - rho0/rho) grad p_hat ]  (input u is the paper's u**) */
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                size_t q = at(&g, i, j, k);
+                us[q] = u[q] - dt / g.rho0 * (grad_x(&g, p, i, j, k) - flux_x(&g, phi, p, p_old, i, j, k));
+                vs[q] = v[q] - dt / g.rho0 * (grad_y(&g, p, i, j, k) - flux_y(&g, phi, p, p_old, i, j, k));
+                ws[q] = w[q] - dt / g.rho0 * (grad_z(&g, p, i, j, k) - flux_z(&g, phi, p, p_old, i, j, k));
+            }
+    /* eq. (17): L psi = rho0/dt div u*_paper */
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) rhs[at(&g, i, j, k)] = g.rho0 / dt * div_at(&g, us, vs, ws, i, j, k);
+    if ((rc = oracle_poisson(nx, ny, nz, lx, ly, lz, bc_z, rhs, psi, NULL, nthreads))) goto done;
+    set_threads(nthreads);
+    /* eq. (18): u = u*_paper - dt/rho0 grad psi */
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                size_t q = at(&g, i, j, k);
+                u[q] = us[q] - dt / g.rho0 * grad_x(&g, psi, i, j, k);
+                v[q] = vs[q] - dt / g.rho0 * grad_y(&g, psi, i, j, k);
+                w[q] = ws[q] - dt / g.rho0 * grad_z(&g, psi, i, j, k);
+            }
+    /* eq. (19): p = p^n + psi, then the zero-mean gauge (R5) */
+    {
+        double mean = 0.0;
+        for (size_t q = 0; q < n; ++q) { p[q] = p[q] + psi[q]; mean += p[q]; }
+        mean /= (double)n;
+        for (size_t q = 0; q < n; ++q) p[q] -= mean;
+    }
+done:
+    free(us); free(vs); free(ws); free(rhs); free(psi);
+    return rc;
+}

@@ -1,0 +1,95 @@
+/*
+ * oracle.h -- TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * Plain, slow, fp64 CPU statement of the pressure-correction (projection) step of
+ * the FluTAS two-fluid method, written from the paper (PAPER.md = arxiv 2204.08834):
+ *   PAPER.md:76   eq. (2)       one-fluid density  rho = rho1*phi + rho2*(1-phi)
+ *   PAPER.md:102  sec. 3        staggered MAC grid, uniform spacing, scalars at centres
+ *   PAPER.md:153-159 eqs.16-19  splitting terms, constant-coefficient Poisson equation,
+ *                               velocity correction, pressure update
+ *   PAPER.md:161                rho0 = min density, p_hat = time-extrapolated pressure,
+ *                               wall remark (normal gradient vanishes at a wall)
+ *   PAPER.md:167, 173-181       Fourier expansion in x, y -> tridiagonal system in z,
+ *                               Gauss elimination; order of the nine solver steps
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+ * leg may load this library.  It shares no code with the CUDA path and imports
+ * nothing from it.  Every function below is pinned by tests/test_oracle_pins.py
+ * (eigenpairs, dense 8^3 bordered solve, residual, gauge, div-free, fixed point,
+ * grouping identity, numpy.fft cross-check); none is "parity unpinned".
+ *
+ * Layout everywhere: x fastest, idx = i + nx*(j + ny*k), no ghost cells.
+ * u[i,j,k] lives on the east face x_{i+1/2}, v on the north face, w on the top face;
+ * p, phi at cell centres.  bc_z = 0: triply periodic; bc_z = 1: x, y periodic, z walls
+ * (no-slip w = 0 at both walls, homogeneous Neumann for p); the bottom wall face is
+ * not stored, the top wall face is w[.,.,nz-1] and must be 0 on entry.
+ *
+ * All functions return 0 on success, non-zero on bad arguments / allocation failure.
+ * nthreads <= 0 means "all cores" (OpenMP default).  OpenMP is used only across
+ * independent lines / systems / grid points, never inside a recurrence or a sum.
+ */
+#ifndef FLUTAS_ORACLE_H
+#define FLUTAS_ORACLE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { ORACLE_BC_Z_PERIODIC = 0, ORACLE_BC_Z_WALL = 1 };
+
+/* rhs = rho0/dt * div(u*) + div[(1 - rho0/rho_f) grad p_hat],  p_hat = 2 p - p_old
+ * (north_star grouping of eqs. 16-17; reading R1 of DESIGN.md). */
+int oracle_rhs(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+               double rho1, double rho2, double dt,
+               const double *u, const double *v, const double *w, const double *phi,
+               const double *p, const double *p_old, double *rhs_out, int nthreads);
+
+/* Solve L p = rhs, L = div grad (7-point Laplacian), zero-mean gauge, by the
+ * eigen-expansion of PAPER.md:167, 173-181 with NAIVE O(n^2) DFTs along x and y and
+ * (periodic z) a naive DFT along z + division by lambda_x+lambda_y+lambda_z with the
+ * (0,0,0) mode set to 0, or (wall z) textbook Thomas per (kx,ky) with the singular
+ * (0,0) column pinned (x_{nz-1} = 0) and its mean removed.
+ * imag_residue_out (nullable): max |Im p| / max |Re p| before the real part is taken. */
+int oracle_poisson(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                   const double *rhs, double *p_out, double *imag_residue_out, int nthreads);
+
+/* One full step, in place on u, v, w, p (phi, p_old untouched):
+ *   rhs as above;  L p_new = rhs;
+ *   u = u* - dt [ (1/rho0) grad p_new + (1/rho_f - 1/rho0) grad p_hat ];  p = p_new.
+ * rhs_out nullable (receives the right-hand side). */
+int oracle_projection_step(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                           double rho1, double rho2, double dt,
+                           double *u, double *v, double *w, const double *phi,
+                           double *p, const double *p_old, double *rhs_out, int nthreads);
+
+/* Same step in the paper's own incremental grouping, eqs. (16)-(19):
+ *   u' = u* - dt/rho0 [ grad p^n - (1 - rho0/rho_f) grad p_hat ];  L psi = rho0/dt div u';
+ *   u = u' - dt/rho0 grad psi;  p = p^n + psi - mean(p^n + psi).
+ * Exact-arithmetic identical to oracle_projection_step; used as a cross-check pin. */
+int oracle_projection_step_paper(int nx, int ny, int nz, double lx, double ly, double lz,
+                                 int bc_z, double rho1, double rho2, double dt,
+                                 double *u, double *v, double *w, const double *phi,
+                                 double *p, const double *p_old, int nthreads);
+
+/* Naive DFT of complex data along one axis of an (n_outer, n, n_inner) array
+ * (C order, n_inner fastest): out[o][k][q] = sum_j in[o][j][q] * exp(sign*2*pi*i*k*j/n),
+ * sign = -1 forward, +1 inverse; NOT normalised.  re/im are separate arrays.
+ * Exposed so that kernel-level parity tests can compare single transform stages. */
+int oracle_dft_axis(long n_outer, int n, long n_inner, int sign,
+                    const double *in_re, const double *in_im,
+                    double *out_re, double *out_im, int nthreads);
+
+/* Discrete operators, exposed for the pins and for sampled checks at full size. */
+int oracle_divergence(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                      const double *u, const double *v, const double *w, double *div_out,
+                      int nthreads);
+int oracle_laplacian(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                     const double *p, double *lap_out, int nthreads);
+
+/* number of OpenMP threads a call with this nthreads argument would use */
+int oracle_threads(int nthreads);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

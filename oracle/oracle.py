@@ -1,0 +1,126 @@
+"""ctypes wrapper around liboracle.so -- TEST INFRASTRUCTURE, NOT PRODUCT.
+
+numpy arrays in, numpy arrays out; fields have shape (nz, ny, nx), C-contiguous, float64
+(x fastest, matching oracle.h).  Argument marshalling only: all arithmetic is in oracle.c.
+"""
+import ctypes
+
+import numpy as np
+
+from .build import build as _build
+
+BC_Z_PERIODIC = 0
+BC_Z_WALL = 1
+
+_lib = ctypes.CDLL(_build())
+_dp = ctypes.POINTER(ctypes.c_double)
+_ci, _cd, _cl = ctypes.c_int, ctypes.c_double, ctypes.c_long
+
+_GRID = [_ci, _ci, _ci, _cd, _cd, _cd, _ci]
+_lib.oracle_rhs.argtypes = _GRID + [_cd, _cd, _cd] + [_dp] * 7 + [_ci]
+_lib.oracle_poisson.argtypes = _GRID + [_dp, _dp, _dp, _ci]
+_lib.oracle_projection_step.argtypes = _GRID + [_cd, _cd, _cd] + [_dp] * 7 + [_ci]
+_lib.oracle_projection_step_paper.argtypes = _GRID + [_cd, _cd, _cd] + [_dp] * 6 + [_ci]
+_lib.oracle_dft_axis.argtypes = [_cl, _ci, _cl, _ci, _dp, _dp, _dp, _dp, _ci]
+_lib.oracle_divergence.argtypes = _GRID + [_dp] * 4 + [_ci]
+_lib.oracle_laplacian.argtypes = _GRID + [_dp] * 2 + [_ci]
+_lib.oracle_threads.argtypes = [_ci]
+for _f in ("oracle_rhs", "oracle_poisson", "oracle_projection_step", "oracle_projection_step_paper",
+           "oracle_dft_axis", "oracle_divergence", "oracle_laplacian", "oracle_threads"):
+    getattr(_lib, _f).restype = _ci
+
+
+def _p(a):
+    return a.ctypes.data_as(_dp)
+
+
+def _field(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if a.ndim != 3 or (shape is not None and a.shape != shape):
+        raise ValueError("oracle fields must be float64 arrays of shape (nz, ny, nx)")
+    return a
+
+
+def _grid(shape, box, bc_z):
+    nz, ny, nx = shape
+    lx, ly, lz = box
+    return [nx, ny, nz, float(lx), float(ly), float(lz), int(bc_z)]
+
+
+def _check(rc, name):
+    if rc != 0:
+        raise RuntimeError(f"{name} failed with code {rc}")
+
+
+def threads(nthreads=0):
+    return _lib.oracle_threads(int(nthreads))
+
+
+def rhs(u, v, w, phi, p, p_old, box, bc_z, rho1, rho2, dt, nthreads=0):
+    u = _field(u)
+    f = [_field(a, u.shape) for a in (v, w, phi, p, p_old)]
+    out = np.empty_like(u)
+    _check(_lib.oracle_rhs(*_grid(u.shape, box, bc_z), rho1, rho2, dt, _p(u), *[_p(a) for a in f],
+                           _p(out), nthreads), "oracle_rhs")
+    return out
+
+
+def poisson(rhs_field, box, bc_z, nthreads=0, return_imag_residue=False):
+    r = _field(rhs_field)
+    out = np.empty_like(r)
+    res = ctypes.c_double(0.0)
+    _check(_lib.oracle_poisson(*_grid(r.shape, box, bc_z), _p(r), _p(out), ctypes.byref(res), nthreads),
+           "oracle_poisson")
+    return (out, res.value) if return_imag_residue else out
+
+
+def projection_step(u, v, w, phi, p, p_old, box, bc_z, rho1, rho2, dt, nthreads=0, return_rhs=False):
+    """Returns new (u, v, w, p) [and rhs]; inputs are not modified."""
+    u = _field(u).copy()
+    v, w, p = (_field(a, u.shape).copy() for a in (v, w, p))
+    phi, p_old = _field(phi, u.shape), _field(p_old, u.shape)
+    r = np.empty_like(u) if return_rhs else None
+    _check(_lib.oracle_projection_step(*_grid(u.shape, box, bc_z), rho1, rho2, dt, _p(u), _p(v), _p(w),
+                                       _p(phi), _p(p), _p(p_old), _p(r) if return_rhs else None,
+                                       nthreads), "oracle_projection_step")
+    return (u, v, w, p, r) if return_rhs else (u, v, w, p)
+
+
+def projection_step_paper(u, v, w, phi, p, p_old, box, bc_z, rho1, rho2, dt, nthreads=0):
+    u = _field(u).copy()
+    v, w, p = (_field(a, u.shape).copy() for a in (v, w, p))
+    phi, p_old = _field(phi, u.shape), _field(p_old, u.shape)
+    _check(_lib.oracle_projection_step_paper(*_grid(u.shape, box, bc_z), rho1, rho2, dt, _p(u), _p(v),
+                                             _p(w), _p(phi), _p(p), _p(p_old), nthreads),
+           "oracle_projection_step_paper")
+    return u, v, w, p
+
+
+def dft_axis(x, axis, sign, nthreads=0):
+    """Naive, unnormalised DFT of a complex array along one axis (sign=-1 forward, +1 inverse)."""
+    x = np.asarray(x)
+    n = x.shape[axis]
+    n_outer = int(np.prod(x.shape[:axis], dtype=np.int64))
+    n_inner = int(np.prod(x.shape[axis + 1:], dtype=np.int64))
+    re = np.ascontiguousarray(x.real, dtype=np.float64)
+    im = np.ascontiguousarray(x.imag, dtype=np.float64) if np.iscomplexobj(x) else np.zeros_like(re)
+    o_re, o_im = np.empty_like(re), np.empty_like(re)
+    _check(_lib.oracle_dft_axis(n_outer, n, n_inner, sign, _p(re), _p(im), _p(o_re), _p(o_im), nthreads),
+           "oracle_dft_axis")
+    return o_re + 1j * o_im
+
+
+def divergence(u, v, w, box, bc_z, nthreads=0):
+    u = _field(u)
+    v, w = _field(v, u.shape), _field(w, u.shape)
+    out = np.empty_like(u)
+    _check(_lib.oracle_divergence(*_grid(u.shape, box, bc_z), _p(u), _p(v), _p(w), _p(out), nthreads),
+           "oracle_divergence")
+    return out
+
+
+def laplacian(p, box, bc_z, nthreads=0):
+    p = _field(p)
+    out = np.empty_like(p)
+    _check(_lib.oracle_laplacian(*_grid(p.shape, box, bc_z), _p(p), _p(out), nthreads), "oracle_laplacian")
+    return out
