@@ -1,0 +1,134 @@
+/*
+ * flutas.h -- C ABI of libflutas_b200.so: the pressure-correction (projection) step of the
+ * FluTAS two-fluid incompressible solver (arxiv 2204.08834; PAPER.md = the paper's text),
+ * hand-written CUDA for NVIDIA B200 (sm_100a), fp64, one GPU.
+ *
+ * What one step computes (sec. 3.3 + 3.3.1; Algorithm 1 lines 10-13,
+ * PAPER.md:211-218), in the grouping fixed by BASELINE.json's north_star (R1):
+ *
+ *   rho_c  = rho1*phi + rho2*(1-phi)                         eq. (2),
+ *   rho_f  = mean of the two adjacent cell densities          (R2)
+ *   p_hat  = 2 p^n - p^(n-1)                                  PAPER.md:161 (constant dt)
+ *   rhs    = rho0/dt * div(u*) + div[(1 - rho0/rho_f) grad p_hat],  rho0 = min(rho1,rho2)
+ *                                                             eqs. (16)-(17)
+ *   L p^(n+1) = rhs, zero mean; L = 7-point Laplacian, solved by Fourier expansion in x, y
+ *            and (periodic z) in z / (wall z) a tridiagonal solve per (kx,ky)
+ *                                                             PAPER.md:163-167, 173-181
+ *   u = u* - dt [ (1/rho0) grad p^(n+1) + (1/rho_f - 1/rho0) grad p_hat ]
+ *                                                             eqs. (18)-(19)
+ *
+ * Grid and layout (R10): uniform spacing dx = lx/nx etc.; every field is
+ * nx*ny*nz contiguous doubles, x fastest: idx = i + nx*(j + ny*k); no ghost cells.  p, phi live at
+ * cell centres; u / v / w[i,j,k] live on the east / north / top face of cell (i,j,k).
+ * x and y are periodic.  bc_z = FLUTAS_BC_Z_PERIODIC: z periodic.  bc_z = FLUTAS_BC_Z_WALL:
+ * no-slip walls at z = 0 and z = lz (w = 0 there), homogeneous Neumann for p; the bottom wall face
+ * is not stored; the top wall face is w[.,.,nz-1], MUST be 0 on entry (not checked) and is left
+ * unchanged.
+ *
+ * All functions are extern "C", never throw and never call exit().  Unless a parameter says HOST,
+ * pointers are DEVICE pointers.  The library never prints, reads no environment variable and has no
+ * CPU fallback: without a CUDA device every call below fails with FLUTAS_ERR_CUDA / NULL.
+ */
+#ifndef FLUTAS_H
+#define FLUTAS_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct flutas_plan flutas_plan;
+
+enum { FLUTAS_BC_Z_PERIODIC = 0, FLUTAS_BC_Z_WALL = 1 };
+
+enum {
+    FLUTAS_OK = 0,
+    FLUTAS_ERR_INVALID_ARG = 1,       /* NULL pointer, non-positive length / density / dt, bad bc_z   */
+    FLUTAS_ERR_UNSUPPORTED_SIZE = 2,  /* see flutas_plan_create                                      */
+    FLUTAS_ERR_ALLOC = 3,             /* cudaMalloc / host allocation failed                          */
+    FLUTAS_ERR_CUDA = 4,              /* any other CUDA runtime error (message: flutas_last_error)    */
+    FLUTAS_ERR_ALIAS = 5              /* two field arguments overlap, or are not 16-byte aligned      */
+};
+
+/* Create a plan for an nx x ny x nz grid on a box lx x ly x lz, on the CURRENT CUDA device.
+ *   sizes:  nx, ny powers of two, 16 <= nx <= 2048, 8 <= ny <= 2048;
+ *           bc_z periodic: nz a power of two, 8 <= nz <= 2048;  bc_z wall: any nz >= 2.
+ *   rho1, rho2 > 0: densities of phase 1 (phi = 1) and phase 2 (phi = 0); rho0 = min(rho1, rho2)
+ *           (R3, R11).
+ * The plan owns, on the device: twiddle and (permuted) eigenvalue tables, and a workspace of
+ * flutas_plan_workspace_bytes() (one padded half-spectrum + the intermediate fields).
+ * Returns NULL on failure; flutas_last_error() / flutas_last_error_code() say why.
+ * A plan may be reused for any number of steps; one step in flight per plan (shared workspace). */
+flutas_plan *flutas_plan_create(int nx, int ny, int nz, double lx, double ly, double lz,
+                                int bc_z, double rho1, double rho2);
+
+/* One projection step, enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy
+ * default stream).  Returns without synchronising; no device<->host copy is made.
+ *   in : u, v, w = provisional velocity u* (the paper's u**, before the splitting terms);
+ *        phi = VoF colour phi^(n+1);  p = p^n;  p_old = p^(n-1);  dt > 0.
+ *   out: u, v, w = u^(n+1) in place;  p = p^(n+1) (zero mean) in place;  phi, p_old untouched.
+ * The six arrays must be 16-byte aligned and pairwise non-overlapping (FLUTAS_ERR_ALIAS).
+ * Launch errors are returned as FLUTAS_ERR_CUDA; asynchronous faults surface at the caller's
+ * next synchronisation. */
+int flutas_projection_step(flutas_plan *plan, double *u, double *v, double *w, const double *phi,
+                           double *p, const double *p_old, double dt, void *stream);
+
+/* The same step for HOST arrays (same layout; pinned memory makes the copies asynchronous):
+ * copies the six inputs host->device into plan-owned staging buffers (allocated on first use,
+ * 6 fields), runs flutas_projection_step, copies u, v, w, p back and SYNCHRONISES `stream`.
+ * This is the end-to-end entry point that bench.py times as `e2e`. */
+int flutas_projection_step_host(flutas_plan *plan, double *u_host, double *v_host, double *w_host,
+                                const double *phi_host, double *p_host, const double *p_old_host,
+                                double dt, void *stream);
+
+/* NULL is a no-op.  Frees every device and host resource of the plan (synchronises the device). */
+void flutas_plan_destroy(flutas_plan *plan);
+
+/* ---- the two halves of the step as calls of their own (used by the kernel-level parity tests) */
+
+/* Part (a) of the step alone: rhs_out[idx] = rho0/dt div(u*) + div[(1-rho0/rho_f) grad p_hat]
+ * (N doubles, device).  Inputs are not modified. */
+int flutas_splitting_rhs(flutas_plan *plan, const double *u, const double *v, const double *w,
+                         const double *phi, const double *p, const double *p_old, double dt,
+                         double *rhs_out, void *stream);
+
+/* Part (b) alone: solve L p = rhs in the zero-mean gauge.  rhs and p_out are
+ * N doubles on the device; p_out may alias rhs. */
+int flutas_poisson_solve(flutas_plan *plan, const double *rhs, double *p_out, void *stream);
+
+/* ---- introspection ---------------------------------------------------------------------- */
+
+/* Thread-local, NUL-terminated description / code of the last failure in this thread. */
+const char *flutas_last_error(void);
+int flutas_last_error_code(void);
+
+/* Device bytes owned by the plan (tables + workspace; staging buffers of the _host entry excluded). */
+size_t flutas_plan_workspace_bytes(const flutas_plan *plan);
+
+/* Number of kernel launches one flutas_projection_step enqueues, and their names
+ * (idx in [0, launches); returns NULL outside). */
+int flutas_plan_kernel_launches(const flutas_plan *plan);
+const char *flutas_plan_kernel_name(const flutas_plan *plan, int idx);
+
+/* Per-kernel device timing.  flutas_plan_set_timing(plan, 1) makes every following step record a
+ * CUDA event before and after each of its kernels on the step's stream (events only; no
+ * synchronisation).  flutas_plan_read_timing SYNCHRONISES the events, adds up the elapsed time of
+ * every kernel since the last read, writes ms_out[idx] = total milliseconds of kernel idx
+ * (n_out >= flutas_plan_kernel_launches) and steps_out = number of steps covered, then resets.
+ * At most 256 steps can be pending between two reads (older ones are dropped from the totals). */
+int flutas_plan_set_timing(flutas_plan *plan, int enabled);
+int flutas_plan_read_timing(flutas_plan *plan, float *ms_out, int n_out, int *steps_out);
+
+/* Algorithmic (modelled) HBM bytes kernel idx moves per launch: 8 bytes x the fields it must read
+ * and write once; used by bench.py for the roofline line. */
+double flutas_plan_kernel_bytes(const flutas_plan *plan, int idx);
+
+/* Advanced tuning knob for experiments (never needed for correctness): "y_cols" / "z_cols" = 4 or 8,
+ * the number of kx columns one CTA transforms in the y / z pass. */
+int flutas_plan_set_option(flutas_plan *plan, const char *name, int value);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FLUTAS_H */

@@ -4,6 +4,6 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl refere
 import this package.  It imports nothing from the CUDA package.
 """
 from .oracle import (  # noqa: F401
-    BC_Z_PERIODIC, BC_Z_WALL, rhs, poisson, projection_step, projection_step_paper,
+    BC_Z_PERIODIC, BC_Z_WALL, rhs, poisson, projection_step, projection_step_paper, correction,
     dft_axis, divergence, laplacian, threads,
 )

@@ -386,6 +386,18 @@ static void correct_velocity(const grid_t *g, double *u, double *v, double *w, c
             }
 }
 
+int oracle_correction(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                      double rho1, double rho2, double dt,
+                      double *u, double *v, double *w, const double *phi,
+                      const double *p, const double *p_old, const double *p_new, int nthreads) {
+    grid_t g;
+    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt)) return 1;
+    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0)) return 1;
+    set_threads(nthreads);
+    correct_velocity(&g, u, v, w, phi, p_new, p, p_old);
+    return 0;
+}
+
 int oracle_projection_step(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
                            double rho1, double rho2, double dt,
                            double *u, double *v, double *w, const double *phi,

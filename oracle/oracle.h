@@ -62,6 +62,14 @@ int oracle_projection_step(int nx, int ny, int nz, double lx, double ly, double 
                            double *u, double *v, double *w, const double *phi,
                            double *p, const double *p_old, double *rhs_out, int nthreads);
 
+/* The last part of the step alone (eq. 18 in the north_star grouping), in place on u, v, w:
+ *   u = u* - dt [ (1/rho0) grad p_new + (1/rho_f - 1/rho0) grad p_hat ],  p_hat = 2 p - p_old.
+ * Lets a test check the velocity correction at full size given any p_new. */
+int oracle_correction(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                      double rho1, double rho2, double dt,
+                      double *u, double *v, double *w, const double *phi,
+                      const double *p, const double *p_old, const double *p_new, int nthreads);
+
 /* Same step in the paper's own incremental grouping, eqs. (16)-(19):
  *   u' = u* - dt/rho0 [ grad p^n - (1 - rho0/rho_f) grad p_hat ];  L psi = rho0/dt div u';
  *   u = u' - dt/rho0 grad psi;  p = p^n + psi - mean(p^n + psi).

@@ -21,6 +21,8 @@ _lib.oracle_rhs.argtypes = _GRID + [_cd, _cd, _cd] + [_dp] * 7 + [_ci]
 _lib.oracle_poisson.argtypes = _GRID + [_dp, _dp, _dp, _ci]
 _lib.oracle_projection_step.argtypes = _GRID + [_cd, _cd, _cd] + [_dp] * 7 + [_ci]
 _lib.oracle_projection_step_paper.argtypes = _GRID + [_cd, _cd, _cd] + [_dp] * 6 + [_ci]
+_lib.oracle_correction.argtypes = _GRID + [_cd, _cd, _cd] + [_dp] * 7 + [_ci]
+_lib.oracle_correction.restype = _ci
 _lib.oracle_dft_axis.argtypes = [_cl, _ci, _cl, _ci, _dp, _dp, _dp, _dp, _ci]
 _lib.oracle_divergence.argtypes = _GRID + [_dp] * 4 + [_ci]
 _lib.oracle_laplacian.argtypes = _GRID + [_dp] * 2 + [_ci]
@@ -84,6 +86,16 @@ def projection_step(u, v, w, phi, p, p_old, box, bc_z, rho1, rho2, dt, nthreads=
                                        _p(phi), _p(p), _p(p_old), _p(r) if return_rhs else None,
                                        nthreads), "oracle_projection_step")
     return (u, v, w, p, r) if return_rhs else (u, v, w, p)
+
+
+def correction(u, v, w, phi, p, p_old, p_new, box, bc_z, rho1, rho2, dt, nthreads=0):
+    """Returns corrected (u, v, w) given p_new; inputs are not modified."""
+    u = _field(u).copy()
+    v, w = (_field(a, u.shape).copy() for a in (v, w))
+    phi, p, p_old, p_new = (_field(a, u.shape) for a in (phi, p, p_old, p_new))
+    _check(_lib.oracle_correction(*_grid(u.shape, box, bc_z), rho1, rho2, dt, _p(u), _p(v), _p(w), _p(phi),
+                                  _p(p), _p(p_old), _p(p_new), nthreads), "oracle_correction")
+    return u, v, w
 
 
 def projection_step_paper(u, v, w, phi, p, p_old, box, bc_z, rho1, rho2, dt, nthreads=0):

@@ -1,0 +1,169 @@
+"""Thin ctypes binding of libflutas_b200.so (include/flutas.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; torch is used for device memory and
+streams.  Importing this module fails loudly if the library cannot be built or loaded: there is
+no CPU fallback.
+"""
+import ctypes
+
+from .build import build as _build
+
+BC_Z_PERIODIC = 0
+BC_Z_WALL = 1
+
+_vp, _ci, _cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+lib = ctypes.CDLL(_build())
+
+lib.flutas_plan_create.argtypes = [_ci, _ci, _ci, _cd, _cd, _cd, _ci, _cd, _cd]
+lib.flutas_plan_create.restype = _vp
+lib.flutas_plan_destroy.argtypes = [_vp]
+lib.flutas_plan_destroy.restype = None
+lib.flutas_projection_step.argtypes = [_vp] * 7 + [_cd, _vp]
+lib.flutas_projection_step.restype = _ci
+lib.flutas_projection_step_host.argtypes = [_vp] * 7 + [_cd, _vp]
+lib.flutas_projection_step_host.restype = _ci
+lib.flutas_splitting_rhs.argtypes = [_vp] * 7 + [_cd, _vp, _vp]
+lib.flutas_splitting_rhs.restype = _ci
+lib.flutas_poisson_solve.argtypes = [_vp, _vp, _vp, _vp]
+lib.flutas_poisson_solve.restype = _ci
+lib.flutas_last_error.argtypes = []
+lib.flutas_last_error.restype = ctypes.c_char_p
+lib.flutas_last_error_code.argtypes = []
+lib.flutas_last_error_code.restype = _ci
+lib.flutas_plan_workspace_bytes.argtypes = [_vp]
+lib.flutas_plan_workspace_bytes.restype = ctypes.c_size_t
+lib.flutas_plan_kernel_launches.argtypes = [_vp]
+lib.flutas_plan_kernel_launches.restype = _ci
+lib.flutas_plan_kernel_name.argtypes = [_vp, _ci]
+lib.flutas_plan_kernel_name.restype = ctypes.c_char_p
+lib.flutas_plan_kernel_bytes.argtypes = [_vp, _ci]
+lib.flutas_plan_kernel_bytes.restype = _cd
+lib.flutas_plan_set_timing.argtypes = [_vp, _ci]
+lib.flutas_plan_set_timing.restype = _ci
+lib.flutas_plan_read_timing.argtypes = [_vp, ctypes.POINTER(ctypes.c_float), _ci, ctypes.POINTER(_ci)]
+lib.flutas_plan_read_timing.restype = _ci
+lib.flutas_plan_set_option.argtypes = [_vp, ctypes.c_char_p, _ci]
+lib.flutas_plan_set_option.restype = _ci
+
+EXPORTS = [
+    "flutas_plan_create", "flutas_projection_step", "flutas_projection_step_host", "flutas_plan_destroy",
+    "flutas_splitting_rhs", "flutas_poisson_solve", "flutas_last_error", "flutas_last_error_code",
+    "flutas_plan_workspace_bytes", "flutas_plan_kernel_launches", "flutas_plan_kernel_name",
+    "flutas_plan_set_timing", "flutas_plan_read_timing", "flutas_plan_kernel_bytes", "flutas_plan_set_option",
+]
+
+
+class FlutasError(RuntimeError):
+    def __init__(self, code, message):
+        super().__init__(f"flutas error {code}: {message}")
+        self.code = code
+
+
+def _raise_last():
+    raise FlutasError(lib.flutas_last_error_code(), lib.flutas_last_error().decode())
+
+
+def _check(rc):
+    if rc != 0:
+        raise FlutasError(rc, lib.flutas_last_error().decode())
+
+
+def _dev_ptr(t, npts):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+            and t.numel() == npts):
+        raise ValueError("expected a contiguous float64 CUDA tensor with nx*ny*nz elements")
+    return t.data_ptr()
+
+
+def _stream():
+    import torch
+    return torch.cuda.current_stream().cuda_stream
+
+
+class Plan:
+    """flutas_plan_create / flutas_projection_step / flutas_plan_destroy with the same argument order."""
+
+    def __init__(self, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2):
+        self._h = None
+        h = lib.flutas_plan_create(int(nx), int(ny), int(nz), float(lx), float(ly), float(lz), int(bc_z),
+                                   float(rho1), float(rho2))
+        if not h:
+            _raise_last()
+        self._h = h
+        self.nx, self.ny, self.nz, self.bc_z = int(nx), int(ny), int(nz), int(bc_z)
+        self.npts = self.nx * self.ny * self.nz
+
+    def destroy(self):
+        if self._h:
+            lib.flutas_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    # --- the step (device tensors, in place on u, v, w, p)
+    def projection_step(self, u, v, w, phi, p, p_old, dt, stream=None):
+        ptrs = [_dev_ptr(t, self.npts) for t in (u, v, w, phi, p, p_old)]
+        _check(lib.flutas_projection_step(self._h, *ptrs, float(dt), _stream() if stream is None else stream))
+
+    # --- the step for host arrays (numpy float64 or pinned torch CPU tensors), in place, synchronous
+    def projection_step_host(self, u, v, w, phi, p, p_old, dt, stream=None):
+        ptrs = [_host_ptr(a, self.npts) for a in (u, v, w, phi, p, p_old)]
+        _check(lib.flutas_projection_step_host(self._h, *ptrs, float(dt), _stream() if stream is None else stream))
+
+    def splitting_rhs(self, u, v, w, phi, p, p_old, dt, rhs_out, stream=None):
+        ptrs = [_dev_ptr(t, self.npts) for t in (u, v, w, phi, p, p_old)]
+        _check(lib.flutas_splitting_rhs(self._h, *ptrs, float(dt), _dev_ptr(rhs_out, self.npts),
+                                        _stream() if stream is None else stream))
+
+    def poisson_solve(self, rhs, p_out, stream=None):
+        _check(lib.flutas_poisson_solve(self._h, _dev_ptr(rhs, self.npts), _dev_ptr(p_out, self.npts),
+                                        _stream() if stream is None else stream))
+
+    # --- introspection
+    @property
+    def workspace_bytes(self):
+        return lib.flutas_plan_workspace_bytes(self._h)
+
+    @property
+    def kernel_names(self):
+        n = lib.flutas_plan_kernel_launches(self._h)
+        return [lib.flutas_plan_kernel_name(self._h, i).decode() for i in range(n)]
+
+    @property
+    def kernel_bytes(self):
+        n = lib.flutas_plan_kernel_launches(self._h)
+        return [lib.flutas_plan_kernel_bytes(self._h, i) for i in range(n)]
+
+    def set_timing(self, enabled):
+        _check(lib.flutas_plan_set_timing(self._h, 1 if enabled else 0))
+
+    def read_timing(self):
+        """returns (list of total ms per kernel, number of steps covered)"""
+        n = lib.flutas_plan_kernel_launches(self._h)
+        ms = (ctypes.c_float * n)()
+        steps = _ci(0)
+        _check(lib.flutas_plan_read_timing(self._h, ms, n, ctypes.byref(steps)))
+        return list(ms), steps.value
+
+    def set_option(self, name, value):
+        _check(lib.flutas_plan_set_option(self._h, name.encode(), int(value)))
+
+
+def _host_ptr(a, npts):
+    import numpy as np
+    try:
+        import torch
+        if isinstance(a, torch.Tensor):
+            if a.is_cuda or a.dtype != torch.float64 or not a.is_contiguous() or a.numel() != npts:
+                raise ValueError("expected a contiguous float64 CPU tensor with nx*ny*nz elements")
+            return a.data_ptr()
+    except ImportError:
+        pass
+    if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags["C_CONTIGUOUS"] and a.size == npts):
+        raise ValueError("expected a C-contiguous float64 numpy array with nx*ny*nz elements")
+    return a.ctypes.data

@@ -1,0 +1,519 @@
+// flutas.cu -- plan, launch sequence and C ABI of libflutas_b200.so (see include/flutas.h).
+//
+// build: nvcc -O3 -std=c++17 -gencode arch=compute_100a,code=sm_100a -lineinfo -Xcompiler -fPIC
+//        -shared (no --use_fast_math: fp64 division / reciprocal stay IEEE)  -- see ../build.py
+#include "flutas.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "kernels.cuh"
+
+using namespace flutas;
+
+// ------------------------------------------------------------------------------------ errors
+static thread_local char g_err[512] = "";
+static thread_local int g_err_code = FLUTAS_OK;
+
+static int fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    g_err_code = code;
+    return code;
+}
+#define CUDA_TRY(expr)                                                                         \
+    do {                                                                                       \
+        cudaError_t e_ = (expr);                                                               \
+        if (e_ != cudaSuccess)                                                                 \
+            return fail(e_ == cudaErrorMemoryAllocation ? FLUTAS_ERR_ALLOC : FLUTAS_ERR_CUDA,  \
+                        "%s: %s", #expr, cudaGetErrorString(e_));                              \
+    } while (0)
+
+extern "C" const char *flutas_last_error(void) { return g_err; }
+extern "C" int flutas_last_error_code(void) { return g_err_code; }
+
+// -------------------------------------------------------------------------------------- plan
+enum KernelId { K_RHS = 0, K_FFTX, K_FFTY, K_Z, K_ZS, K_IFFTY, K_IFFTX, K_CORR, K_MAX };
+
+static const int kMaxPendingSteps = 256;
+
+struct flutas_plan {
+    int nx, ny, nz, bc_z;
+    double lx, ly, lz, rho1, rho2;
+    GridParams grid;
+    int n2, nxh, pitch;          // nx/2, nx/2+1, padded row length of the half-spectrum (multiple of 8)
+    long long npts, nspec;       // nx*ny*nz, pitch*ny*nz
+    // device tables
+    double2 *tw_x, *tw_y, *tw_z;
+    double *lam_x, *lam_y, *lam_z;   // storage (permuted) order
+    // device workspace
+    double2 *spec;
+    double *rhs, *up, *vp, *wp, *cp;
+    size_t bytes;
+    // staging for the host entry point
+    double *stage[6];
+    // launch list
+    int n_launch;
+    int launch_ids[K_MAX];
+    // tuning
+    int y_cols, z_cols;          // tile width (columns of kx) of the strided passes
+    // timing
+    int timing;
+    cudaEvent_t *events;         // kMaxPendingSteps * (n_launch + 1)
+    int pending;
+};
+
+static const char *kKernelNames[K_MAX] = {"splitting_rhs", "fft_x_r2c", "fft_y_fwd", "z_solve", "z_singular",
+                                          "fft_y_inv", "fft_x_c2r", "correction"};
+
+static bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+// storage position -> frequency for the run-time length n (same digit order as fft_core.cuh)
+static int host_freq_of_pos(int n, int pos) {
+    int lg = 0;
+    while ((1 << lg) < n) ++lg;
+    const int P = (lg + 2) / 3, rlast = 1 << (lg - 3 * (P - 1));
+    int k = 0, w = 1, m = n;
+    for (int p = 1; p <= P; ++p) {
+        const int r = p < P ? 8 : rlast;
+        m /= r;
+        k += ((pos / m) % r) * w;
+        w *= r;
+    }
+    return k;
+}
+
+static void host_twiddles(int n, std::vector<double2> &t) {
+    t.resize(n);
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int m = 0; m < n; ++m) {
+        const long double a = -two_pi * (long double)m / (long double)n;
+        t[m] = make_double2((double)cosl(a), (double)sinl(a));
+    }
+}
+// eigenvalue of the periodic second difference, lambda(m) = -2 (1 - cos(2 pi m / n)) / d^2  (R6)
+static double host_lambda(int m, int n, double d) {
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    return (double)(-2.0L * (1.0L - cosl(two_pi * (long double)m / (long double)n))) / (d * d);
+}
+
+template <typename T> static int upload(T **dst, const std::vector<T> &src, size_t *bytes) {
+    CUDA_TRY(cudaMalloc((void **)dst, src.size() * sizeof(T)));
+    CUDA_TRY(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    *bytes += src.size() * sizeof(T);
+    return FLUTAS_OK;
+}
+
+static int plan_build(flutas_plan *pl) {
+    const int nx = pl->nx, ny = pl->ny, nz = pl->nz;
+    const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
+    const double dx = pl->lx / nx, dy = pl->ly / ny, dz = pl->lz / nz;
+    pl->grid = GridParams{nx, ny, nz, wall ? 1 : 0, 1.0 / dx, 1.0 / dy, 1.0 / dz, pl->rho1, pl->rho2,
+                          pl->rho1 < pl->rho2 ? pl->rho1 : pl->rho2};
+    pl->n2 = nx / 2;
+    pl->nxh = nx / 2 + 1;
+    pl->pitch = nx / 2 + 8;
+    pl->npts = (long long)nx * ny * nz;
+    pl->nspec = (long long)pl->pitch * ny * nz;
+
+    std::vector<double2> t;
+    host_twiddles(nx, t);
+    if (int rc = upload(&pl->tw_x, t, &pl->bytes)) return rc;
+    host_twiddles(ny, t);
+    if (int rc = upload(&pl->tw_y, t, &pl->bytes)) return rc;
+    if (!wall) {
+        host_twiddles(nz, t);
+        if (int rc = upload(&pl->tw_z, t, &pl->bytes)) return rc;
+    }
+    std::vector<double> lam(pl->pitch, 1.0);
+    for (int pos = 0; pos < pl->n2; ++pos) lam[pos] = host_lambda(host_freq_of_pos(pl->n2, pos), nx, dx);
+    lam[pl->n2] = host_lambda(pl->n2, nx, dx);
+    if (int rc = upload(&pl->lam_x, lam, &pl->bytes)) return rc;
+    lam.assign(ny, 0.0);
+    for (int pos = 0; pos < ny; ++pos) lam[pos] = host_lambda(host_freq_of_pos(ny, pos), ny, dy);
+    if (int rc = upload(&pl->lam_y, lam, &pl->bytes)) return rc;
+    if (!wall) {
+        lam.assign(nz, 0.0);
+        for (int pos = 0; pos < nz; ++pos) lam[pos] = host_lambda(host_freq_of_pos(nz, pos), nz, dz);
+        if (int rc = upload(&pl->lam_z, lam, &pl->bytes)) return rc;
+    }
+
+    const size_t fb = sizeof(double) * (size_t)pl->npts, sb = sizeof(double2) * (size_t)pl->nspec;
+    CUDA_TRY(cudaMalloc((void **)&pl->spec, sb));
+    CUDA_TRY(cudaMemset(pl->spec, 0, sb));
+    CUDA_TRY(cudaMalloc((void **)&pl->rhs, fb));
+    CUDA_TRY(cudaMalloc((void **)&pl->up, fb));
+    CUDA_TRY(cudaMalloc((void **)&pl->vp, fb));
+    CUDA_TRY(cudaMalloc((void **)&pl->wp, fb));
+    pl->bytes += sb + 4 * fb;
+    if (wall) {
+        CUDA_TRY(cudaMalloc((void **)&pl->cp, sb / 2));
+        pl->bytes += sb / 2;
+    }
+
+    int n = 0;
+    pl->launch_ids[n++] = K_RHS;
+    pl->launch_ids[n++] = K_FFTX;
+    pl->launch_ids[n++] = K_FFTY;
+    pl->launch_ids[n++] = K_Z;
+    if (wall) pl->launch_ids[n++] = K_ZS;
+    pl->launch_ids[n++] = K_IFFTY;
+    pl->launch_ids[n++] = K_IFFTX;
+    pl->launch_ids[n++] = K_CORR;
+    pl->n_launch = n;
+    pl->y_cols = ny >= 2048 ? 4 : 8;
+    pl->z_cols = nz >= 2048 ? 4 : 8;
+    return FLUTAS_OK;
+}
+
+extern "C" flutas_plan *flutas_plan_create(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                                           double rho1, double rho2) {
+    if (bc_z != FLUTAS_BC_Z_PERIODIC && bc_z != FLUTAS_BC_Z_WALL) {
+        fail(FLUTAS_ERR_INVALID_ARG, "bc_z must be FLUTAS_BC_Z_PERIODIC or FLUTAS_BC_Z_WALL");
+        return nullptr;
+    }
+    if (!(lx > 0.0) || !(ly > 0.0) || !(lz > 0.0) || !(rho1 > 0.0) || !(rho2 > 0.0) || !std::isfinite(lx + ly + lz + rho1 + rho2)) {
+        fail(FLUTAS_ERR_INVALID_ARG, "box lengths and densities must be positive and finite");
+        return nullptr;
+    }
+    const bool wall = bc_z == FLUTAS_BC_Z_WALL;
+    if (!is_pow2(nx) || nx < 16 || nx > 2048 || !is_pow2(ny) || ny < 8 || ny > 2048 ||
+        (wall ? (nz < 2) : (!is_pow2(nz) || nz < 8 || nz > 2048))) {
+        fail(FLUTAS_ERR_UNSUPPORTED_SIZE,
+             "unsupported grid %d x %d x %d: nx in [16,2048], ny in [8,2048] powers of two; nz power of two in "
+             "[8,2048] (periodic) or >= 2 (wall)", nx, ny, nz);
+        return nullptr;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        fail(FLUTAS_ERR_CUDA, "no CUDA device available (there is no CPU fallback)");
+        return nullptr;
+    }
+    flutas_plan *pl = new (std::nothrow) flutas_plan();
+    if (!pl) {
+        fail(FLUTAS_ERR_ALLOC, "host allocation failed");
+        return nullptr;
+    }
+    memset(pl, 0, sizeof(*pl));
+    pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->bc_z = bc_z;
+    pl->lx = lx; pl->ly = ly; pl->lz = lz; pl->rho1 = rho1; pl->rho2 = rho2;
+    if (plan_build(pl) != FLUTAS_OK) {
+        flutas_plan_destroy(pl);   // keeps g_err of the failure
+        return nullptr;
+    }
+    return pl;
+}
+
+extern "C" void flutas_plan_destroy(flutas_plan *pl) {
+    if (!pl) return;
+    cudaDeviceSynchronize();
+    cudaFree(pl->tw_x); cudaFree(pl->tw_y); cudaFree(pl->tw_z);
+    cudaFree(pl->lam_x); cudaFree(pl->lam_y); cudaFree(pl->lam_z);
+    cudaFree(pl->spec); cudaFree(pl->rhs); cudaFree(pl->up); cudaFree(pl->vp); cudaFree(pl->wp); cudaFree(pl->cp);
+    for (int i = 0; i < 6; ++i) cudaFree(pl->stage[i]);
+    if (pl->events) {
+        for (int i = 0; i < kMaxPendingSteps * (pl->n_launch + 1); ++i) cudaEventDestroy(pl->events[i]);
+        delete[] pl->events;
+    }
+    cudaGetLastError();
+    delete pl;
+}
+
+extern "C" size_t flutas_plan_workspace_bytes(const flutas_plan *pl) { return pl ? pl->bytes : 0; }
+extern "C" int flutas_plan_kernel_launches(const flutas_plan *pl) { return pl ? pl->n_launch : 0; }
+extern "C" const char *flutas_plan_kernel_name(const flutas_plan *pl, int idx) {
+    if (!pl || idx < 0 || idx >= pl->n_launch) return nullptr;
+    return kKernelNames[pl->launch_ids[idx]];
+}
+
+extern "C" double flutas_plan_kernel_bytes(const flutas_plan *pl, int idx) {
+    if (!pl || idx < 0 || idx >= pl->n_launch) return 0.0;
+    const double f = 8.0 * (double)pl->npts;                    // one real field
+    const double s = 16.0 * (double)pl->nxh * pl->ny * pl->nz;  // the half-spectrum (valid columns)
+    switch (pl->launch_ids[idx]) {
+        case K_RHS: return 6 * f + 4 * f;          // read u*,v*,w*,phi,p,p_old; write rhs,u',v',w'
+        case K_FFTX: return f + s;                 // read rhs, write spectrum
+        case K_FFTY: case K_IFFTY: return 2 * s;   // read + write spectrum
+        case K_Z: return pl->bc_z == FLUTAS_BC_Z_WALL ? 4 * s + 2 * (s / 2) : 2 * s;  // Thomas: two sweeps + c'
+        case K_ZS: return 2.0 * 16.0 * pl->nz;
+        case K_IFFTX: return s + f;                // read spectrum, write p
+        case K_CORR: return 4 * f + 3 * f;         // read p,u',v',w'; write u,v,w
+    }
+    return 0.0;
+}
+
+extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int value) {
+    if (!pl || !name) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan or option name");
+    if (!strcmp(name, "y_cols") && (value == 4 || value == 8)) { pl->y_cols = value; return FLUTAS_OK; }
+    if (!strcmp(name, "z_cols") && (value == 4 || value == 8)) { pl->z_cols = value; return FLUTAS_OK; }
+    return fail(FLUTAS_ERR_INVALID_ARG, "unknown option or value: %s = %d", name, value);
+}
+
+// ---------------------------------------------------------------------------- launch helpers
+template <typename K> static cudaError_t set_smem(K kernel, size_t bytes) {
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+constexpr int clamp_nt(int n) { return n < 32 ? 32 : (n > 256 ? 256 : n); }
+
+template <int N, int C, int MODE> static cudaError_t launch_strided_nc(const StridedArgs &a, int n_outer, cudaStream_t st) {
+    constexpr int NT = clamp_nt(N * C / 8);
+    const size_t smem = sizeof(double2) * (size_t)N * C;
+    auto kern = fft_strided_kernel<N, C, MODE, NT>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<(unsigned)(a.n_tiles_x * n_outer), NT, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <int N, int MODE> static cudaError_t launch_strided_n(int cols, StridedArgs a, int nxh, int n_outer, cudaStream_t st) {
+    a.n_tiles_x = (nxh + cols - 1) / cols;
+    if (cols == 4) return launch_strided_nc<N, 4, MODE>(a, n_outer, st);
+    if constexpr (N >= 2048) return cudaErrorInvalidValue;   // 8 columns of 2048 do not fit in shared memory
+    else return launch_strided_nc<N, 8, MODE>(a, n_outer, st);
+}
+
+template <int MODE> static cudaError_t launch_strided(int n, int cols, const StridedArgs &a, int nxh, int n_outer, cudaStream_t st) {
+    switch (n) {
+        case 8: return launch_strided_n<8, MODE>(cols, a, nxh, n_outer, st);
+        case 16: return launch_strided_n<16, MODE>(cols, a, nxh, n_outer, st);
+        case 32: return launch_strided_n<32, MODE>(cols, a, nxh, n_outer, st);
+        case 64: return launch_strided_n<64, MODE>(cols, a, nxh, n_outer, st);
+        case 128: return launch_strided_n<128, MODE>(cols, a, nxh, n_outer, st);
+        case 256: return launch_strided_n<256, MODE>(cols, a, nxh, n_outer, st);
+        case 512: return launch_strided_n<512, MODE>(cols, a, nxh, n_outer, st);
+        case 1024: return launch_strided_n<1024, MODE>(cols, a, nxh, n_outer, st);
+        case 2048: return launch_strided_n<2048, MODE>(4, a, nxh, n_outer, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <int N2> static cudaError_t launch_r2c_n(const flutas_plan *pl, const double *rhs, cudaStream_t st) {
+    constexpr int NT = clamp_nt(N2);
+    const size_t smem = sizeof(double2) * (size_t)(N2 + 1) * 8;
+    auto kern = fft_x_r2c_kernel<N2, NT>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<(unsigned)((long long)pl->ny * pl->nz / 8), NT, smem, st>>>(rhs, pl->spec, pl->pitch, pl->tw_x);
+    return cudaGetLastError();
+}
+template <int N2> static cudaError_t launch_c2r_n(const flutas_plan *pl, double *out, double scale, cudaStream_t st) {
+    constexpr int NT = clamp_nt(N2);
+    const size_t smem = sizeof(double2) * (size_t)(N2 + 1) * 8;
+    auto kern = fft_x_c2r_kernel<N2, NT>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<(unsigned)((long long)pl->ny * pl->nz / 8), NT, smem, st>>>(pl->spec, out, pl->pitch, pl->tw_x, scale);
+    return cudaGetLastError();
+}
+#define FOR_EACH_N2(X) X(8) X(16) X(32) X(64) X(128) X(256) X(512) X(1024)
+static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStream_t st) {
+    switch (pl->n2) {
+#define X(n) case n: return launch_r2c_n<n>(pl, rhs, st);
+        FOR_EACH_N2(X)
+#undef X
+    }
+    return cudaErrorInvalidValue;
+}
+static cudaError_t launch_c2r(const flutas_plan *pl, double *out, double scale, cudaStream_t st) {
+    switch (pl->n2) {
+#define X(n) case n: return launch_c2r_n<n>(pl, out, scale, st);
+        FOR_EACH_N2(X)
+#undef X
+    }
+    return cudaErrorInvalidValue;
+}
+
+// -------------------------------------------------------------------------- the launch sequence
+struct StepTimer {
+    flutas_plan *pl;
+    cudaStream_t st;
+    cudaEvent_t *ev;
+    int n;
+    StepTimer(flutas_plan *p, cudaStream_t s) : pl(p), st(s), ev(nullptr), n(0) {
+        if (p->timing && p->events) {
+            if (p->pending == kMaxPendingSteps) p->pending = 0;   // drop the oldest batch
+            ev = p->events + (size_t)p->pending * (p->n_launch + 1);
+        }
+    }
+    void mark() { if (ev) cudaEventRecord(ev[n++], st); }
+    void done() { if (ev) pl->pending++; }
+};
+
+static int check_launch(cudaError_t e, const char *what) {
+    if (e != cudaSuccess) return fail(FLUTAS_ERR_CUDA, "launch of %s failed: %s", what, cudaGetErrorString(e));
+    return FLUTAS_OK;
+}
+
+static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
+                       const double *p, const double *po, double dt, double *rhs, cudaStream_t st) {
+    const unsigned nb = (unsigned)((pl->npts + 255) / 256);
+    splitting_rhs_kernel<<<nb, 256, 0, st>>>(pl->grid, dt, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+    return check_launch(cudaGetLastError(), "splitting_rhs");
+}
+
+// spectrum (already holding the x-transformed rhs) -> spectrum of the solution; timer marks between kernels
+static int enqueue_solve_core(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
+    const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
+    StridedArgs ay{};
+    ay.data = pl->spec;
+    ay.row_stride = pl->pitch;
+    ay.outer_stride = (long long)pl->pitch * pl->ny;
+    ay.nxh = pl->nxh;
+    ay.tw = pl->tw_y;
+    if (int rc = check_launch(launch_strided<MODE_FWD>(pl->ny, pl->y_cols, ay, pl->nxh, pl->nz, st), "fft_y_fwd")) return rc;
+    if (tm) tm->mark();
+    if (!wall) {
+        StridedArgs az{};
+        az.data = pl->spec;
+        az.row_stride = (long long)pl->pitch * pl->ny;
+        az.outer_stride = pl->pitch;
+        az.nxh = pl->nxh;
+        az.tw = pl->tw_z;
+        az.lam_x = pl->lam_x;
+        az.lam_outer = pl->lam_y;
+        az.lam_pos = pl->lam_z;
+        if (int rc = check_launch(launch_strided<MODE_SOLVE>(pl->nz, pl->z_cols, az, pl->nxh, pl->ny, st), "z_solve")) return rc;
+        if (tm) tm->mark();
+    } else {
+        const long long ncol = (long long)pl->pitch * pl->ny;
+        const double inv_dz2 = pl->grid.inv_dz * pl->grid.inv_dz;
+        thomas_kernel<<<(unsigned)((ncol + 127) / 128), 128, 0, st>>>(pl->spec, pl->cp, pl->pitch, pl->ny, pl->nz, pl->nxh,
+                                                                    pl->lam_x, pl->lam_y, inv_dz2);
+        if (int rc = check_launch(cudaGetLastError(), "z_solve (thomas)")) return rc;
+        if (tm) tm->mark();
+        const size_t smem = sizeof(double) * 3 * (size_t)pl->nz;
+        if (smem > 200 * 1024) return fail(FLUTAS_ERR_UNSUPPORTED_SIZE, "nz too large for the singular-column kernel");
+        if (set_smem(thomas_singular_kernel, smem) != cudaSuccess) return check_launch(cudaGetLastError(), "z_singular attr");
+        thomas_singular_kernel<<<1, 256, smem, st>>>(pl->spec, ncol, pl->nz, inv_dz2);
+        if (int rc = check_launch(cudaGetLastError(), "z_singular")) return rc;
+        if (tm) tm->mark();
+    }
+    if (int rc = check_launch(launch_strided<MODE_INV>(pl->ny, pl->y_cols, ay, pl->nxh, pl->nz, st), "fft_y_inv")) return rc;
+    if (tm) tm->mark();
+    return FLUTAS_OK;
+}
+
+static double norm_scale(const flutas_plan *pl) {
+    const double n = (double)pl->nx * (double)pl->ny * (pl->bc_z == FLUTAS_BC_Z_WALL ? 1.0 : (double)pl->nz);
+    return 1.0 / n;
+}
+
+static int check_fields(const flutas_plan *pl, const void *const *ptrs, int n) {
+    const size_t fb = sizeof(double) * (size_t)pl->npts;
+    for (int a = 0; a < n; ++a) {
+        if (!ptrs[a]) return fail(FLUTAS_ERR_INVALID_ARG, "NULL field pointer (argument %d)", a);
+        if (((size_t)ptrs[a]) & 15) return fail(FLUTAS_ERR_ALIAS, "field pointer %d is not 16-byte aligned", a);
+    }
+    for (int a = 0; a < n; ++a)
+        for (int b = a + 1; b < n; ++b) {
+            const char *x = (const char *)ptrs[a], *y = (const char *)ptrs[b];
+            if (x < y + fb && y < x + fb) return fail(FLUTAS_ERR_ALIAS, "field arguments %d and %d overlap", a, b);
+        }
+    return FLUTAS_OK;
+}
+
+extern "C" int flutas_projection_step(flutas_plan *pl, double *u, double *v, double *w, const double *phi, double *p,
+                                      const double *p_old, double dt, void *stream) {
+    if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
+    if (!(dt > 0.0) || !std::isfinite(dt)) return fail(FLUTAS_ERR_INVALID_ARG, "dt must be positive and finite");
+    const void *ptrs[6] = {u, v, w, phi, p, p_old};
+    if (int rc = check_fields(pl, ptrs, 6)) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    StepTimer tm(pl, st);
+    tm.mark();
+    if (int rc = enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, pl->rhs, st)) return rc;
+    tm.mark();
+    if (int rc = check_launch(launch_r2c(pl, pl->rhs, st), "fft_x_r2c")) return rc;
+    tm.mark();
+    if (int rc = enqueue_solve_core(pl, st, &tm)) return rc;
+    // p, p_old and phi are dead after the RHS kernel: p^(n+1) goes straight into the caller's p
+    if (int rc = check_launch(launch_c2r(pl, p, norm_scale(pl), st), "fft_x_c2r")) return rc;
+    tm.mark();
+    const unsigned nb = (unsigned)((pl->npts + 255) / 256);
+    correction_kernel<<<nb, 256, 0, st>>>(pl->grid, dt, p, pl->up, pl->vp, pl->wp, u, v, w);
+    if (int rc = check_launch(cudaGetLastError(), "correction")) return rc;
+    tm.mark();
+    tm.done();
+    return FLUTAS_OK;
+}
+
+extern "C" int flutas_splitting_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
+                                    const double *p, const double *p_old, double dt, double *rhs_out, void *stream) {
+    if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
+    if (!(dt > 0.0) || !std::isfinite(dt)) return fail(FLUTAS_ERR_INVALID_ARG, "dt must be positive and finite");
+    const void *ptrs[7] = {u, v, w, phi, p, p_old, rhs_out};
+    if (int rc = check_fields(pl, ptrs, 7)) return rc;
+    return enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, rhs_out, (cudaStream_t)stream);
+}
+
+extern "C" int flutas_poisson_solve(flutas_plan *pl, const double *rhs, double *p_out, void *stream) {
+    if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
+    const void *ptrs[2] = {rhs, p_out};
+    if (rhs == p_out) { if (int rc = check_fields(pl, ptrs, 1)) return rc; }
+    else if (int rc = check_fields(pl, ptrs, 2)) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (int rc = check_launch(launch_r2c(pl, rhs, st), "fft_x_r2c")) return rc;
+    if (int rc = enqueue_solve_core(pl, st, nullptr)) return rc;
+    return check_launch(launch_c2r(pl, p_out, norm_scale(pl), st), "fft_x_c2r");
+}
+
+extern "C" int flutas_projection_step_host(flutas_plan *pl, double *u, double *v, double *w, const double *phi, double *p,
+                                           const double *p_old, double dt, void *stream) {
+    if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
+    const void *src[6] = {u, v, w, phi, p, p_old};
+    for (int i = 0; i < 6; ++i)
+        if (!src[i]) return fail(FLUTAS_ERR_INVALID_ARG, "NULL host pointer (argument %d)", i);
+    const size_t fb = sizeof(double) * (size_t)pl->npts;
+    for (int i = 0; i < 6; ++i)
+        if (!pl->stage[i]) CUDA_TRY(cudaMalloc((void **)&pl->stage[i], fb));
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int i = 0; i < 6; ++i) CUDA_TRY(cudaMemcpyAsync(pl->stage[i], src[i], fb, cudaMemcpyHostToDevice, st));
+    if (int rc = flutas_projection_step(pl, pl->stage[0], pl->stage[1], pl->stage[2], pl->stage[3], pl->stage[4],
+                                        pl->stage[5], dt, stream))
+        return rc;
+    double *dst[4] = {u, v, w, p};
+    const int from[4] = {0, 1, 2, 4};
+    for (int i = 0; i < 4; ++i) CUDA_TRY(cudaMemcpyAsync(dst[i], pl->stage[from[i]], fb, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return FLUTAS_OK;
+}
+
+// -------------------------------------------------------------------------------------- timing
+extern "C" int flutas_plan_set_timing(flutas_plan *pl, int enabled) {
+    if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
+    if (enabled && !pl->events) {
+        const int n = kMaxPendingSteps * (pl->n_launch + 1);
+        pl->events = new (std::nothrow) cudaEvent_t[n];
+        if (!pl->events) return fail(FLUTAS_ERR_ALLOC, "host allocation failed");
+        for (int i = 0; i < n; ++i) CUDA_TRY(cudaEventCreate(&pl->events[i]));
+    }
+    pl->timing = enabled ? 1 : 0;
+    pl->pending = 0;
+    return FLUTAS_OK;
+}
+
+extern "C" int flutas_plan_read_timing(flutas_plan *pl, float *ms_out, int n_out, int *steps_out) {
+    if (!pl || !ms_out || n_out < pl->n_launch) return fail(FLUTAS_ERR_INVALID_ARG, "bad arguments to read_timing");
+    for (int i = 0; i < n_out; ++i) ms_out[i] = 0.0f;
+    const int steps = pl->pending;
+    for (int s = 0; s < steps; ++s) {
+        cudaEvent_t *ev = pl->events + (size_t)s * (pl->n_launch + 1);
+        CUDA_TRY(cudaEventSynchronize(ev[pl->n_launch]));
+        for (int i = 0; i < pl->n_launch; ++i) {
+            float ms = 0.0f;
+            CUDA_TRY(cudaEventElapsedTime(&ms, ev[i], ev[i + 1]));
+            ms_out[i] += ms;
+        }
+    }
+    if (steps_out) *steps_out = steps;
+    pl->pending = 0;
+    return FLUTAS_OK;
+}
