@@ -1,0 +1,295 @@
+#!/usr/bin/env python
+"""bench.py -- fp64 projection-step throughput on synthetic fields shaped like the paper's runs.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workloads cfg4,cfg5]
+
+A "step" is one pass of the whole hot path (splitting RHS -> Poisson solve -> correction) over one
+batch of synthetic input.  Workloads (BASELINE.json `metric` names both):
+  cfg4  512^3 triply periodic, box (2 pi)^3, drops at 5 % volume fraction, rho2/rho1 = 50   [primary line]
+  cfg5  1024 x 1024 x 512 wall-bounded, box 4 x 4 x 1, two-layer, rho2/rho1 = 1000          [under "also"]
+N > 1 (torchrun): N independent replicas, one per GPU, no data-path collective ("replicas only").
+Prints ONE JSON line on rank 0.  --impl reference times the CPU oracle (tests' ground truth) on a
+bounded sample of the same workload; it is a deliberately slow baseline, not a target.
+"""
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 projection-step throughput"
+UNIT = "Mpts/s"
+WORKLOAD_DESC = {
+    "cfg4": "cfg4: 512^3 triply periodic, box (2pi)^3, drops R=16 cells at 5% volume, rho2/rho1=50, dt=1e-3",
+    "cfg5": "cfg5: 1024x1024x512 wall-bounded (Neumann p, Thomas in z), box 4x4x1, two-layer, rho2/rho1=1000, dt=1e-3",
+    "cfg2": "cfg2: 128^3 triply periodic emulsion-shaped (small case)",
+    "cfg3": "cfg3: 256x256x128 wall-bounded two-layer (small case)",
+}
+
+
+def make_workload(name, ratio=None):
+    from paper_2204_08834_b200 import workloads as wl
+    if name == "cfg4":
+        return wl.config4(512, 50.0 if ratio is None else ratio)
+    if name == "cfg5":
+        return wl.config5()
+    if name == "cfg2":
+        return wl.config2()
+    if name == "cfg3":
+        return wl.config3()
+    raise ValueError(name)
+
+
+def load_peak():
+    """(HBM GB/s, label): the driver-measured copy bandwidth, else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def load_ncu_traffic():
+    """per-launch DRAM bytes from the committed ncu capture (profiles/ncu_traffic.json), if present"""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
+class ClockSampler(threading.Thread):
+    """samples SM clock and throttle reasons through NVML while the timed region runs"""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.mask, self.max_mhz, self.stop_flag = index, [], 0, None, False
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            pass
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        getr = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or nv.nvmlDeviceGetCurrentClocksThrottleReasons
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.mask |= int(getr(self.h))
+            except Exception:
+                pass
+            time.sleep(0.004)
+
+    def result(self):
+        self.stop_flag = True
+        if self.is_alive():
+            self.join(timeout=2)
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz, "samples": len(self.samples),
+                "reasons": sorted(v for k, v in self.REASONS.items() if self.mask & k)}
+
+
+def visible_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+# ------------------------------------------------------------------------------------- our arm
+def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, with_e2e, traffic):
+    import torch
+    import paper_2204_08834_b200 as fl
+    from paper_2204_08834_b200 import replicas
+
+    ratio = replicas.replica_density_ratio(rank) if (name == "cfg4" and world > 1) else None
+    t0 = time.time()
+    W = make_workload(name, ratio)
+    gen_s = time.time() - t0
+    plan = fl.Plan(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2)
+    host = list(W.fields())
+    dev = [torch.from_numpy(a).cuda() for a in host]
+    torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        plan.projection_step(*dev, W.dt)
+    torch.cuda.synchronize()
+    plan.set_timing(True)
+    sampler = ClockSampler(visible_gpu_index(local_rank))
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    replicas.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    ev0.record()
+    for _ in range(args.steps):
+        plan.projection_step(*dev, W.dt)
+    ev1.record()
+    torch.cuda.synchronize()
+    replicas.barrier()
+    clocks = sampler.result()
+    ms_local = ev0.elapsed_time(ev1)
+    kms, ksteps = plan.read_timing()
+    plan.set_timing(False)
+    finite = bool(torch.isfinite(dev[4]).all().item() and torch.isfinite(dev[0]).all().item())
+    units, ms = replicas.aggregate_throughput(float(W.npts) * args.steps, ms_local)
+
+    names, kbytes = plan.kernel_names, plan.kernel_bytes
+    kernels = []
+    for n_, b_, t_ in zip(names, kbytes, kms):
+        avg = t_ / max(ksteps, 1)
+        kernels.append({"name": n_, "ms": round(avg, 4), "alg_bytes": b_, "gbs": round(b_ / (avg * 1e-3) / 1e9, 1) if avg > 0 else None,
+                        "frac": round(b_ / (avg * 1e-3) / 1e9 / peak_gbs, 4) if avg > 0 else None})
+    dom = max(kernels, key=lambda k: k["ms"])
+    tr = traffic.get(name, {}).get(dom["name"])
+    roofline = {"bound": "hbm", "kernel": dom["name"], "achieved": dom["gbs"], "peak": peak_gbs, "unit": "GB/s",
+                "frac": dom["frac"], "traffic": tr, "peak_source": peak_label,
+                "alg_bytes_per_launch": dom["alg_bytes"], "kernel_ms": dom["ms"]}
+    step_ms = ms_local / args.steps
+    model_bytes = sum(kbytes)
+    step = {"ms": round(step_ms, 4), "model_bytes_per_pt": round(model_bytes / W.npts, 1), "min_bytes_per_pt": 80,
+            "model_gbs": round(model_bytes / (step_ms * 1e-3) / 1e9, 1),
+            "frac_of_peak_model_bytes": round(model_bytes / (step_ms * 1e-3) / 1e9 / peak_gbs, 4),
+            "frac_of_peak_min_bytes": round(80.0 * W.npts / (step_ms * 1e-3) / 1e9 / peak_gbs, 4),
+            "frac_of_8TBs_model_bytes": round(model_bytes / (step_ms * 1e-3) / 1e9 / 8000.0, 4)}
+
+    out = {
+        "metric": METRIC, "value": round(units / (ms * 1e-3) / 1e6, 1), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms / args.steps, 4),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD_DESC[name], "grid": [W.nx, W.ny, W.nz], "bc_z": "wall" if W.bc_z else "periodic",
+                   "rho2_over_rho1": W.rho2 / W.rho1, "parallelism": f"replicas x{world} (no data-path collective)",
+                   "l2": "inputs larger than L2 (6 fields of %.1f GiB each); steps run back to back in place" % (W.npts * 8 / 2**30),
+                   "input_generation_s": round(gen_s, 1)},
+        "clocks": clocks, "gpu_launches": args.steps * len(names), "launches_per_step": len(names),
+        "roofline": roofline, "step": step, "kernels": kernels, "finite": finite,
+        "workspace_gib": round(plan.workspace_bytes / 2**30, 2),
+    }
+
+    if with_e2e:
+        # end to end through the host entry point of the C ABI: pinned host buffers, H2D of the six inputs
+        # and D2H of u, v, w, p inside the timed region, every step
+        e_steps = max(1, min(args.steps, args.e2e_steps))
+        pinned = [torch.from_numpy(a).pin_memory() for a in host]
+        plan.projection_step_host(*pinned, W.dt)            # warm-up (allocates the staging buffers)
+        replicas.barrier()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(e_steps):
+            plan.projection_step_host(*pinned, W.dt)
+        e1.record()
+        torch.cuda.synchronize()
+        replicas.barrier()
+        eu, ems = replicas.aggregate_throughput(float(W.npts) * e_steps, e0.elapsed_time(e1))
+        out["e2e"] = {"value": round(eu / (ems * 1e-3) / 1e6, 1), "unit": UNIT, "h2d_bytes_per_step": 6 * W.npts * 8,
+                      "d2h_bytes_per_step": 4 * W.npts * 8, "steps": e_steps, "ms_per_step": round(ems / e_steps, 2),
+                      "api": "flutas_projection_step_host (pinned host buffers)"}
+        del pinned
+    plan.destroy()
+    del dev
+    torch.cuda.empty_cache()
+    return out
+
+
+def oracle_sample(threads=0):
+    """time the CPU oracle, as it stands, on a bounded sample of the primary workload: a 256^3 box of the cfg4
+    recipe (same drop radius in cells, same volume fraction, |k| <= 16)"""
+    import oracle
+    from paper_2204_08834_b200 import workloads as wl
+    W = wl.config4(256, 50.0, 16, 0.05, 16)
+    t0 = time.perf_counter()
+    oracle.projection_step(*W.fields(), W.box, W.bc_z, W.rho1, W.rho2, W.dt, nthreads=threads)
+    dt = time.perf_counter() - t0
+    return {"value": round(W.npts / dt / 1e6, 3), "unit": UNIT, "cores": oracle.threads(threads), "kind": "oracle",
+            "sample": "one step of a 256^3 box of the cfg4 recipe (1/8 of the grid points; naive O(n^2) DFT per line)",
+            "seconds": round(dt, 2)}
+
+
+def run_ours(args):
+    import torch
+    from paper_2204_08834_b200 import replicas
+    rank, local_rank, world = replicas.init_from_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    peak_gbs, peak_label = load_peak()
+    traffic = load_ncu_traffic()
+    names = [w for w in args.workloads.split(",") if w]
+    results = [bench_workload(n, args, rank, local_rank, world, peak_gbs, peak_label, with_e2e=(i == 0 or args.e2e_all),
+                              traffic=traffic) for i, n in enumerate(names)]
+    out = results[0]
+    if len(results) > 1:
+        out["also"] = results[1:]
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            out["cpu_baseline"] = oracle_sample()
+        print(json.dumps(out), flush=True)
+    replicas.barrier()
+
+
+# ------------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    t_all = time.perf_counter()
+    samples = []
+    for _ in range(args.warmup if args.warmup < 2 else 1):
+        oracle_sample()
+    for _ in range(max(1, min(args.steps, 3))):
+        samples.append(oracle_sample())
+    best = max(samples, key=lambda s: s["value"])
+    val = statistics.median(s["value"] for s in samples)
+    npts = 256 ** 3
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": len(samples),
+           "warmup": min(args.warmup, 1), "ms_per_step": round(npts / (val * 1e6) * 1e3, 1), "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": WORKLOAD_DESC["cfg4"], "sample": best["sample"]},
+           "cpu_baseline": dict(best, value=val),
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0, "wall_s": round(time.perf_counter() - t_all, 1)}
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workloads", default="cfg4,cfg5")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-all", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        if args.warmup < 3:
+            args.warmup = 3
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
