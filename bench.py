@@ -128,6 +128,9 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     W = make_workload(name, ratio)
     gen_s = time.time() - t0
     plan = fl.Plan(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2)
+    for kv in (args.opt or []):                       # experiments only: plan tuning knobs
+        k_, v_ = kv.split("=")
+        plan.set_option(k_, int(v_))
     host = list(W.fields())
     dev = [torch.from_numpy(a).cuda() for a in host]
     torch.cuda.synchronize()
@@ -282,6 +285,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-all", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", help="plan tuning knob name=value (experiments)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -62,6 +62,7 @@ struct flutas_plan {
     int launch_ids[K_MAX];
     // tuning
     int y_cols, z_cols;          // tile width (columns of kx) of the strided passes
+    int rhs_kc;                  // planes one thread of the RHS kernel marches through
     // timing
     int timing;
     cudaEvent_t *events;         // kMaxPendingSteps * (n_launch + 1)
@@ -168,6 +169,7 @@ static int plan_build(flutas_plan *pl) {
     pl->n_launch = n;
     pl->y_cols = ny >= 2048 ? 4 : 8;
     pl->z_cols = nz >= 2048 ? 4 : 8;
+    pl->rhs_kc = 32;
     return FLUTAS_OK;
 }
 
@@ -252,6 +254,7 @@ extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int val
     if (!pl || !name) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan or option name");
     if (!strcmp(name, "y_cols") && (value == 4 || value == 8)) { pl->y_cols = value; return FLUTAS_OK; }
     if (!strcmp(name, "z_cols") && (value == 4 || value == 8)) { pl->z_cols = value; return FLUTAS_OK; }
+    if (!strcmp(name, "rhs_kc") && value >= 1) { pl->rhs_kc = value; return FLUTAS_OK; }
     return fail(FLUTAS_ERR_INVALID_ARG, "unknown option or value: %s = %d", name, value);
 }
 
@@ -301,7 +304,7 @@ template <int N2> static cudaError_t launch_r2c_n(const flutas_plan *pl, const d
     auto kern = fft_x_r2c_kernel<N2, NT>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
-    kern<<<(unsigned)((long long)pl->ny * pl->nz / 8), NT, smem, st>>>(rhs, pl->spec, pl->pitch, pl->tw_x);
+    kern<<<(unsigned)((long long)pl->ny * pl->nz / 8), NT, smem, st>>>(rhs, pl->spec, pl->tw_x);
     return cudaGetLastError();
 }
 template <int N2> static cudaError_t launch_c2r_n(const flutas_plan *pl, double *out, double scale, cudaStream_t st) {
@@ -310,7 +313,7 @@ template <int N2> static cudaError_t launch_c2r_n(const flutas_plan *pl, double 
     auto kern = fft_x_c2r_kernel<N2, NT>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
-    kern<<<(unsigned)((long long)pl->ny * pl->nz / 8), NT, smem, st>>>(pl->spec, out, pl->pitch, pl->tw_x, scale);
+    kern<<<(unsigned)((long long)pl->ny * pl->nz / 8), NT, smem, st>>>(pl->spec, out, pl->tw_x, scale);
     return cudaGetLastError();
 }
 #define FOR_EACH_N2(X) X(8) X(16) X(32) X(64) X(128) X(256) X(512) X(1024)
@@ -354,8 +357,13 @@ static int check_launch(cudaError_t e, const char *what) {
 
 static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
                        const double *p, const double *po, double dt, double *rhs, cudaStream_t st) {
-    const unsigned nb = (unsigned)((pl->npts + 255) / 256);
-    splitting_rhs_kernel<<<nb, 256, 0, st>>>(pl->grid, dt, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+    // block = (bx threads x 2 points) x ty rows; nx/2 and ny are powers of two, so the grid divides evenly
+    const int bx = pl->nx / 2 < 64 ? pl->nx / 2 : 64;
+    int ty = 256 / bx;
+    if (ty > pl->ny) ty = pl->ny;
+    const int kc = pl->rhs_kc < pl->nz ? pl->rhs_kc : pl->nz;
+    dim3 block(bx, ty), grid(pl->nx / 2 / bx, pl->ny / ty, (pl->nz + kc - 1) / kc);
+    splitting_rhs_kernel<<<grid, block, 0, st>>>(pl->grid, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
     return check_launch(cudaGetLastError(), "splitting_rhs");
 }
 

@@ -25,60 +25,128 @@ struct GridParams {
 };
 
 // ------------------------------------------------------------------------------------------------
-// a1-a3: fused density + splitting right-hand side (eqs. 2, 16, 17)
-// One thread per grid point.  Reads u*, v*, w*, phi, p, p_old; writes rhs and u', v', w'.
+// a1-a3: fused density + splitting right-hand side (eqs. 2, 16, 17).
+// Reads u*, v*, w*, phi, p, p_old once; writes rhs and the half-corrected velocity u', v', w'.
+//
+// 2.5-D register-marching stencil: a block is (bx threads along x, 2 points each) x (ty rows of j); each
+// thread marches over `kc` planes in z carrying, in registers, the centre and top values of rho_c and p_hat,
+// the bottom-face flux (= the previous plane's top-face flux) and w below.  x neighbours come from warp
+// shuffles (edge lanes load them), y neighbours from L1/L2 (the rows were loaded one iteration earlier by
+// the neighbouring threads).  Per point: 4 reciprocals, no integer division, 32-bit index arithmetic.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
-splitting_rhs_kernel(GridParams g, double dt, const double *__restrict__ u, const double *__restrict__ v,
+struct Flux { double f, r; };   // f = (1 - rho0/rho_f) * g,  r = 1/rho_f
+__device__ __forceinline__ Flux face_flux(double rc_a, double rc_b, double g, double rho0) {
+    Flux o;
+    o.r = 1.0 / (0.5 * (rc_a + rc_b));
+    o.f = (1.0 - rho0 * o.r) * g;
+    return o;
+}
+
+__global__ void __launch_bounds__(256, 2)
+splitting_rhs_kernel(GridParams g, double dt, int kc, const double *__restrict__ u, const double *__restrict__ v,
                      const double *__restrict__ w, const double *__restrict__ phi,
                      const double *__restrict__ p, const double *__restrict__ po,
                      double *__restrict__ rhs, double *__restrict__ up, double *__restrict__ vp,
                      double *__restrict__ wp) {
-    const long long n = (long long)g.nx * g.ny * g.nz;
-    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= n) return;
-    const int i = (int)(q % g.nx);
-    const long long r = q / g.nx;
-    const int j = (int)(r % g.ny), k = (int)(r / g.ny);
-    const long long sx = 1, sy = g.nx, sz = (long long)g.nx * g.ny;
-    const long long qip = (i + 1 == g.nx) ? q - (g.nx - 1) * sx : q + sx;
-    const long long qim = (i == 0) ? q + (g.nx - 1) * sx : q - sx;
-    const long long qjp = (j + 1 == g.ny) ? q - (g.ny - 1) * sy : q + sy;
-    const long long qjm = (j == 0) ? q + (g.ny - 1) * sy : q - sy;
-    const long long qkp = (k + 1 == g.nz) ? q - (g.nz - 1) * sz : q + sz;
-    const long long qkm = (k == 0) ? q + (g.nz - 1) * sz : q - sz;
-    const bool top = g.wall && (k + 1 == g.nz), bot = g.wall && (k == 0);
+    const int nx = g.nx, ny = g.ny, nz = g.nz;
+    const int i0 = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(k0 + kc, nz);
+    const int jn = (j + 1 == ny) ? 0 : j + 1, js = (j == 0) ? ny - 1 : j - 1;
+    const int iw = (i0 == 0) ? nx - 1 : i0 - 1, ie = (i0 + 2 == nx) ? 0 : i0 + 2;
+    // shuffle neighbourhood: a "row" of lanes is min(32, blockDim.x) wide
+    const int lane = (threadIdx.x + threadIdx.y * blockDim.x) & 31;
+    const int rw = blockDim.x < 32 ? blockDim.x : 32;
+    const bool edge_l = (lane % rw) == 0, edge_r = (lane % rw) == rw - 1;
+    const long long plane = (long long)nx * ny;
+    const long long col = (long long)j * nx + i0, col_n = (long long)jn * nx + i0, col_s = (long long)js * nx + i0;
+    const long long row_j = (long long)j * nx;
+    const double rho1 = g.rho1, rho2 = g.rho2, rho0 = g.rho0, inv_rho0 = 1.0 / g.rho0;
+    const double c_div = g.rho0 / dt;
 
-    auto rho_c = [&](long long a) { const double f = phi[a]; return g.rho1 * f + g.rho2 * (1.0 - f); };
-    auto p_hat = [&](long long a) { return 2.0 * p[a] - po[a]; };
+    auto ld2 = [](const double *f, long long q) { return *reinterpret_cast<const double2 *>(f + q); };
+    auto rho_of = [&](double f) { return rho1 * f + rho2 * (1.0 - f); };
+    auto rho2_of = [&](double2 f) { return make_double2(rho_of(f.x), rho_of(f.y)); };
+    auto phat2 = [&](double2 a, double2 b) { return make_double2(2.0 * a.x - b.x, 2.0 * a.y - b.y); };
 
-    const double rc = rho_c(q), ph = p_hat(q);
-    // east / west faces
-    const double r_e = 1.0 / (0.5 * (rc + rho_c(qip))), r_w = 1.0 / (0.5 * (rc + rho_c(qim)));
-    const double g_e = (p_hat(qip) - ph) * g.inv_dx, g_w = (ph - p_hat(qim)) * g.inv_dx;
-    // north / south
-    const double r_n = 1.0 / (0.5 * (rc + rho_c(qjp))), r_s = 1.0 / (0.5 * (rc + rho_c(qjm)));
-    const double g_n = (p_hat(qjp) - ph) * g.inv_dy, g_s = (ph - p_hat(qjm)) * g.inv_dy;
-    // top / bottom (wall faces carry zero flux)
-    const double r_t = top ? 0.0 : 1.0 / (0.5 * (rc + rho_c(qkp)));
-    const double r_b = bot ? 0.0 : 1.0 / (0.5 * (rc + rho_c(qkm)));
-    const double g_t = top ? 0.0 : (p_hat(qkp) - ph) * g.inv_dz;
-    const double g_b = bot ? 0.0 : (ph - p_hat(qkm)) * g.inv_dz;
+    // prologue: centre plane k0, bottom flux and w below
+    long long qk = (long long)k0 * plane;
+    double2 rc_c = rho2_of(ld2(phi, qk + col)), ph_c = phat2(ld2(p, qk + col), ld2(po, qk + col));
+    double2 fb = make_double2(0.0, 0.0), wb = make_double2(0.0, 0.0);
+    if (!(g.wall && k0 == 0)) {
+        const long long qb = (long long)((k0 == 0) ? nz - 1 : k0 - 1) * plane + col;
+        const double2 rc_b = rho2_of(ld2(phi, qb)), ph_b = phat2(ld2(p, qb), ld2(po, qb));
+        fb.x = face_flux(rc_b.x, rc_c.x, (ph_c.x - ph_b.x) * g.inv_dz, rho0).f;
+        fb.y = face_flux(rc_b.y, rc_c.y, (ph_c.y - ph_b.y) * g.inv_dz, rho0).f;
+        wb = ld2(w, qb);
+    }
 
-    const double f_e = (1.0 - g.rho0 * r_e) * g_e, f_w = (1.0 - g.rho0 * r_w) * g_w;
-    const double f_n = (1.0 - g.rho0 * r_n) * g_n, f_s = (1.0 - g.rho0 * r_s) * g_s;
-    const double f_t = (1.0 - g.rho0 * r_t) * g_t, f_b = (1.0 - g.rho0 * r_b) * g_b;
+    for (int k = k0; k < k1; ++k, qk += plane) {
+        const bool top = g.wall && (k + 1 == nz);
+        // next plane (becomes the centre of the next iteration)
+        double2 rc_t = rc_c, ph_t = ph_c;
+        if (!top) {
+            const long long qt = (long long)((k + 1 == nz) ? 0 : k + 1) * plane + col;
+            rc_t = rho2_of(ld2(phi, qt));
+            ph_t = phat2(ld2(p, qt), ld2(po, qt));
+        }
+        // y neighbours of the centre plane
+        const double2 rc_n = rho2_of(ld2(phi, qk + col_n)), ph_n = phat2(ld2(p, qk + col_n), ld2(po, qk + col_n));
+        const double2 rc_s = rho2_of(ld2(phi, qk + col_s)), ph_s = phat2(ld2(p, qk + col_s), ld2(po, qk + col_s));
+        const double2 uc = ld2(u, qk + col), vc = ld2(v, qk + col), wc = ld2(w, qk + col), vs = ld2(v, qk + col_s);
 
-    const double uc = u[q], vc = v[q], wc = w[q];
-    const double um = u[qim], vm = v[qjm], wm = bot ? 0.0 : w[qkm];
-    const double div_u = (uc - um) * g.inv_dx + (vc - vm) * g.inv_dy + (wc - wm) * g.inv_dz;
-    const double div_f = (f_e - f_w) * g.inv_dx + (f_n - f_s) * g.inv_dy + (f_t - f_b) * g.inv_dz;
-    rhs[q] = g.rho0 / dt * div_u + div_f;
+        // x faces: m between (i0, i0+1), e between (i0+1, i0+2), wf between (i0-1, i0)
+        double rc_e = __shfl_down_sync(0xffffffffu, rc_c.x, 1), ph_e = __shfl_down_sync(0xffffffffu, ph_c.x, 1);
+        if (edge_r) {
+            const long long qe = qk + row_j + ie;
+            rc_e = rho_of(phi[qe]);
+            ph_e = 2.0 * p[qe] - po[qe];
+        }
+        const Flux fm = face_flux(rc_c.x, rc_c.y, (ph_c.y - ph_c.x) * g.inv_dx, rho0);
+        const Flux fe = face_flux(rc_c.y, rc_e, (ph_e - ph_c.y) * g.inv_dx, rho0);
+        double f_w = __shfl_up_sync(0xffffffffu, fe.f, 1), u_w = __shfl_up_sync(0xffffffffu, uc.y, 1);
+        if (edge_l) {
+            const long long qw = qk + row_j + iw;
+            f_w = face_flux(rho_of(phi[qw]), rc_c.x, (ph_c.x - (2.0 * p[qw] - po[qw])) * g.inv_dx, rho0).f;
+            u_w = u[qw];
+        }
+        // y faces
+        const Flux fn0 = face_flux(rc_c.x, rc_n.x, (ph_n.x - ph_c.x) * g.inv_dy, rho0);
+        const Flux fn1 = face_flux(rc_c.y, rc_n.y, (ph_n.y - ph_c.y) * g.inv_dy, rho0);
+        const double fs0 = face_flux(rc_s.x, rc_c.x, (ph_c.x - ph_s.x) * g.inv_dy, rho0).f;
+        const double fs1 = face_flux(rc_s.y, rc_c.y, (ph_c.y - ph_s.y) * g.inv_dy, rho0).f;
+        // z faces (wall faces carry zero flux)
+        Flux ft0{0.0, 0.0}, ft1{0.0, 0.0};
+        double gz0 = 0.0, gz1 = 0.0;
+        if (!top) {
+            gz0 = (ph_t.x - ph_c.x) * g.inv_dz;
+            gz1 = (ph_t.y - ph_c.y) * g.inv_dz;
+            ft0 = face_flux(rc_c.x, rc_t.x, gz0, rho0);
+            ft1 = face_flux(rc_c.y, rc_t.y, gz1, rho0);
+        }
 
-    const double inv_rho0 = 1.0 / g.rho0;
-    up[q] = uc - dt * ((r_e - inv_rho0) * g_e);
-    vp[q] = vc - dt * ((r_n - inv_rho0) * g_n);
-    wp[q] = top ? wc : wc - dt * ((r_t - inv_rho0) * g_t);
+        double2 out;
+        out.x = c_div * ((uc.x - u_w) * g.inv_dx + (vc.x - vs.x) * g.inv_dy + (wc.x - wb.x) * g.inv_dz) +
+                ((fm.f - f_w) * g.inv_dx + (fn0.f - fs0) * g.inv_dy + (ft0.f - fb.x) * g.inv_dz);
+        out.y = c_div * ((uc.y - uc.x) * g.inv_dx + (vc.y - vs.y) * g.inv_dy + (wc.y - wb.y) * g.inv_dz) +
+                ((fe.f - fm.f) * g.inv_dx + (fn1.f - fs1) * g.inv_dy + (ft1.f - fb.y) * g.inv_dz);
+        *reinterpret_cast<double2 *>(rhs + qk + col) = out;
+
+        out.x = uc.x - dt * ((fm.r - inv_rho0) * ((ph_c.y - ph_c.x) * g.inv_dx));
+        out.y = uc.y - dt * ((fe.r - inv_rho0) * ((ph_e - ph_c.y) * g.inv_dx));
+        *reinterpret_cast<double2 *>(up + qk + col) = out;
+        out.x = vc.x - dt * ((fn0.r - inv_rho0) * ((ph_n.x - ph_c.x) * g.inv_dy));
+        out.y = vc.y - dt * ((fn1.r - inv_rho0) * ((ph_n.y - ph_c.y) * g.inv_dy));
+        *reinterpret_cast<double2 *>(vp + qk + col) = out;
+        out.x = top ? wc.x : wc.x - dt * ((ft0.r - inv_rho0) * gz0);
+        out.y = top ? wc.y : wc.y - dt * ((ft1.r - inv_rho0) * gz1);
+        *reinterpret_cast<double2 *>(wp + qk + col) = out;
+
+        fb = make_double2(ft0.f, ft1.f);
+        wb = wc;
+        rc_c = rc_t;
+        ph_c = ph_t;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -149,40 +217,69 @@ struct StridedArgs {
     const double *lam_x, *lam_outer, *lam_pos;
 };
 
+// The first pass reads its 8 elements straight from global memory into registers and the last pass
+// writes them straight back (the permuted order makes every pass in place), so shared memory is only
+// the exchange buffer between passes: P-1 exchanges, P-1 barriers, no staging copies.
 template <int N, int C, int MODE, int NT>
-__global__ void __launch_bounds__(NT) fft_strided_kernel(StridedArgs a) {
+__global__ void __launch_bounds__(NT, (N * C * 16 <= 72 * 1024 && NT == 256) ? 3 : 1) fft_strided_kernel(StridedArgs a) {
     extern __shared__ double2 smem[];
     double2 *s = smem;
+    constexpr int P = Fact<N>::P;
     const int tid = threadIdx.x;
     const int tx = blockIdx.x % a.n_tiles_x, outer = blockIdx.x / a.n_tiles_x;
     const int l = tid % C;
     const int kx = tx * C + l;
     const bool valid = kx < a.nxh;
     double2 *gp = a.data + (long long)outer * a.outer_stride + kx;
+    const long long rs = a.row_stride;
 
-#pragma unroll 8
-    for (int r = tid / C; r < N; r += NT / C)
-        s[r * C + l] = valid ? gp[(long long)r * a.row_stride] : make_double2(0.0, 0.0);
-    __syncthreads();
+    auto load8 = [&](bool from_global, const int *pos, double2 *v) {
+        if (from_global) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) v[e] = valid ? gp[(long long)pos[e] * rs] : make_double2(0.0, 0.0);
+        } else {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) v[e] = s[pos[e] * C + l];
+        }
+    };
+    auto store8 = [&](bool to_global, const int *pos, const double2 *v) {
+        if (to_global) {
+            if (valid) {
+#pragma unroll
+                for (int e = 0; e < 8; ++e) gp[(long long)pos[e] * rs] = v[e];
+            }
+        } else {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) s[pos[e] * C + l] = v[e];
+        }
+    };
 
-    if (MODE == MODE_FWD) {
-        tile_fft<N, C, false, NT, -1>(s, a.tw, 1, tid);
-    } else if (MODE == MODE_INV) {
-        tile_fft<N, C, false, NT, +1>(s, a.tw, 1, tid);
+    if (MODE == MODE_FWD || MODE == MODE_INV) {
+#pragma unroll
+        for (int pp = 0; pp < P; ++pp) {
+            const int p = (MODE == MODE_FWD) ? pp + 1 : P - pp;
+            for (int t = tid / C; t < N / 8; t += NT / C) {
+                int pos[8], n2;
+                double2 v[8];
+                pass_positions<N>(p, t, pos, n2);
+                load8(pp == 0, pos, v);
+                if (MODE == MODE_FWD) fwd_pass_regs<N>(p, n2, v, a.tw, 1);
+                else inv_pass_regs<N>(p, n2, v, a.tw, 1);
+                store8(pp == P - 1, pos, v);
+            }
+            if (pp + 1 < P) __syncthreads();
+        }
     } else {
-        // forward passes 1..P-1 through shared memory
-        constexpr int P = Fact<N>::P;
+        // forward passes 1..P-1
 #pragma unroll
         for (int p = 1; p < P; ++p) {
             for (int t = tid / C; t < N / 8; t += NT / C) {
                 int pos[8], n2;
                 double2 v[8];
                 pass_positions<N>(p, t, pos, n2);
-#pragma unroll
-                for (int e = 0; e < 8; ++e) v[e] = s[pos[e] * C + l];
+                load8(p == 1, pos, v);
                 fwd_pass_regs<N>(p, n2, v, a.tw, 1);
-#pragma unroll
-                for (int e = 0; e < 8; ++e) s[pos[e] * C + l] = v[e];
+                store8(false, pos, v);
             }
             __syncthreads();
         }
@@ -192,8 +289,7 @@ __global__ void __launch_bounds__(NT) fft_strided_kernel(StridedArgs a) {
             int pos[8], n2;
             double2 v[8];
             pass_positions<N>(P, t, pos, n2);
-#pragma unroll
-            for (int e = 0; e < 8; ++e) v[e] = s[pos[e] * C + l];
+            load8(P == 1, pos, v);
             fwd_pass_regs<N>(P, n2, v, a.tw, 1);
 #pragma unroll
             for (int e = 0; e < 8; ++e) {
@@ -202,59 +298,71 @@ __global__ void __launch_bounds__(NT) fft_strided_kernel(StridedArgs a) {
                 v[e] = cscale(v[e], inv);
             }
             inv_pass_regs<N>(P, n2, v, a.tw, 1);
-#pragma unroll
-            for (int e = 0; e < 8; ++e) s[pos[e] * C + l] = v[e];
+            store8(P == 1, pos, v);
         }
-        if (P > 1) __syncthreads();
 #pragma unroll
         for (int p = P - 1; p >= 1; --p) {
+            __syncthreads();
             for (int t = tid / C; t < N / 8; t += NT / C) {
                 int pos[8], n2;
                 double2 v[8];
                 pass_positions<N>(p, t, pos, n2);
-#pragma unroll
-                for (int e = 0; e < 8; ++e) v[e] = s[pos[e] * C + l];
+                load8(false, pos, v);
                 inv_pass_regs<N>(p, n2, v, a.tw, 1);
-#pragma unroll
-                for (int e = 0; e < 8; ++e) s[pos[e] * C + l] = v[e];
+                store8(p == 1, pos, v);
             }
-            if (p > 1) __syncthreads();
         }
     }
-    __syncthreads();
+}
 
-    if (valid) {
-#pragma unroll 8
-        for (int r = tid / C; r < N; r += NT / C) gp[(long long)r * a.row_stride] = s[r * C + l];
+// ------------------------------------------------------------------------------------------------
+// Cooperative copy of TOT contiguous elements with B loads in flight per thread: all loads of a batch are
+// issued before the first use, so a CTA pays one memory latency per batch instead of one per element.
+// ------------------------------------------------------------------------------------------------
+template <int TOT, int NT, int B, typename T, typename Load, typename Store>
+__device__ __forceinline__ void batched_copy(int tid, Load load, Store store) {
+    for (int base = 0; base < TOT; base += NT * B) {
+        T vals[B];
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const int idx = base + b * NT + tid;
+            if (idx < TOT) vals[b] = load(idx);
+        }
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const int idx = base + b * NT + tid;
+            if (idx < TOT) store(idx, vals[b]);
+        }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
 // a4: real-to-complex along x.  CTA = 8 consecutive lines (contiguous in memory), N2 = nx/2.
-// Output row (line) layout: positions 0..N2-1 in permuted order, Nyquist at N2; row pitch `pitch`.
+// Output row (line) layout: positions 0..N2-1 in permuted order, Nyquist at N2; row pitch = N2 + 8,
+// so the 8 output rows of a CTA are one contiguous block as well.
 // ------------------------------------------------------------------------------------------------
 template <int N2, int NT>
-__global__ void __launch_bounds__(NT)
-fft_x_r2c_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec, int pitch,
+__global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1)
+fft_x_r2c_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec,
                  const double2 *__restrict__ tw /* e^{-2 pi i m / nx} */) {
     extern __shared__ double2 smem[];
     double2 *s = smem;
+    constexpr int PITCH = N2 + 8;
     const int tid = threadIdx.x;
     const long long line0 = (long long)blockIdx.x * 8;
     const double2 *src = reinterpret_cast<const double2 *>(rhs) + line0 * N2;
-#pragma unroll 4
-    for (int idx = tid; idx < 8 * N2; idx += NT) {
-        const int l = idx / N2, i = idx % N2;
-        s[tile_index<8, true>(i, l)] = src[idx];
-    }
+    batched_copy<8 * N2, NT, 8, double2>(
+        tid, [&](int idx) { return src[idx]; },
+        [&](int idx, double2 val) { s[tile_index<8, true>(idx % N2, idx / N2)] = val; });
     __syncthreads();
     tile_fft<N2, 8, true, NT, -1>(s, tw, 2, tid);
     __syncthreads();
     for (int item = tid; item < 8 * (N2 / 2 + 1); item += NT) r2c_post_item<N2, 8, true>(s, item / 8, item % 8, tw);
     __syncthreads();
-    for (int l = 0; l < 8; ++l) {
-        double2 *dst = spec + (line0 + l) * pitch;
-        for (int pos = tid; pos <= N2; pos += NT) dst[pos] = s[tile_index<8, true>(pos, l)];
+    double2 *dst = spec + line0 * PITCH;
+    for (int idx = tid; idx < 8 * PITCH; idx += NT) {
+        const int l = idx / PITCH, pos = idx % PITCH;
+        if (pos <= N2) dst[idx] = s[tile_index<8, true>(pos, l)];
     }
 }
 
@@ -262,28 +370,29 @@ fft_x_r2c_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec, int
 // a8: complex-to-real along x with the normalisation of the whole transform chain; writes p^(n+1).
 // ------------------------------------------------------------------------------------------------
 template <int N2, int NT>
-__global__ void __launch_bounds__(NT)
-fft_x_c2r_kernel(const double2 *__restrict__ spec, double *__restrict__ out, int pitch,
+__global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1)
+fft_x_c2r_kernel(const double2 *__restrict__ spec, double *__restrict__ out,
                  const double2 *__restrict__ tw, double scale) {
     extern __shared__ double2 smem[];
     double2 *s = smem;
+    constexpr int PITCH = N2 + 8;
     const int tid = threadIdx.x;
     const long long line0 = (long long)blockIdx.x * 8;
-    for (int l = 0; l < 8; ++l) {
-        const double2 *src = spec + (line0 + l) * pitch;
-        for (int pos = tid; pos <= N2; pos += NT) s[tile_index<8, true>(pos, l)] = src[pos];
-    }
+    const double2 *src = spec + line0 * PITCH;
+    batched_copy<8 * PITCH, NT, 9, double2>(
+        tid, [&](int idx) { return src[idx]; },
+        [&](int idx, double2 val) {
+            const int l = idx / PITCH, pos = idx % PITCH;
+            if (pos <= N2) s[tile_index<8, true>(pos, l)] = val;
+        });
     __syncthreads();
     for (int item = tid; item < 8 * (N2 / 2 + 1); item += NT) c2r_pre_item<N2, 8, true>(s, item / 8, item % 8, tw);
     __syncthreads();
     tile_fft<N2, 8, true, NT, +1>(s, tw, 2, tid);
     __syncthreads();
     double2 *dst = reinterpret_cast<double2 *>(out) + line0 * N2;
-#pragma unroll 4
-    for (int idx = tid; idx < 8 * N2; idx += NT) {
-        const int l = idx / N2, i = idx % N2;
-        dst[idx] = cscale(s[tile_index<8, true>(i, l)], scale);
-    }
+    for (int idx = tid; idx < 8 * N2; idx += NT)
+        dst[idx] = cscale(s[tile_index<8, true>(idx % N2, idx / N2)], scale);
 }
 
 // ------------------------------------------------------------------------------------------------
