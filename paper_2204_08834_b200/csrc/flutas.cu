@@ -11,6 +11,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "kernels_tma.cuh"
 
 using namespace flutas;
 
@@ -63,6 +64,9 @@ struct flutas_plan {
     // tuning
     int y_cols, z_cols;          // tile width (columns of kx) of the strided passes
     int rhs_kc;                  // planes one thread of the RHS kernel marches through
+    int use_tma;                 // strided passes: 1 = TMA prefetch + register-resident twiddles (default), 2 = generic TMA in/out, 0 = plain loads
+    int num_sms;
+    CUtensorMap map_y, map_z;    // boxes {2*y_cols, rows, 1} and {2*z_cols, 1, rows} over the half-spectrum
     // timing
     int timing;
     cudaEvent_t *events;         // kMaxPendingSteps * (n_launch + 1)
@@ -107,6 +111,40 @@ template <typename T> static int upload(T **dst, const std::vector<T> &src, size
     CUDA_TRY(cudaMalloc((void **)dst, src.size() * sizeof(T)));
     CUDA_TRY(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
     *bytes += src.size() * sizeof(T);
+    return FLUTAS_OK;
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time dependency on libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static int make_spectrum_map(flutas_plan *pl, CUtensorMap *map, int cols, int line_dim, int n) {
+    static EncodeTiledFn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+        if (!fn || q != cudaDriverEntryPointSuccess) return fail(FLUTAS_ERR_CUDA, "cuTensorMapEncodeTiled is not available");
+        encode = (EncodeTiledFn)fn;
+    }
+    const cuuint32_t rows = (cuuint32_t)(n < 256 ? n : 256);
+    const cuuint64_t gdim[3] = {(cuuint64_t)2 * pl->nxh, (cuuint64_t)pl->ny, (cuuint64_t)pl->nz};
+    const cuuint64_t gstride[2] = {(cuuint64_t)pl->pitch * 16, (cuuint64_t)pl->pitch * pl->ny * 16};
+    const cuuint32_t box[3] = {(cuuint32_t)(2 * cols), line_dim == 1 ? rows : 1u, line_dim == 2 ? rows : 1u};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, pl->spec, gdim, gstride, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              cols >= 8 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(FLUTAS_ERR_CUDA, "cuTensorMapEncodeTiled failed with code %d", (int)r);
+    return FLUTAS_OK;
+}
+
+static int plan_make_maps(flutas_plan *pl) {
+    if (int rc = make_spectrum_map(pl, &pl->map_y, pl->y_cols, 1, pl->ny)) return rc;
+    if (pl->bc_z == FLUTAS_BC_Z_PERIODIC)
+        if (int rc = make_spectrum_map(pl, &pl->map_z, pl->z_cols, 2, pl->nz)) return rc;
     return FLUTAS_OK;
 }
 
@@ -167,9 +205,14 @@ static int plan_build(flutas_plan *pl) {
     pl->launch_ids[n++] = K_IFFTX;
     pl->launch_ids[n++] = K_CORR;
     pl->n_launch = n;
-    pl->y_cols = ny >= 2048 ? 4 : 8;
-    pl->z_cols = nz >= 2048 ? 4 : 8;
+    pl->y_cols = ny >= 1024 ? 4 : 8;
+    pl->z_cols = nz >= 1024 ? 4 : 8;
     pl->rhs_kc = 32;
+    pl->use_tma = 1;
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&pl->num_sms, cudaDevAttrMultiProcessorCount, dev));
+    if (int rc = plan_make_maps(pl)) return rc;
     return FLUTAS_OK;
 }
 
@@ -252,8 +295,9 @@ extern "C" double flutas_plan_kernel_bytes(const flutas_plan *pl, int idx) {
 
 extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int value) {
     if (!pl || !name) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan or option name");
-    if (!strcmp(name, "y_cols") && (value == 4 || value == 8)) { pl->y_cols = value; return FLUTAS_OK; }
-    if (!strcmp(name, "z_cols") && (value == 4 || value == 8)) { pl->z_cols = value; return FLUTAS_OK; }
+    if (!strcmp(name, "y_cols") && (value == 4 || (value == 8 && pl->ny < 2048))) { pl->y_cols = value; return plan_make_maps(pl); }
+    if (!strcmp(name, "z_cols") && (value == 4 || (value == 8 && pl->nz < 2048))) { pl->z_cols = value; return plan_make_maps(pl); }
+    if (!strcmp(name, "tma") && value >= 0 && value <= 2) { pl->use_tma = value; return FLUTAS_OK; }
     if (!strcmp(name, "rhs_kc") && value >= 1) { pl->rhs_kc = value; return FLUTAS_OK; }
     return fail(FLUTAS_ERR_INVALID_ARG, "unknown option or value: %s = %d", name, value);
 }
@@ -294,6 +338,76 @@ template <int MODE> static cudaError_t launch_strided(int n, int cols, const Str
         case 512: return launch_strided_n<512, MODE>(cols, a, nxh, n_outer, st);
         case 1024: return launch_strided_n<1024, MODE>(cols, a, nxh, n_outer, st);
         case 2048: return launch_strided_n<2048, MODE>(4, a, nxh, n_outer, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+// ---- persistent TMA-fed strided passes
+constexpr int tma_nt(int n, int c) { return n * c / 8 < 32 ? 32 : (n * c / 8 > 512 ? 512 : n * c / 8); }
+constexpr int tma_nbuf(int n, int c) { return 2 * n * c * 16 + 4096 <= 227 * 1024 ? 2 : 1; }
+
+template <int N, int C, int MODE>
+static cudaError_t launch_tma_nc(const CUtensorMap &map, const TmaFftArgs &a, const Tma1Args &a1, int variant, int num_sms,
+                                 cudaStream_t st) {
+    const long long ntiles = (long long)a.n_tiles_x * a.n_outer;
+    if constexpr (N * C / 8 <= 512) {
+        if (variant == 1) {
+            // one butterfly per thread: register-cached twiddles, direct stores, TMA prefetch only
+            constexpr int NT = N * C / 8 < 32 ? 32 : N * C / 8;
+            constexpr int P = Fact<N>::P, NCACHE = P - 1 < 2 ? P - 1 : 2;
+            const size_t smem = (size_t)2 * N * C * 16 + 128;
+            auto kern = fft_tma1_kernel<N, C, MODE, NT, NCACHE>;
+            cudaError_t e = set_smem(kern, smem);
+            if (e != cudaSuccess) return e;
+            int per_sm = 0;
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem);
+            if (e != cudaSuccess) return e;
+            if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+            long long grid = (long long)num_sms * per_sm;
+            if (grid > ntiles) grid = ntiles;
+            kern<<<(unsigned)grid, NT, smem, st>>>(map, a1);
+            return cudaGetLastError();
+        }
+    }
+    constexpr int NT = tma_nt(N, C), NBUF = tma_nbuf(N, C);
+    const size_t smem = (size_t)NBUF * N * C * 16 + 128;
+    auto kern = fft_tma_kernel<N, C, MODE, NT, NBUF>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    long long grid = (long long)num_sms * per_sm;
+    if (grid > ntiles) grid = ntiles;
+    kern<<<(unsigned)grid, NT, smem, st>>>(map, a);
+    return cudaGetLastError();
+}
+template <int N, int MODE>
+static cudaError_t launch_tma_n(int cols, const CUtensorMap &map, TmaFftArgs a, Tma1Args a1, int variant, cudaStream_t st,
+                                int num_sms) {
+    a.n_tiles_x = a1.n_tiles_x = (a.nxh + cols - 1) / cols;
+    if (cols == 4) return launch_tma_nc<N, 4, MODE>(map, a, a1, variant, num_sms, st);
+    if constexpr (N >= 2048) return cudaErrorInvalidValue;
+    else return launch_tma_nc<N, 8, MODE>(map, a, a1, variant, num_sms, st);
+}
+template <int MODE>
+static cudaError_t launch_tma(int n, int cols, const CUtensorMap &map, const TmaFftArgs &a, long long row_stride,
+                              long long outer_stride, double2 *data, int variant, cudaStream_t st, int num_sms) {
+    Tma1Args a1{};
+    a1.data = data; a1.row_stride = row_stride; a1.outer_stride = outer_stride;
+    a1.n_outer = a.n_outer; a1.line_dim = a.line_dim; a1.nxh = a.nxh; a1.tw = a.tw;
+    a1.lam_x = a.lam_x; a1.lam_outer = a.lam_outer; a1.lam_pos = a.lam_pos;
+    switch (n) {
+        case 8: return launch_tma_n<8, MODE>(cols, map, a, a1, variant, st, num_sms);
+        case 16: return launch_tma_n<16, MODE>(cols, map, a, a1, variant, st, num_sms);
+        case 32: return launch_tma_n<32, MODE>(cols, map, a, a1, variant, st, num_sms);
+        case 64: return launch_tma_n<64, MODE>(cols, map, a, a1, variant, st, num_sms);
+        case 128: return launch_tma_n<128, MODE>(cols, map, a, a1, variant, st, num_sms);
+        case 256: return launch_tma_n<256, MODE>(cols, map, a, a1, variant, st, num_sms);
+        case 512: return launch_tma_n<512, MODE>(cols, map, a, a1, variant, st, num_sms);
+        case 1024: return launch_tma_n<1024, MODE>(cols, map, a, a1, variant, st, num_sms);
+        case 2048: return launch_tma_n<2048, MODE>(4, map, a, a1, variant, st, num_sms);
     }
     return cudaErrorInvalidValue;
 }
@@ -376,7 +490,14 @@ static int enqueue_solve_core(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
     ay.outer_stride = (long long)pl->pitch * pl->ny;
     ay.nxh = pl->nxh;
     ay.tw = pl->tw_y;
-    if (int rc = check_launch(launch_strided<MODE_FWD>(pl->ny, pl->y_cols, ay, pl->nxh, pl->nz, st), "fft_y_fwd")) return rc;
+    TmaFftArgs ty{};
+    ty.n_outer = pl->nz;
+    ty.line_dim = 1;
+    ty.nxh = pl->nxh;
+    ty.tw = pl->tw_y;
+    if (pl->use_tma) {
+        if (int rc = check_launch(launch_tma<MODE_FWD>(pl->ny, pl->y_cols, pl->map_y, ty, ay.row_stride, ay.outer_stride, pl->spec, pl->use_tma, st, pl->num_sms), "fft_y_fwd (tma)")) return rc;
+    } else if (int rc = check_launch(launch_strided<MODE_FWD>(pl->ny, pl->y_cols, ay, pl->nxh, pl->nz, st), "fft_y_fwd")) return rc;
     if (tm) tm->mark();
     if (!wall) {
         StridedArgs az{};
@@ -388,7 +509,17 @@ static int enqueue_solve_core(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
         az.lam_x = pl->lam_x;
         az.lam_outer = pl->lam_y;
         az.lam_pos = pl->lam_z;
-        if (int rc = check_launch(launch_strided<MODE_SOLVE>(pl->nz, pl->z_cols, az, pl->nxh, pl->ny, st), "z_solve")) return rc;
+        TmaFftArgs tz{};
+        tz.n_outer = pl->ny;
+        tz.line_dim = 2;
+        tz.nxh = pl->nxh;
+        tz.tw = pl->tw_z;
+        tz.lam_x = pl->lam_x;
+        tz.lam_outer = pl->lam_y;
+        tz.lam_pos = pl->lam_z;
+        if (pl->use_tma) {
+            if (int rc = check_launch(launch_tma<MODE_SOLVE>(pl->nz, pl->z_cols, pl->map_z, tz, az.row_stride, az.outer_stride, pl->spec, pl->use_tma, st, pl->num_sms), "z_solve (tma)")) return rc;
+        } else if (int rc = check_launch(launch_strided<MODE_SOLVE>(pl->nz, pl->z_cols, az, pl->nxh, pl->ny, st), "z_solve")) return rc;
         if (tm) tm->mark();
     } else {
         const long long ncol = (long long)pl->pitch * pl->ny;
@@ -404,7 +535,9 @@ static int enqueue_solve_core(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
         if (int rc = check_launch(cudaGetLastError(), "z_singular")) return rc;
         if (tm) tm->mark();
     }
-    if (int rc = check_launch(launch_strided<MODE_INV>(pl->ny, pl->y_cols, ay, pl->nxh, pl->nz, st), "fft_y_inv")) return rc;
+    if (pl->use_tma) {
+        if (int rc = check_launch(launch_tma<MODE_INV>(pl->ny, pl->y_cols, pl->map_y, ty, ay.row_stride, ay.outer_stride, pl->spec, pl->use_tma, st, pl->num_sms), "fft_y_inv (tma)")) return rc;
+    } else if (int rc = check_launch(launch_strided<MODE_INV>(pl->ny, pl->y_cols, ay, pl->nxh, pl->nz, st), "fft_y_inv")) return rc;
     if (tm) tm->mark();
     return FLUTAS_OK;
 }

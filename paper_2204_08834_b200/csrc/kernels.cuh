@@ -34,10 +34,21 @@ struct GridParams {
 // shuffles (edge lanes load them), y neighbours from L1/L2 (the rows were loaded one iteration earlier by
 // the neighbouring threads).  Per point: 4 reciprocals, no integer division, 32-bit index arithmetic.
 // ------------------------------------------------------------------------------------------------
+// Reciprocal of a normal, positive double: hardware seed (MUFU.RCP64H, ~2^-23) + two Newton steps
+// (relative error <= ~1 ulp, branch-free, 5 instructions instead of the ~30 of an IEEE division).
+// Used only where the operand is a face density (rho > 0, far from the denormal / overflow ranges).
+__device__ __forceinline__ double rcp_density(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(fma(-x, r, 1.0), r, r);
+    r = fma(fma(-x, r, 1.0), r, r);
+    return r;
+}
+
 struct Flux { double f, r; };   // f = (1 - rho0/rho_f) * g,  r = 1/rho_f
 __device__ __forceinline__ Flux face_flux(double rc_a, double rc_b, double g, double rho0) {
     Flux o;
-    o.r = 1.0 / (0.5 * (rc_a + rc_b));
+    o.r = rcp_density(0.5 * (rc_a + rc_b));
     o.f = (1.0 - rho0 * o.r) * g;
     return o;
 }
