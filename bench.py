@@ -239,7 +239,7 @@ def run_ours(args):
     peak_gbs, peak_label = load_peak()
     traffic = load_ncu_traffic()
     names = [w for w in args.workloads.split(",") if w]
-    results = [bench_workload(n, args, rank, local_rank, world, peak_gbs, peak_label, with_e2e=(i == 0 or args.e2e_all),
+    results = [bench_workload(n, args, rank, local_rank, world, peak_gbs, peak_label, with_e2e=(not args.no_e2e) and (i == 0 or args.e2e_all),
                               traffic=traffic) for i, n in enumerate(names)]
     out = results[0]
     if len(results) > 1:
@@ -285,6 +285,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-all", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--opt", action="append", help="plan tuning knob name=value (experiments)")
     args = ap.parse_args()
     if args.impl == "reference":
