@@ -64,6 +64,7 @@ struct flutas_plan {
     // tuning
     int y_cols, z_cols;          // tile width (columns of kx) of the strided passes
     int rhs_kc;                  // planes one thread of the RHS kernel marches through
+    int rhs_variant, rhs_bx;     // 2 = software-pipelined kernel (default), 1 = first form; threads along x per block
     int use_tma;                 // strided passes: 1 = TMA prefetch + register-resident twiddles (default), 2 = generic TMA in/out, 0 = plain loads
     int num_sms;
     CUtensorMap map_y, map_z;    // boxes {2*y_cols, rows, 1} and {2*z_cols, 1, rows} over the half-spectrum
@@ -208,6 +209,8 @@ static int plan_build(flutas_plan *pl) {
     pl->y_cols = ny >= 1024 ? 4 : 8;
     pl->z_cols = nz >= 1024 ? 4 : 8;
     pl->rhs_kc = 32;
+    pl->rhs_variant = 2;
+    pl->rhs_bx = 64;
     pl->use_tma = 1;
     int dev = 0;
     CUDA_TRY(cudaGetDevice(&dev));
@@ -299,6 +302,8 @@ extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int val
     if (!strcmp(name, "z_cols") && (value == 4 || (value == 8 && pl->nz < 2048))) { pl->z_cols = value; return plan_make_maps(pl); }
     if (!strcmp(name, "tma") && value >= 0 && value <= 2) { pl->use_tma = value; return FLUTAS_OK; }
     if (!strcmp(name, "rhs_kc") && value >= 1) { pl->rhs_kc = value; return FLUTAS_OK; }
+    if (!strcmp(name, "rhs_variant") && (value == 1 || value == 2)) { pl->rhs_variant = value; return FLUTAS_OK; }
+    if (!strcmp(name, "rhs_bx") && (value == 8 || value == 16 || value == 32 || value == 64 || value == 128)) { pl->rhs_bx = value; return FLUTAS_OK; }
     return fail(FLUTAS_ERR_INVALID_ARG, "unknown option or value: %s = %d", name, value);
 }
 
@@ -472,12 +477,17 @@ static int check_launch(cudaError_t e, const char *what) {
 static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
                        const double *p, const double *po, double dt, double *rhs, cudaStream_t st) {
     // block = (bx threads x 2 points) x ty rows; nx/2 and ny are powers of two, so the grid divides evenly
-    const int bx = pl->nx / 2 < 64 ? pl->nx / 2 : 64;
+    const int bx = pl->nx / 2 < pl->rhs_bx ? pl->nx / 2 : pl->rhs_bx;
     int ty = 256 / bx;
     if (ty > pl->ny) ty = pl->ny;
     const int kc = pl->rhs_kc < pl->nz ? pl->rhs_kc : pl->nz;
     dim3 block(bx, ty), grid(pl->nx / 2 / bx, pl->ny / ty, (pl->nz + kc - 1) / kc);
-    splitting_rhs_kernel<<<grid, block, 0, st>>>(pl->grid, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+    if (pl->rhs_variant == 1)
+        splitting_rhs_kernel<<<grid, block, 0, st>>>(pl->grid, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+    else if (pl->bc_z == FLUTAS_BC_Z_WALL)
+        splitting_rhs_kernel2<true><<<grid, block, 0, st>>>(pl->grid, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+    else
+        splitting_rhs_kernel2<false><<<grid, block, 0, st>>>(pl->grid, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
     return check_launch(cudaGetLastError(), "splitting_rhs");
 }
 

@@ -161,6 +161,129 @@ splitting_rhs_kernel(GridParams g, double dt, int kc, const double *__restrict__
 }
 
 // ------------------------------------------------------------------------------------------------
+// Second form of the same kernel: identical decomposition (thread = 2 x-points, marching in z), but
+//  * software-pipelined: the operands that miss in cache (phi, p, p_old of plane k+2 and u*, v*, w* of plane
+//    k+1) are requested one iteration before they are used, so a warp waits on DRAM once per kernel instead
+//    of once per plane; the row / edge neighbours of the current plane (L1 / L2 hits) are requested at the top
+//    of the iteration and consumed last;
+//  * trimmed arithmetic: rho_c = fma(rho1 - rho2, phi, rho2); 1 - rho0/rho_f = 1 - 2 rho0 / (rho_a + rho_b);
+//    u' = u* + (dt/rho0) F, because (1/rho_f - 1/rho0) = -(1 - rho0/rho_f)/rho0, so the face flux F already
+//    computed for the right-hand side is all the half-corrected velocity needs.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double2 ldg2(const double *f, long long q) {
+    return __ldg(reinterpret_cast<const double2 *>(f + q));
+}
+__device__ __forceinline__ void stcs2(double *f, long long q, double2 v) {
+    __stcs(reinterpret_cast<double2 *>(f + q), v);
+}
+// (1 - rho0/rho_f) for the face between cells of density ra and rb
+__device__ __forceinline__ double flux_coef(double ra, double rb, double m2rho0) {
+    return fma(m2rho0, rcp_density(ra + rb), 1.0);
+}
+
+template <bool WALL>
+__global__ void __launch_bounds__(256, 2)
+splitting_rhs_kernel2(GridParams g, double dt, int kc, const double *__restrict__ u, const double *__restrict__ v,
+                      const double *__restrict__ w, const double *__restrict__ phi,
+                      const double *__restrict__ p, const double *__restrict__ po,
+                      double *__restrict__ rhs, double *__restrict__ up, double *__restrict__ vp,
+                      double *__restrict__ wp) {
+    const int nx = g.nx, ny = g.ny, nz = g.nz;
+    const int i0 = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(k0 + kc, nz);
+    const int jn = (j + 1 == ny) ? 0 : j + 1, js = (j == 0) ? ny - 1 : j - 1;
+    const int iw = (i0 == 0) ? nx - 1 : i0 - 1, ie = (i0 + 2 == nx) ? 0 : i0 + 2;
+    const int lane = (threadIdx.x + threadIdx.y * blockDim.x) & 31;
+    const int rw = blockDim.x < 32 ? blockDim.x : 32;
+    const bool edge_l = (lane % rw) == 0, edge_r = (lane % rw) == rw - 1;
+    const long long plane = (long long)nx * ny;
+    const long long col = (long long)j * nx + i0, col_n = (long long)jn * nx + i0, col_s = (long long)js * nx + i0;
+    const long long q_e = (long long)j * nx + ie, q_w = (long long)j * nx + iw;
+    const double drho = g.rho1 - g.rho2, rho2 = g.rho2, m2rho0 = -2.0 * g.rho0;
+    const double c_div = g.rho0 / dt, c_up = dt / g.rho0;
+    const double idx = g.inv_dx, idy = g.inv_dy, idz = g.inv_dz;
+
+    auto rho_of = [&](double f) { return fma(drho, f, rho2); };
+    auto rho2_of = [&](double2 f) { return make_double2(rho_of(f.x), rho_of(f.y)); };
+    auto phat = [&](double a, double b) { return fma(2.0, a, -b); };
+    auto phat2 = [&](double2 a, double2 b) { return make_double2(phat(a.x, b.x), phat(a.y, b.y)); };
+
+    // prologue: centre plane k0, the bottom-face flux and w below
+    long long qk = (long long)k0 * plane;
+    double2 rc_c = rho2_of(ldg2(phi, qk + col)), ph_c = phat2(ldg2(p, qk + col), ldg2(po, qk + col));
+    double2 fb = make_double2(0.0, 0.0), wb = make_double2(0.0, 0.0);
+    if (!(WALL && k0 == 0)) {
+        const long long qb = (long long)((k0 == 0) ? nz - 1 : k0 - 1) * plane + col;
+        const double2 rc_b = rho2_of(ldg2(phi, qb)), ph_b = phat2(ldg2(p, qb), ldg2(po, qb));
+        fb.x = flux_coef(rc_b.x, rc_c.x, m2rho0) * ((ph_c.x - ph_b.x) * idz);
+        fb.y = flux_coef(rc_b.y, rc_c.y, m2rho0) * ((ph_c.y - ph_b.y) * idz);
+        wb = ldg2(w, qb);
+    }
+    // pipeline registers: plane k+1 (phi, p, p_old at the centre column) and plane k (u*, v*, w*, v* south)
+    auto plane_of = [&](int k) { return WALL ? min(k, nz - 1) : (k >= nz ? k - nz : k); };
+    long long qt = (long long)plane_of(k0 + 1) * plane + col;
+    double2 a_phi = ldg2(phi, qt), a_p = ldg2(p, qt), a_po = ldg2(po, qt);
+    double2 uc = ldg2(u, qk + col), vc = ldg2(v, qk + col), wc = ldg2(w, qk + col), vs = ldg2(v, qk + col_s);
+
+    for (int k = k0; k < k1; ++k, qk += plane) {
+        const bool top = WALL && (k + 1 == nz);
+        // ---- requests for the NEXT iteration (DRAM latency, consumed one iteration later)
+        double2 n_phi = a_phi, n_p = a_p, n_po = a_po, n_uc = uc, n_vc = vc, n_wc = wc, n_vs = vs;
+        if (k + 1 < k1) {
+            const long long q2 = (long long)plane_of(k + 2) * plane + col, q1 = qk + plane;
+            n_phi = ldg2(phi, q2); n_p = ldg2(p, q2); n_po = ldg2(po, q2);
+            n_uc = ldg2(u, q1 + col); n_vc = ldg2(v, q1 + col); n_wc = ldg2(w, q1 + col); n_vs = ldg2(v, q1 + col_s);
+        }
+        // ---- requests for THIS iteration that hit in L1 / L2: row neighbours and the two edge columns
+        const double2 r_nphi = ldg2(phi, qk + col_n), r_np = ldg2(p, qk + col_n), r_npo = ldg2(po, qk + col_n);
+        const double2 r_sphi = ldg2(phi, qk + col_s), r_sp = ldg2(p, qk + col_s), r_spo = ldg2(po, qk + col_s);
+        double e_phi = 0.0, e_p = 0.0, e_po = 0.0, w_phi = 0.0, w_p = 0.0, w_po = 0.0, w_u = 0.0;
+        if (edge_r) { e_phi = __ldg(phi + qk + q_e); e_p = __ldg(p + qk + q_e); e_po = __ldg(po + qk + q_e); }
+        if (edge_l) { w_phi = __ldg(phi + qk + q_w); w_p = __ldg(p + qk + q_w); w_po = __ldg(po + qk + q_w); w_u = __ldg(u + qk + q_w); }
+
+        // ---- z faces (top of this plane; wall faces carry zero flux)
+        double2 rc_t = rc_c, ph_t = ph_c, ft = make_double2(0.0, 0.0);
+        if (!top) {
+            rc_t = rho2_of(a_phi);
+            ph_t = phat2(a_p, a_po);
+            ft.x = flux_coef(rc_c.x, rc_t.x, m2rho0) * ((ph_t.x - ph_c.x) * idz);
+            ft.y = flux_coef(rc_c.y, rc_t.y, m2rho0) * ((ph_t.y - ph_c.y) * idz);
+        }
+        // ---- x faces: m between (i0, i0+1), e between (i0+1, i0+2), west face from the left lane
+        double rc_e = __shfl_down_sync(0xffffffffu, rc_c.x, 1), ph_e = __shfl_down_sync(0xffffffffu, ph_c.x, 1);
+        if (edge_r) { rc_e = rho_of(e_phi); ph_e = phat(e_p, e_po); }
+        const double fm = flux_coef(rc_c.x, rc_c.y, m2rho0) * ((ph_c.y - ph_c.x) * idx);
+        const double fe = flux_coef(rc_c.y, rc_e, m2rho0) * ((ph_e - ph_c.y) * idx);
+        double f_w = __shfl_up_sync(0xffffffffu, fe, 1), u_w = __shfl_up_sync(0xffffffffu, uc.y, 1);
+        if (edge_l) {
+            f_w = flux_coef(rho_of(w_phi), rc_c.x, m2rho0) * ((ph_c.x - phat(w_p, w_po)) * idx);
+            u_w = w_u;
+        }
+        // ---- y faces
+        const double2 rc_n = rho2_of(r_nphi), ph_n = phat2(r_np, r_npo);
+        const double2 rc_s = rho2_of(r_sphi), ph_s = phat2(r_sp, r_spo);
+        const double fn0 = flux_coef(rc_c.x, rc_n.x, m2rho0) * ((ph_n.x - ph_c.x) * idy);
+        const double fn1 = flux_coef(rc_c.y, rc_n.y, m2rho0) * ((ph_n.y - ph_c.y) * idy);
+        const double fs0 = flux_coef(rc_s.x, rc_c.x, m2rho0) * ((ph_c.x - ph_s.x) * idy);
+        const double fs1 = flux_coef(rc_s.y, rc_c.y, m2rho0) * ((ph_c.y - ph_s.y) * idy);
+
+        double2 out;
+        out.x = c_div * ((uc.x - u_w) * idx + (vc.x - vs.x) * idy + (wc.x - wb.x) * idz) +
+                ((fm - f_w) * idx + (fn0 - fs0) * idy + (ft.x - fb.x) * idz);
+        out.y = c_div * ((uc.y - uc.x) * idx + (vc.y - vs.y) * idy + (wc.y - wb.y) * idz) +
+                ((fe - fm) * idx + (fn1 - fs1) * idy + (ft.y - fb.y) * idz);
+        stcs2(rhs, qk + col, out);
+        stcs2(up, qk + col, make_double2(fma(c_up, fm, uc.x), fma(c_up, fe, uc.y)));
+        stcs2(vp, qk + col, make_double2(fma(c_up, fn0, vc.x), fma(c_up, fn1, vc.y)));
+        stcs2(wp, qk + col, make_double2(fma(c_up, ft.x, wc.x), fma(c_up, ft.y, wc.y)));   // top wall: ft = 0
+
+        fb = ft; wb = wc; rc_c = rc_t; ph_c = ph_t;
+        a_phi = n_phi; a_p = n_p; a_po = n_po; uc = n_uc; vc = n_vc; wc = n_wc; vs = n_vs;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // a9: u = u' - dt/rho0 grad p^(n+1)   (eq. 18; p^(n+1) was already stored by a8)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
