@@ -66,23 +66,21 @@ template <int N> struct Fact {
 template <int N> FL_HD int pass_radix(int p) { return p < Fact<N>::P ? 8 : Fact<N>::RLAST; }
 template <int N> FL_HD int pass_stride(int p) { return p < Fact<N>::P ? N / ipow8(p) : 1; }
 
-// position (storage index after the forward transform) <-> frequency
+// position (storage index after the forward transform) <-> frequency.  All radices are powers of two, so
+// the digit exchange is shifts and masks (no division): digit p (p < P) of the frequency is 3 bits wide and
+// weighs N / 8^p in the position; the last digit (radix RLAST) weighs 1.
 template <int N> FL_HD int freq_of_pos(int pos) {
-    int k = 0, w = 1;
-    for (int p = 1; p <= Fact<N>::P; ++p) {
-        int r = pass_radix<N>(p), m = pass_stride<N>(p);
-        k += ((pos / m) % r) * w;
-        w *= r;
-    }
+    constexpr int P = Fact<N>::P;
+    int k = (pos & (Fact<N>::RLAST - 1)) << (3 * (P - 1));
+#pragma unroll
+    for (int p = 1; p < P; ++p) k += ((pos >> (Fact<N>::LOG - 3 * p)) & 7) << (3 * (p - 1));
     return k;
 }
 template <int N> FL_HD int pos_of_freq(int k) {
-    int pos = 0, w = 1;
-    for (int p = 1; p <= Fact<N>::P; ++p) {
-        int r = pass_radix<N>(p), m = pass_stride<N>(p);
-        pos += ((k / w) % r) * m;
-        w *= r;
-    }
+    constexpr int P = Fact<N>::P;
+    int pos = k >> (3 * (P - 1));
+#pragma unroll
+    for (int p = 1; p < P; ++p) pos += ((k >> (3 * (p - 1))) & 7) << (Fact<N>::LOG - 3 * p);
     return pos;
 }
 

@@ -12,6 +12,7 @@
 
 #include "kernels.cuh"
 #include "kernels_tma.cuh"
+#include "kernels_x.cuh"
 
 using namespace flutas;
 
@@ -64,6 +65,7 @@ struct flutas_plan {
     // tuning
     int y_cols, z_cols;          // tile width (columns of kx) of the strided passes
     int rhs_kc;                  // planes one thread of the RHS kernel marches through
+    int x_variant;               // x transforms: 1 = persistent bulk-copy-fed kernels (nx = 128..1024), 0 = staged kernels
     int rhs_variant, rhs_bx;     // 2 = software-pipelined kernel (default), 1 = first form; threads along x per block
     int use_tma;                 // strided passes: 1 = TMA prefetch + register-resident twiddles (default), 2 = generic TMA in/out, 0 = plain loads
     int num_sms;
@@ -171,8 +173,7 @@ static int plan_build(flutas_plan *pl) {
         if (int rc = upload(&pl->tw_z, t, &pl->bytes)) return rc;
     }
     std::vector<double> lam(pl->pitch, 1.0);
-    for (int pos = 0; pos < pl->n2; ++pos) lam[pos] = host_lambda(host_freq_of_pos(pl->n2, pos), nx, dx);
-    lam[pl->n2] = host_lambda(pl->n2, nx, dx);
+    for (int k = 0; k <= pl->n2; ++k) lam[k] = host_lambda(k, nx, dx);   // x columns are stored in natural order
     if (int rc = upload(&pl->lam_x, lam, &pl->bytes)) return rc;
     lam.assign(ny, 0.0);
     for (int pos = 0; pos < ny; ++pos) lam[pos] = host_lambda(host_freq_of_pos(ny, pos), ny, dy);
@@ -210,6 +211,7 @@ static int plan_build(flutas_plan *pl) {
     pl->z_cols = nz >= 1024 ? 4 : 8;
     pl->rhs_kc = 32;
     pl->rhs_variant = 2;
+    pl->x_variant = 1;
     pl->rhs_bx = 64;
     pl->use_tma = 1;
     int dev = 0;
@@ -302,6 +304,7 @@ extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int val
     if (!strcmp(name, "z_cols") && (value == 4 || (value == 8 && pl->nz < 2048))) { pl->z_cols = value; return plan_make_maps(pl); }
     if (!strcmp(name, "tma") && value >= 0 && value <= 2) { pl->use_tma = value; return FLUTAS_OK; }
     if (!strcmp(name, "rhs_kc") && value >= 1) { pl->rhs_kc = value; return FLUTAS_OK; }
+    if (!strcmp(name, "x_variant") && (value == 0 || value == 1)) { pl->x_variant = value; return FLUTAS_OK; }
     if (!strcmp(name, "rhs_variant") && (value == 1 || value == 2)) { pl->rhs_variant = value; return FLUTAS_OK; }
     if (!strcmp(name, "rhs_bx") && (value == 8 || value == 16 || value == 32 || value == 64 || value == 128)) { pl->rhs_bx = value; return FLUTAS_OK; }
     return fail(FLUTAS_ERR_INVALID_ARG, "unknown option or value: %s = %d", name, value);
@@ -435,8 +438,46 @@ template <int N2> static cudaError_t launch_c2r_n(const flutas_plan *pl, double 
     kern<<<(unsigned)((long long)pl->ny * pl->nz / 8), NT, smem, st>>>(pl->spec, out, pl->tw_x, scale);
     return cudaGetLastError();
 }
+// persistent bulk-copy-fed x kernels (nx = 128 .. 1024)
+template <int N2> static cudaError_t launch_r2c_tma_n(const flutas_plan *pl, const double *rhs, cudaStream_t st) {
+    const size_t smem = (size_t)2 * 8 * N2 * 16 + 128;
+    auto kern = fft_x_r2c_tma_kernel<N2>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, N2, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    const long long ntiles = (long long)pl->ny * pl->nz / 8;
+    long long grid = (long long)pl->num_sms * per_sm;
+    if (grid > ntiles) grid = ntiles;
+    kern<<<(unsigned)grid, N2, smem, st>>>(rhs, pl->spec, pl->tw_x, (int)ntiles);
+    return cudaGetLastError();
+}
+template <int N2> static cudaError_t launch_c2r_tma_n(const flutas_plan *pl, double *out, double scale, cudaStream_t st) {
+    const size_t smem = (size_t)8 * (N2 + 8) * 16 + (size_t)8 * N2 * 16 + 128;
+    auto kern = fft_x_c2r_tma_kernel<N2>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, N2, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    const long long ntiles = (long long)pl->ny * pl->nz / 8;
+    long long grid = (long long)pl->num_sms * per_sm;
+    if (grid > ntiles) grid = ntiles;
+    kern<<<(unsigned)grid, N2, smem, st>>>(pl->spec, out, pl->tw_x, scale, (int)ntiles);
+    return cudaGetLastError();
+}
+#define FOR_EACH_N2_TMA(X) X(64) X(128) X(256) X(512)
 #define FOR_EACH_N2(X) X(8) X(16) X(32) X(64) X(128) X(256) X(512) X(1024)
 static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStream_t st) {
+    if (pl->x_variant == 1)
+        switch (pl->n2) {
+#define X(n) case n: return launch_r2c_tma_n<n>(pl, rhs, st);
+            FOR_EACH_N2_TMA(X)
+#undef X
+        }
     switch (pl->n2) {
 #define X(n) case n: return launch_r2c_n<n>(pl, rhs, st);
         FOR_EACH_N2(X)
@@ -445,6 +486,12 @@ static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStre
     return cudaErrorInvalidValue;
 }
 static cudaError_t launch_c2r(const flutas_plan *pl, double *out, double scale, cudaStream_t st) {
+    if (pl->x_variant == 1)
+        switch (pl->n2) {
+#define X(n) case n: return launch_c2r_tma_n<n>(pl, out, scale, st);
+            FOR_EACH_N2_TMA(X)
+#undef X
+        }
     switch (pl->n2) {
 #define X(n) case n: return launch_c2r_n<n>(pl, out, scale, st);
         FOR_EACH_N2(X)

@@ -472,7 +472,7 @@ __device__ __forceinline__ void batched_copy(int tid, Load load, Store store) {
 
 // ------------------------------------------------------------------------------------------------
 // a4: real-to-complex along x.  CTA = 8 consecutive lines (contiguous in memory), N2 = nx/2.
-// Output row (line) layout: positions 0..N2-1 in permuted order, Nyquist at N2; row pitch = N2 + 8,
+// Output row (line) layout: kx = 0..N2 in natural order; row pitch = N2 + 8,
 // so the 8 output rows of a CTA are one contiguous block as well.
 // ------------------------------------------------------------------------------------------------
 template <int N2, int NT>
@@ -495,8 +495,8 @@ fft_x_r2c_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec,
     __syncthreads();
     double2 *dst = spec + line0 * PITCH;
     for (int idx = tid; idx < 8 * PITCH; idx += NT) {
-        const int l = idx / PITCH, pos = idx % PITCH;
-        if (pos <= N2) dst[idx] = s[tile_index<8, true>(pos, l)];
+        const int l = idx / PITCH, k = idx % PITCH;     // spectrum rows are stored in natural kx order
+        if (k <= N2) dst[idx] = s[tile_index<8, true>(k == N2 ? N2 : pos_of_freq<N2>(k), l)];
     }
 }
 
@@ -516,8 +516,8 @@ fft_x_c2r_kernel(const double2 *__restrict__ spec, double *__restrict__ out,
     batched_copy<8 * PITCH, NT, 9, double2>(
         tid, [&](int idx) { return src[idx]; },
         [&](int idx, double2 val) {
-            const int l = idx / PITCH, pos = idx % PITCH;
-            if (pos <= N2) s[tile_index<8, true>(pos, l)] = val;
+            const int l = idx / PITCH, k = idx % PITCH;
+            if (k <= N2) s[tile_index<8, true>(k == N2 ? N2 : pos_of_freq<N2>(k), l)] = val;
         });
     __syncthreads();
     for (int item = tid; item < 8 * (N2 / 2 + 1); item += NT) c2r_pre_item<N2, 8, true>(s, item / 8, item % 8, tw);
