@@ -22,6 +22,7 @@ typedef struct {
     int nx, ny, nz, wall;
     double dx, dy, dz;
     double rho1, rho2, rho0, dt;
+    double r;   /* dt^(n+1) / dt^n, the time-step ratio of the pressure extrapolation; 1 = constant dt */
 } grid_t;
 
 static int grid_init(grid_t *g, int nx, int ny, int nz, double lx, double ly, double lz,
@@ -35,6 +36,7 @@ static int grid_init(grid_t *g, int nx, int ny, int nz, double lx, double ly, do
     g->rho1 = rho1; g->rho2 = rho2;
     g->rho0 = rho1 < rho2 ? rho1 : rho2;                        /* rho0 = min density, PAPER.md:161 (R3) */
     g->dt = dt;
+    g->r = 1.0;
     return 0;
 }
 
@@ -54,10 +56,11 @@ static inline double rho_c(const grid_t *g, const double *phi, int i, int j, int
     double f = phi[at(g, i, j, k)];
     return g->rho1 * f + g->rho2 * (1.0 - f);
 }
-/* time-extrapolated pressure for constant dt: p_hat = 2 p^n - p^(n-1) (R4) */
+/* time-extrapolated pressure: p_hat = (1 + r) p^n - r p^(n-1), r = dt^(n+1)/dt^n;
+ * constant dt (r = 1, R4) gives p_hat = 2 p^n - p^(n-1) */
 static inline double p_hat(const grid_t *g, const double *p, const double *p_old, int i, int j, int k) {
     size_t q = at(g, i, j, k);
-    return 2.0 * p[q] - p_old[q];
+    return (1.0 + g->r) * p[q] - g->r * p_old[q];
 }
 
 /* gradient of a centred field f on the east / north / top face of cell (i,j,k) */
@@ -152,13 +155,14 @@ int oracle_laplacian(int nx, int ny, int nz, double lx, double ly, double lz, in
 
 /* ------------------------------------------------------------ splitting RHS */
 
-int oracle_rhs(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
-               double rho1, double rho2, double dt,
-               const double *u, const double *v, const double *w, const double *phi,
-               const double *p, const double *p_old, double *rhs_out, int nthreads) {
+int oracle_rhs_vdt(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                   double rho1, double rho2, double dt, double dt_ratio,
+                   const double *u, const double *v, const double *w, const double *phi,
+                   const double *p, const double *p_old, double *rhs_out, int nthreads) {
     grid_t g;
     if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt)) return 1;
-    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0)) return 1;
+    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0) || !(dt_ratio > 0.0)) return 1;
+    g.r = dt_ratio;
     set_threads(nthreads);
 #pragma omp parallel for collapse(2) schedule(static)
     for (int k = 0; k < nz; ++k)
@@ -177,6 +181,13 @@ int oracle_rhs(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z
                 rhs_out[at(&g, i, j, k)] = g.rho0 / g.dt * d_u + d_f;
             }
     return 0;
+}
+
+int oracle_rhs(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+               double rho1, double rho2, double dt,
+               const double *u, const double *v, const double *w, const double *phi,
+               const double *p, const double *p_old, double *rhs_out, int nthreads) {
+    return oracle_rhs_vdt(nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt, 1.0, u, v, w, phi, p, p_old, rhs_out, nthreads);
 }
 
 /* ------------------------------------------------------------- naive DFT */
@@ -398,18 +409,19 @@ int oracle_correction(int nx, int ny, int nz, double lx, double ly, double lz, i
     return 0;
 }
 
-int oracle_projection_step(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
-                           double rho1, double rho2, double dt,
-                           double *u, double *v, double *w, const double *phi,
-                           double *p, const double *p_old, double *rhs_out, int nthreads) {
+int oracle_projection_step_vdt(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                               double rho1, double rho2, double dt, double dt_ratio,
+                               double *u, double *v, double *w, const double *phi,
+                               double *p, const double *p_old, double *rhs_out, int nthreads) {
     grid_t g;
     if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt)) return 1;
-    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0)) return 1;
+    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0) || !(dt_ratio > 0.0)) return 1;
+    g.r = dt_ratio;
     const size_t n = (size_t)nx * ny * nz;
     double *rhs = (double *)malloc(sizeof(double) * n), *p_new = (double *)malloc(sizeof(double) * n);
     int rc = 0;
     if (!rhs || !p_new) { rc = 2; goto done; }
-    if ((rc = oracle_rhs(nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt, u, v, w, phi, p, p_old, rhs, nthreads))) goto done;
+    if ((rc = oracle_rhs_vdt(nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt, dt_ratio, u, v, w, phi, p, p_old, rhs, nthreads))) goto done;
     if (rhs_out) memcpy(rhs_out, rhs, sizeof(double) * n);
     if ((rc = oracle_poisson(nx, ny, nz, lx, ly, lz, bc_z, rhs, p_new, NULL, nthreads))) goto done;
     set_threads(nthreads);
@@ -418,6 +430,14 @@ int oracle_projection_step(int nx, int ny, int nz, double lx, double ly, double 
 done:
     free(rhs); free(p_new);
     return rc;
+}
+
+int oracle_projection_step(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                           double rho1, double rho2, double dt,
+                           double *u, double *v, double *w, const double *phi,
+                           double *p, const double *p_old, double *rhs_out, int nthreads) {
+    return oracle_projection_step_vdt(nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt, 1.0, u, v, w, phi, p, p_old,
+                                      rhs_out, nthreads);
 }
 
 /* the paper's incremental grouping, eqs. (16)-(19), with the sign of R1 */

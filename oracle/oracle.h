@@ -62,6 +62,18 @@ int oracle_projection_step(int nx, int ny, int nz, double lx, double ly, double 
                            double *u, double *v, double *w, const double *phi,
                            double *p, const double *p_old, double *rhs_out, int nthreads);
 
+/* The same two calls for a variable time step:
+ *   p_hat = (1 + r) p^n - r p^(n-1),  r = dt_ratio = dt^(n+1) / dt^n > 0;  dt = dt^(n+1).
+ * dt_ratio = 1 is the constant-dt step above, bit for bit. */
+int oracle_rhs_vdt(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                   double rho1, double rho2, double dt, double dt_ratio,
+                   const double *u, const double *v, const double *w, const double *phi,
+                   const double *p, const double *p_old, double *rhs_out, int nthreads);
+int oracle_projection_step_vdt(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                               double rho1, double rho2, double dt, double dt_ratio,
+                               double *u, double *v, double *w, const double *phi,
+                               double *p, const double *p_old, double *rhs_out, int nthreads);
+
 /* The last part of the step alone (eq. 18 in the north_star grouping), in place on u, v, w:
  *   u = u* - dt [ (1/rho0) grad p_new + (1/rho_f - 1/rho0) grad p_hat ],  p_hat = 2 p - p_old.
  * Lets a test check the velocity correction at full size given any p_new. */

@@ -20,6 +20,8 @@ _GRID = [_ci, _ci, _ci, _cd, _cd, _cd, _ci]
 _lib.oracle_rhs.argtypes = _GRID + [_cd, _cd, _cd] + [_dp] * 7 + [_ci]
 _lib.oracle_poisson.argtypes = _GRID + [_dp, _dp, _dp, _ci]
 _lib.oracle_projection_step.argtypes = _GRID + [_cd, _cd, _cd] + [_dp] * 7 + [_ci]
+_lib.oracle_rhs_vdt.argtypes = _GRID + [_cd, _cd, _cd, _cd] + [_dp] * 7 + [_ci]
+_lib.oracle_projection_step_vdt.argtypes = _GRID + [_cd, _cd, _cd, _cd] + [_dp] * 7 + [_ci]
 _lib.oracle_projection_step_paper.argtypes = _GRID + [_cd, _cd, _cd] + [_dp] * 6 + [_ci]
 _lib.oracle_correction.argtypes = _GRID + [_cd, _cd, _cd] + [_dp] * 7 + [_ci]
 _lib.oracle_correction.restype = _ci
@@ -27,7 +29,7 @@ _lib.oracle_dft_axis.argtypes = [_cl, _ci, _cl, _ci, _dp, _dp, _dp, _dp, _ci]
 _lib.oracle_divergence.argtypes = _GRID + [_dp] * 4 + [_ci]
 _lib.oracle_laplacian.argtypes = _GRID + [_dp] * 2 + [_ci]
 _lib.oracle_threads.argtypes = [_ci]
-for _f in ("oracle_rhs", "oracle_poisson", "oracle_projection_step", "oracle_projection_step_paper",
+for _f in ("oracle_rhs_vdt", "oracle_projection_step_vdt", "oracle_rhs", "oracle_poisson", "oracle_projection_step", "oracle_projection_step_paper",
            "oracle_dft_axis", "oracle_divergence", "oracle_laplacian", "oracle_threads"):
     getattr(_lib, _f).restype = _ci
 
@@ -58,12 +60,17 @@ def threads(nthreads=0):
     return _lib.oracle_threads(int(nthreads))
 
 
-def rhs(u, v, w, phi, p, p_old, box, bc_z, rho1, rho2, dt, nthreads=0):
+def rhs(u, v, w, phi, p, p_old, box, bc_z, rho1, rho2, dt, nthreads=0, dt_ratio=None):
+    """dt_ratio = dt^(n+1)/dt^n selects the variable-time-step p_hat; None = constant dt."""
     u = _field(u)
     f = [_field(a, u.shape) for a in (v, w, phi, p, p_old)]
     out = np.empty_like(u)
-    _check(_lib.oracle_rhs(*_grid(u.shape, box, bc_z), rho1, rho2, dt, _p(u), *[_p(a) for a in f],
-                           _p(out), nthreads), "oracle_rhs")
+    if dt_ratio is None:
+        _check(_lib.oracle_rhs(*_grid(u.shape, box, bc_z), rho1, rho2, dt, _p(u), *[_p(a) for a in f],
+                               _p(out), nthreads), "oracle_rhs")
+    else:
+        _check(_lib.oracle_rhs_vdt(*_grid(u.shape, box, bc_z), rho1, rho2, dt, float(dt_ratio), _p(u),
+                                   *[_p(a) for a in f], _p(out), nthreads), "oracle_rhs_vdt")
     return out
 
 
@@ -76,15 +83,22 @@ def poisson(rhs_field, box, bc_z, nthreads=0, return_imag_residue=False):
     return (out, res.value) if return_imag_residue else out
 
 
-def projection_step(u, v, w, phi, p, p_old, box, bc_z, rho1, rho2, dt, nthreads=0, return_rhs=False):
-    """Returns new (u, v, w, p) [and rhs]; inputs are not modified."""
+def projection_step(u, v, w, phi, p, p_old, box, bc_z, rho1, rho2, dt, nthreads=0, return_rhs=False,
+                    dt_ratio=None):
+    """Returns new (u, v, w, p) [and rhs]; inputs are not modified.  dt_ratio as in rhs()."""
     u = _field(u).copy()
     v, w, p = (_field(a, u.shape).copy() for a in (v, w, p))
     phi, p_old = _field(phi, u.shape), _field(p_old, u.shape)
     r = np.empty_like(u) if return_rhs else None
-    _check(_lib.oracle_projection_step(*_grid(u.shape, box, bc_z), rho1, rho2, dt, _p(u), _p(v), _p(w),
-                                       _p(phi), _p(p), _p(p_old), _p(r) if return_rhs else None,
-                                       nthreads), "oracle_projection_step")
+    if dt_ratio is None:
+        _check(_lib.oracle_projection_step(*_grid(u.shape, box, bc_z), rho1, rho2, dt, _p(u), _p(v), _p(w),
+                                           _p(phi), _p(p), _p(p_old), _p(r) if return_rhs else None,
+                                           nthreads), "oracle_projection_step")
+    else:
+        _check(_lib.oracle_projection_step_vdt(*_grid(u.shape, box, bc_z), rho1, rho2, dt, float(dt_ratio),
+                                               _p(u), _p(v), _p(w), _p(phi), _p(p), _p(p_old),
+                                               _p(r) if return_rhs else None, nthreads),
+               "oracle_projection_step_vdt")
     return (u, v, w, p, r) if return_rhs else (u, v, w, p)
 
 

@@ -14,6 +14,8 @@ pressure or a divergence), so the pins are structural:
   P7  linearity and shift covariance
   P8  the paper's incremental grouping (eqs. 16-19) == the north_star grouping
   P9  independent numpy.fft + vectorised-Thomas restatement of the whole step
+  P10 variable time step: p_hat is the linear extrapolation of the pressure history to
+      t^(n+1); r = 1 is the constant-dt step bit for bit; a pressure linear in time is extrapolated exactly
 """
 import numpy as np
 import pytest
@@ -219,6 +221,60 @@ def test_p8_paper_grouping_equals_north_star_grouping(oracle_mod, idx):
     b = oracle_mod.projection_step_paper(*W.fields(), W.box, W.bc_z, W.rho1, W.rho2, W.dt)
     for x, y in zip(a, b):
         assert ops.rel_l2(y, x) < 1e-13 * (10 if W.rho2 > 100 else 1)
+
+
+# ------------------------------------------------------------- P10: variable time step
+@pytest.mark.parametrize("bc", [PER, WALL])
+def test_p10_unit_ratio_is_the_constant_dt_step_bit_for_bit(oracle_mod, bc):
+    W = wl.random_case(12, 10, 8, bc, 50.0, 51)
+    a = _step(oracle_mod, W, return_rhs=True)
+    b = _step(oracle_mod, W, return_rhs=True, dt_ratio=1.0)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+
+
+@pytest.mark.parametrize("bc,r", [(PER, 0.5), (WALL, 1.7), (PER, 2.0)])
+def test_p10_variable_dt_is_linear_extrapolation_in_time(oracle_mod, bc, r):
+    """p_hat = (1 + r) p^n - r p^(n-1), r = dt^(n+1)/dt^n, is the straight line through
+    (t^(n-1), p^(n-1)) and (t^n, p^n) evaluated at t^(n+1).  So for a history p(t) = A + t B sampled at
+    t^(n-1) = -dt_n and t^n = 0, the step with ratio r must equal the CONSTANT-dt step fed the history
+    resampled at -dt_(n+1) (whose 2 p^n - p^(n-1) is the same p(t^(n+1)) = A + dt_(n+1) B); a wrong sign,
+    a swapped coefficient or an inverted ratio all change p_hat by O(1) and fail this."""
+    W = wl.random_case(10, 12, 8, bc, 20.0, 52)
+    rng = np.random.default_rng(53)
+    A, B = rng.uniform(-0.1, 0.1, W.shape), rng.uniform(-30.0, 30.0, W.shape)
+    dt_new = W.dt
+    dt_old = dt_new / r
+    p_n, p_nm1 = A, A - dt_old * B
+    got = oracle_mod.projection_step(W.u, W.v, W.w, W.phi, p_n, p_nm1, W.box, bc, W.rho1, W.rho2, dt_new,
+                                     return_rhs=True, dt_ratio=r)
+    want = oracle_mod.projection_step(W.u, W.v, W.w, W.phi, p_n, A - dt_new * B, W.box, bc, W.rho1, W.rho2,
+                                      dt_new, return_rhs=True)
+    for x, y in zip(got, want):
+        assert ops.rel_l2(x, y) < 1e-12
+    # and the two histories really differ: with the wrong ratio the result moves by far more than round-off
+    wrong = oracle_mod.projection_step(W.u, W.v, W.w, W.phi, p_n, p_nm1, W.box, bc, W.rho1, W.rho2, dt_new,
+                                       dt_ratio=1.0 / r)
+    assert ops.rel_l2(wrong[3], want[3]) > 1e-6
+
+
+def test_p10_fixed_point_and_divfree_hold_for_any_ratio(oracle_mod):
+    """p_old = p makes p_hat = p for every r, so the steady state of P3b is a fixed point for every r;
+    div u^(n+1) = 0 holds for every r because rhs and correction share the same p_hat."""
+    bc, ratio, r = WALL, 100.0, 0.37
+    W = wl.random_case(12, 10, 8, bc, ratio, 54)
+    ut, vt, wt, _ = oracle_mod.projection_step(W.u, W.v, W.w, W.phi, W.p, W.p_old, W.box, bc, 1.0, 1.0, W.dt)
+    p = W.p - W.p.mean()
+    rx, ry, rz = ops.face_density(W.phi, W.rho1, W.rho2, True)
+    gx, gy, gz = ops.grad(p, W.box, True)
+    us, vs, ws = ut + W.dt * gx / rx, vt + W.dt * gy / ry, wt + W.dt * gz / rz
+    u, v, w, pn = oracle_mod.projection_step(us, vs, ws, W.phi, p, p, W.box, bc, W.rho1, W.rho2, W.dt, dt_ratio=r)
+    assert ops.rel_l2(pn, p) < 1e-10
+    for a, b in ((u, ut), (v, vt), (w, wt)):
+        assert ops.rel_l2(a, b) < 1e-12
+    u, v, w, _ = _step(oracle_mod, W, dt_ratio=r)
+    d0, d1 = ops.div(W.u, W.v, W.w, W.box, True), ops.div(u, v, w, W.box, True)
+    assert np.linalg.norm(d1) / np.linalg.norm(d0) < 1e-12
 
 
 # ------------------------------------------------------ P9: independent numpy restatement
