@@ -74,6 +74,23 @@ flutas_plan *flutas_plan_create(int nx, int ny, int nz, double lx, double ly, do
 int flutas_projection_step(flutas_plan *plan, double *u, double *v, double *w, const double *phi,
                            double *p, const double *p_old, double dt, void *stream);
 
+/* The time-stepping form of the same step:
+ *   dt_ratio = r = dt^(n+1) / dt^n > 0 selects the variable-time-step extrapolation
+ *              p_hat = (1 + r) p^n - r p^(n-1)   (r = 1: p_hat = 2 p^n - p^(n-1), the call above, bit for bit);
+ *              dt = dt^(n+1).
+ *   p_out    receives p^(n+1) (zero mean).  It may be
+ *              == p      in place (what flutas_projection_step does),
+ *              == p_old  ping-pong: a time loop then just swaps the two pointers for the next step
+ *                        (p^(n-1) is dead once the right-hand side has been formed) -- no copy of p per step,
+ *              or a seventh array (p and p_old are then left untouched).
+ *            Any other overlap between the seven arrays is FLUTAS_ERR_ALIAS.
+ * Everything else as flutas_projection_step.  The call only enqueues kernels on `stream` (no allocation,
+ * no synchronisation, no host<->device copy), so it may be recorded into a CUDA graph by stream capture
+ * (per-kernel timing must be off while capturing). */
+int flutas_projection_step_ex(flutas_plan *plan, double *u, double *v, double *w, const double *phi,
+                              const double *p, const double *p_old, double *p_out, double dt,
+                              double dt_ratio, void *stream);
+
 /* The same step for HOST arrays (same layout; pinned memory makes the copies asynchronous):
  * copies the six inputs host->device into plan-owned staging buffers (allocated on first use,
  * 6 fields), runs flutas_projection_step, copies u, v, w, p back and SYNCHRONISES `stream`.
@@ -92,6 +109,11 @@ void flutas_plan_destroy(flutas_plan *plan);
 int flutas_splitting_rhs(flutas_plan *plan, const double *u, const double *v, const double *w,
                          const double *phi, const double *p, const double *p_old, double dt,
                          double *rhs_out, void *stream);
+
+/* flutas_splitting_rhs with the variable-time-step p_hat (dt_ratio as in flutas_projection_step_ex). */
+int flutas_splitting_rhs_ex(flutas_plan *plan, const double *u, const double *v, const double *w,
+                            const double *phi, const double *p, const double *p_old, double dt,
+                            double dt_ratio, double *rhs_out, void *stream);
 
 /* Part (b) alone: solve L p = rhs in the zero-mean gauge.  rhs and p_out are
  * N doubles on the device; p_out may alias rhs. */

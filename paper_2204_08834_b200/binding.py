@@ -20,6 +20,10 @@ lib.flutas_plan_destroy.argtypes = [_vp]
 lib.flutas_plan_destroy.restype = None
 lib.flutas_projection_step.argtypes = [_vp] * 7 + [_cd, _vp]
 lib.flutas_projection_step.restype = _ci
+lib.flutas_projection_step_ex.argtypes = [_vp] * 8 + [_cd, _cd, _vp]
+lib.flutas_projection_step_ex.restype = _ci
+lib.flutas_splitting_rhs_ex.argtypes = [_vp] * 7 + [_cd, _cd, _vp, _vp]
+lib.flutas_splitting_rhs_ex.restype = _ci
 lib.flutas_projection_step_host.argtypes = [_vp] * 7 + [_cd, _vp]
 lib.flutas_projection_step_host.restype = _ci
 lib.flutas_splitting_rhs.argtypes = [_vp] * 7 + [_cd, _vp, _vp]
@@ -50,6 +54,7 @@ EXPORTS = [
     "flutas_splitting_rhs", "flutas_poisson_solve", "flutas_last_error", "flutas_last_error_code",
     "flutas_plan_workspace_bytes", "flutas_plan_kernel_launches", "flutas_plan_kernel_name",
     "flutas_plan_set_timing", "flutas_plan_read_timing", "flutas_plan_kernel_bytes", "flutas_plan_set_option",
+    "flutas_projection_step_ex", "flutas_splitting_rhs_ex",
 ]
 
 
@@ -109,6 +114,17 @@ class Plan:
     def projection_step(self, u, v, w, phi, p, p_old, dt, stream=None):
         ptrs = [_dev_ptr(t, self.npts) for t in (u, v, w, phi, p, p_old)]
         _check(lib.flutas_projection_step(self._h, *ptrs, float(dt), _stream() if stream is None else stream))
+
+    # --- time-stepping form: variable dt (dt_ratio = dt_new / dt_old) and p_out = p | p_old | a seventh tensor
+    def projection_step_ex(self, u, v, w, phi, p, p_old, p_out, dt, dt_ratio=1.0, stream=None):
+        ptrs = [_dev_ptr(t, self.npts) for t in (u, v, w, phi, p, p_old, p_out)]
+        _check(lib.flutas_projection_step_ex(self._h, *ptrs, float(dt), float(dt_ratio),
+                                             _stream() if stream is None else stream))
+
+    def splitting_rhs_ex(self, u, v, w, phi, p, p_old, dt, dt_ratio, rhs_out, stream=None):
+        ptrs = [_dev_ptr(t, self.npts) for t in (u, v, w, phi, p, p_old)]
+        _check(lib.flutas_splitting_rhs_ex(self._h, *ptrs, float(dt), float(dt_ratio),
+                                           _dev_ptr(rhs_out, self.npts), _stream() if stream is None else stream))
 
     # --- the step for host arrays (numpy float64 or pinned torch CPU tensors), in place, synchronous
     def projection_step_host(self, u, v, w, phi, p, p_old, dt, stream=None):

@@ -156,7 +156,7 @@ static int plan_build(flutas_plan *pl) {
     const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
     const double dx = pl->lx / nx, dy = pl->ly / ny, dz = pl->lz / nz;
     pl->grid = GridParams{nx, ny, nz, wall ? 1 : 0, 1.0 / dx, 1.0 / dy, 1.0 / dz, pl->rho1, pl->rho2,
-                          pl->rho1 < pl->rho2 ? pl->rho1 : pl->rho2};
+                          pl->rho1 < pl->rho2 ? pl->rho1 : pl->rho2, 2.0, 1.0};
     pl->n2 = nx / 2;
     pl->nxh = nx / 2 + 1;
     pl->pitch = nx / 2 + 8;
@@ -522,7 +522,10 @@ static int check_launch(cudaError_t e, const char *what) {
 }
 
 static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
-                       const double *p, const double *po, double dt, double *rhs, cudaStream_t st) {
+                       const double *p, const double *po, double dt, double dt_ratio, double *rhs, cudaStream_t st) {
+    GridParams g = pl->grid;
+    g.c_pn = 1.0 + dt_ratio;    // p_hat = (1 + r) p^n - r p^(n-1)
+    g.c_po = dt_ratio;
     // block = (bx threads x 2 points) x ty rows; nx/2 and ny are powers of two, so the grid divides evenly
     const int bx = pl->nx / 2 < pl->rhs_bx ? pl->nx / 2 : pl->rhs_bx;
     int ty = 256 / bx;
@@ -530,11 +533,11 @@ static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const 
     const int kc = pl->rhs_kc < pl->nz ? pl->rhs_kc : pl->nz;
     dim3 block(bx, ty), grid(pl->nx / 2 / bx, pl->ny / ty, (pl->nz + kc - 1) / kc);
     if (pl->rhs_variant == 1)
-        splitting_rhs_kernel<<<grid, block, 0, st>>>(pl->grid, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+        splitting_rhs_kernel<<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
     else if (pl->bc_z == FLUTAS_BC_Z_WALL)
-        splitting_rhs_kernel2<true><<<grid, block, 0, st>>>(pl->grid, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+        splitting_rhs_kernel2<true><<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
     else
-        splitting_rhs_kernel2<false><<<grid, block, 0, st>>>(pl->grid, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+        splitting_rhs_kernel2<false><<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
     return check_launch(cudaGetLastError(), "splitting_rhs");
 }
 
@@ -618,38 +621,59 @@ static int check_fields(const flutas_plan *pl, const void *const *ptrs, int n) {
     return FLUTAS_OK;
 }
 
-extern "C" int flutas_projection_step(flutas_plan *pl, double *u, double *v, double *w, const double *phi, double *p,
-                                      const double *p_old, double dt, void *stream) {
+// p_out may be p (in place) or p_old (ping-pong) exactly, or a seventh field; anything else must not overlap
+static int check_step_fields(const flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
+                             const double *p, const double *p_old, const double *p_out) {
+    const void *ptrs[7] = {u, v, w, phi, p, p_old, p_out};
+    const int n = (p_out == p || p_out == p_old) ? 6 : 7;
+    return check_fields(pl, ptrs, n);
+}
+
+extern "C" int flutas_projection_step_ex(flutas_plan *pl, double *u, double *v, double *w, const double *phi,
+                                         const double *p, const double *p_old, double *p_out, double dt,
+                                         double dt_ratio, void *stream) {
     if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail(FLUTAS_ERR_INVALID_ARG, "dt must be positive and finite");
-    const void *ptrs[6] = {u, v, w, phi, p, p_old};
-    if (int rc = check_fields(pl, ptrs, 6)) return rc;
+    if (!(dt_ratio > 0.0) || !std::isfinite(dt_ratio)) return fail(FLUTAS_ERR_INVALID_ARG, "dt_ratio must be positive and finite");
+    if (int rc = check_step_fields(pl, u, v, w, phi, p, p_old, p_out)) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     StepTimer tm(pl, st);
     tm.mark();
-    if (int rc = enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, pl->rhs, st)) return rc;
+    if (int rc = enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, dt_ratio, pl->rhs, st)) return rc;
     tm.mark();
     if (int rc = check_launch(launch_r2c(pl, pl->rhs, st), "fft_x_r2c")) return rc;
     tm.mark();
     if (int rc = enqueue_solve_core(pl, st, &tm)) return rc;
-    // p, p_old and phi are dead after the RHS kernel: p^(n+1) goes straight into the caller's p
-    if (int rc = check_launch(launch_c2r(pl, p, norm_scale(pl), st), "fft_x_c2r")) return rc;
+    // p, p_old and phi are dead after the RHS kernel: p^(n+1) may go straight into either of them
+    if (int rc = check_launch(launch_c2r(pl, p_out, norm_scale(pl), st), "fft_x_c2r")) return rc;
     tm.mark();
     const unsigned nb = (unsigned)((pl->npts + 255) / 256);
-    correction_kernel<<<nb, 256, 0, st>>>(pl->grid, dt, p, pl->up, pl->vp, pl->wp, u, v, w);
+    correction_kernel<<<nb, 256, 0, st>>>(pl->grid, dt, p_out, pl->up, pl->vp, pl->wp, u, v, w);
     if (int rc = check_launch(cudaGetLastError(), "correction")) return rc;
     tm.mark();
     tm.done();
     return FLUTAS_OK;
 }
 
-extern "C" int flutas_splitting_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
-                                    const double *p, const double *p_old, double dt, double *rhs_out, void *stream) {
+extern "C" int flutas_projection_step(flutas_plan *pl, double *u, double *v, double *w, const double *phi, double *p,
+                                      const double *p_old, double dt, void *stream) {
+    return flutas_projection_step_ex(pl, u, v, w, phi, p, p_old, p, dt, 1.0, stream);
+}
+
+extern "C" int flutas_splitting_rhs_ex(flutas_plan *pl, const double *u, const double *v, const double *w,
+                                       const double *phi, const double *p, const double *p_old, double dt,
+                                       double dt_ratio, double *rhs_out, void *stream) {
     if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail(FLUTAS_ERR_INVALID_ARG, "dt must be positive and finite");
+    if (!(dt_ratio > 0.0) || !std::isfinite(dt_ratio)) return fail(FLUTAS_ERR_INVALID_ARG, "dt_ratio must be positive and finite");
     const void *ptrs[7] = {u, v, w, phi, p, p_old, rhs_out};
     if (int rc = check_fields(pl, ptrs, 7)) return rc;
-    return enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, rhs_out, (cudaStream_t)stream);
+    return enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, dt_ratio, rhs_out, (cudaStream_t)stream);
+}
+
+extern "C" int flutas_splitting_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
+                                    const double *p, const double *p_old, double dt, double *rhs_out, void *stream) {
+    return flutas_splitting_rhs_ex(pl, u, v, w, phi, p, p_old, dt, 1.0, rhs_out, stream);
 }
 
 extern "C" int flutas_poisson_solve(flutas_plan *pl, const double *rhs, double *p_out, void *stream) {
