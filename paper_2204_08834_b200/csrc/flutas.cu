@@ -11,6 +11,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "kernels_rhs.cuh"
 #include "kernels_tma.cuh"
 #include "kernels_x.cuh"
 
@@ -66,7 +67,7 @@ struct flutas_plan {
     int y_cols, z_cols;          // tile width (columns of kx) of the strided passes
     int rhs_kc;                  // planes one thread of the RHS kernel marches through
     int x_variant;               // x transforms: 1 = persistent bulk-copy-fed kernels (nx = 128..1024), 0 = staged kernels
-    int rhs_variant, rhs_bx;     // 2 = software-pipelined kernel (default), 1 = first form; threads along x per block
+    int rhs_variant, rhs_bx;     // 3 = bulk-copy-fed kernel (default), 2 = software-pipelined register form, 1 = first form; threads along x per block (forms 1, 2)
     int use_tma;                 // strided passes: 1 = TMA prefetch + register-resident twiddles (default), 2 = generic TMA in/out, 0 = plain loads
     int num_sms;
     CUtensorMap map_y, map_z;    // boxes {2*y_cols, rows, 1} and {2*z_cols, 1, rows} over the half-spectrum
@@ -210,7 +211,7 @@ static int plan_build(flutas_plan *pl) {
     pl->y_cols = ny >= 1024 ? 4 : 8;
     pl->z_cols = nz >= 1024 ? 4 : 8;
     pl->rhs_kc = 32;
-    pl->rhs_variant = 2;
+    pl->rhs_variant = 3;   // falls back to the second form when nx % 128 or ny % 4 is non-zero
     pl->x_variant = 1;
     pl->rhs_bx = 64;
     pl->use_tma = 1;
@@ -305,7 +306,7 @@ extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int val
     if (!strcmp(name, "tma") && value >= 0 && value <= 2) { pl->use_tma = value; return FLUTAS_OK; }
     if (!strcmp(name, "rhs_kc") && value >= 1) { pl->rhs_kc = value; return FLUTAS_OK; }
     if (!strcmp(name, "x_variant") && (value == 0 || value == 1)) { pl->x_variant = value; return FLUTAS_OK; }
-    if (!strcmp(name, "rhs_variant") && (value == 1 || value == 2)) { pl->rhs_variant = value; return FLUTAS_OK; }
+    if (!strcmp(name, "rhs_variant") && value >= 1 && value <= 3) { pl->rhs_variant = value; return FLUTAS_OK; }
     if (!strcmp(name, "rhs_bx") && (value == 8 || value == 16 || value == 32 || value == 64 || value == 128)) { pl->rhs_bx = value; return FLUTAS_OK; }
     return fail(FLUTAS_ERR_INVALID_ARG, "unknown option or value: %s = %d", name, value);
 }
@@ -532,6 +533,14 @@ static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const 
     if (ty > pl->ny) ty = pl->ny;
     const int kc = pl->rhs_kc < pl->nz ? pl->rhs_kc : pl->nz;
     dim3 block(bx, ty), grid(pl->nx / 2 / bx, pl->ny / ty, (pl->nz + kc - 1) / kc);
+    if (pl->rhs_variant == 3 && pl->nx % Rhs3Geom::X == 0 && pl->ny % Rhs3Geom::TY == 0) {
+        // bulk-copy-fed form: tile = 128 x 4 cells, three plane slabs in shared memory
+        const dim3 b3(Rhs3Geom::NTX, Rhs3Geom::TY), g3(pl->nx / Rhs3Geom::X, pl->ny / Rhs3Geom::TY, (pl->nz + kc - 1) / kc);
+        auto k3 = pl->bc_z == FLUTAS_BC_Z_WALL ? splitting_rhs_kernel3<true> : splitting_rhs_kernel3<false>;
+        if (set_smem(k3, Rhs3Geom::SMEM) != cudaSuccess) return check_launch(cudaGetLastError(), "splitting_rhs attr");
+        k3<<<g3, b3, Rhs3Geom::SMEM, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+        return check_launch(cudaGetLastError(), "splitting_rhs");
+    }
     if (pl->rhs_variant == 1)
         splitting_rhs_kernel<<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
     else if (pl->bc_z == FLUTAS_BC_Z_WALL)
