@@ -12,6 +12,7 @@
 
 #include "kernels.cuh"
 #include "kernels_rhs.cuh"
+#include "kernels_thomas.cuh"
 #include "kernels_tma.cuh"
 #include "kernels_x.cuh"
 
@@ -57,6 +58,9 @@ struct flutas_plan {
     // device workspace
     double2 *spec;
     double *rhs, *up, *vp, *wp, *cp;
+    double *ttab;                // wall: elimination coefficients of the one-pass solve, [tile][j][8] (kernels_thomas.cuh)
+    int thomas_warps;            // solving warps per CTA of the one-pass kernel (1 or 2)
+    int thomas_variant;          // wall: 1 = one-pass shared-memory solve (nz <= 512), 0 = two sweeps through HBM
     size_t bytes;
     // staging for the host entry point
     double *stage[6];
@@ -67,6 +71,12 @@ struct flutas_plan {
     int y_cols, z_cols;          // tile width (columns of kx) of the strided passes
     int rhs_kc;                  // planes one thread of the RHS kernel marches through
     int x_variant;               // x transforms: 1 = persistent bulk-copy-fed kernels (nx = 128..1024), 0 = staged kernels
+    int chunk;                   // planes per launch group of the step (0 = whole grid per kernel)
+    int overlap;                 // chunked only: 1 = the three kernels of a group run on three internal streams (low, mid, high
+                                 // priority; producer -> consumer), so groups overlap and tails are filled
+    cudaStream_t lane[3];        // internal streams, created on first use
+    cudaEvent_t ev_fork, *ev_dep;   // fork from the caller's stream; ev_dep[2 * chunk_index + {0, 1}]
+    int n_dep;
     int rhs_variant, rhs_bx;     // 3 = bulk-copy-fed kernel (default), 2 = software-pipelined register form, 1 = first form; threads along x per block (forms 1, 2)
     int use_tma;                 // strided passes: 1 = TMA prefetch + register-resident twiddles (default), 2 = generic TMA in/out, 0 = plain loads
     int num_sms;
@@ -147,8 +157,11 @@ static int make_spectrum_map(flutas_plan *pl, CUtensorMap *map, int cols, int li
 
 static int plan_make_maps(flutas_plan *pl) {
     if (int rc = make_spectrum_map(pl, &pl->map_y, pl->y_cols, 1, pl->ny)) return rc;
-    if (pl->bc_z == FLUTAS_BC_Z_PERIODIC)
+    if (pl->bc_z == FLUTAS_BC_Z_PERIODIC) {
         if (int rc = make_spectrum_map(pl, &pl->map_z, pl->z_cols, 2, pl->nz)) return rc;
+    } else if (pl->thomas_variant == 1) {
+        if (int rc = make_spectrum_map(pl, &pl->map_z, ThomasGeom::C, 2, pl->nz)) return rc;
+    }
     return FLUTAS_OK;
 }
 
@@ -194,8 +207,22 @@ static int plan_build(flutas_plan *pl) {
     CUDA_TRY(cudaMalloc((void **)&pl->wp, fb));
     pl->bytes += sb + 4 * fb;
     if (wall) {
-        CUDA_TRY(cudaMalloc((void **)&pl->cp, sb / 2));
-        pl->bytes += sb / 2;
+        pl->thomas_variant = ThomasGeom::smem_bytes(nz) <= 227 * 1024 ? 1 : 0;
+        pl->thomas_warps = 2;
+        if (pl->thomas_variant == 1) {
+            const int n_tiles_x = (pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C;
+            const size_t tb = sizeof(double) * ThomasGeom::tab_doubles(nz) * (size_t)n_tiles_x * ny;
+            CUDA_TRY(cudaMalloc((void **)&pl->ttab, tb));
+            pl->bytes += tb;
+            const long long ncol = (long long)n_tiles_x * ny * ThomasGeom::C;
+            thomas_table_kernel<<<(unsigned)((ncol + 127) / 128), 128>>>(pl->ttab, n_tiles_x, ny, nz, pl->nxh, pl->lam_x, pl->lam_y,
+                                                                       1.0 / (dz * dz));
+            CUDA_TRY(cudaGetLastError());
+            CUDA_TRY(cudaDeviceSynchronize());
+        } else {
+            CUDA_TRY(cudaMalloc((void **)&pl->cp, sb / 2));
+            pl->bytes += sb / 2;
+        }
     }
 
     int n = 0;
@@ -266,8 +293,14 @@ extern "C" void flutas_plan_destroy(flutas_plan *pl) {
     cudaDeviceSynchronize();
     cudaFree(pl->tw_x); cudaFree(pl->tw_y); cudaFree(pl->tw_z);
     cudaFree(pl->lam_x); cudaFree(pl->lam_y); cudaFree(pl->lam_z);
-    cudaFree(pl->spec); cudaFree(pl->rhs); cudaFree(pl->up); cudaFree(pl->vp); cudaFree(pl->wp); cudaFree(pl->cp);
+    cudaFree(pl->spec); cudaFree(pl->rhs); cudaFree(pl->up); cudaFree(pl->vp); cudaFree(pl->wp); cudaFree(pl->cp); cudaFree(pl->ttab);
     for (int i = 0; i < 6; ++i) cudaFree(pl->stage[i]);
+    for (int i = 0; i < 3; ++i) if (pl->lane[i]) cudaStreamDestroy(pl->lane[i]);
+    if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
+    if (pl->ev_dep) {
+        for (int i = 0; i < pl->n_dep; ++i) cudaEventDestroy(pl->ev_dep[i]);
+        delete[] pl->ev_dep;
+    }
     if (pl->events) {
         for (int i = 0; i < kMaxPendingSteps * (pl->n_launch + 1); ++i) cudaEventDestroy(pl->events[i]);
         delete[] pl->events;
@@ -291,7 +324,11 @@ extern "C" double flutas_plan_kernel_bytes(const flutas_plan *pl, int idx) {
         case K_RHS: return 6 * f + 4 * f;          // read u*,v*,w*,phi,p,p_old; write rhs,u',v',w'
         case K_FFTX: return f + s;                 // read rhs, write spectrum
         case K_FFTY: case K_IFFTY: return 2 * s;   // read + write spectrum
-        case K_Z: return pl->bc_z == FLUTAS_BC_Z_WALL ? 4 * s + 2 * (s / 2) : 2 * s;  // Thomas: two sweeps + c'
+        case K_Z:
+            if (pl->bc_z != FLUTAS_BC_Z_WALL) return 2 * s;
+            if (pl->thomas_variant == 1)   // one pass + the coefficient table (one double per column and half the planes)
+                return 2 * s + 8.0 * ThomasGeom::tab_doubles(pl->nz) * ((pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C) * pl->ny;
+            return 4 * s + 2 * (s / 2);    // two sweeps + c'
         case K_ZS: return 2.0 * 16.0 * pl->nz;
         case K_IFFTX: return s + f;                // read spectrum, write p
         case K_CORR: return 4 * f + 3 * f;         // read p,u',v',w'; write u,v,w
@@ -304,6 +341,17 @@ extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int val
     if (!strcmp(name, "y_cols") && (value == 4 || (value == 8 && pl->ny < 2048))) { pl->y_cols = value; return plan_make_maps(pl); }
     if (!strcmp(name, "z_cols") && (value == 4 || (value == 8 && pl->nz < 2048))) { pl->z_cols = value; return plan_make_maps(pl); }
     if (!strcmp(name, "tma") && value >= 0 && value <= 2) { pl->use_tma = value; return FLUTAS_OK; }
+    if (!strcmp(name, "thomas") && pl->bc_z == FLUTAS_BC_Z_WALL && (value == 0 || (value == 1 && pl->ttab))) {
+        if (value == 0 && !pl->cp) {   // the two-sweep kernel keeps c' in a half-spectrum of its own
+            CUDA_TRY(cudaMalloc((void **)&pl->cp, sizeof(double) * (size_t)pl->nspec));
+            pl->bytes += sizeof(double) * (size_t)pl->nspec;
+        }
+        pl->thomas_variant = value;
+        return FLUTAS_OK;
+    }
+    if (!strcmp(name, "thomas_warps") && (value == 1 || value == 2)) { pl->thomas_warps = value; return FLUTAS_OK; }
+    if (!strcmp(name, "chunk") && value >= 0) { pl->chunk = value; return FLUTAS_OK; }
+    if (!strcmp(name, "overlap") && (value == 0 || value == 1)) { pl->overlap = value; return FLUTAS_OK; }
     if (!strcmp(name, "rhs_kc") && value >= 1) { pl->rhs_kc = value; return FLUTAS_OK; }
     if (!strcmp(name, "x_variant") && (value == 0 || value == 1)) { pl->x_variant = value; return FLUTAS_OK; }
     if (!strcmp(name, "rhs_variant") && value >= 1 && value <= 3) { pl->rhs_variant = value; return FLUTAS_OK; }
@@ -401,9 +449,12 @@ static cudaError_t launch_tma_n(int cols, const CUtensorMap &map, TmaFftArgs a, 
     else return launch_tma_nc<N, 8, MODE>(map, a, a1, variant, num_sms, st);
 }
 template <int MODE>
-static cudaError_t launch_tma(int n, int cols, const CUtensorMap &map, const TmaFftArgs &a, long long row_stride,
-                              long long outer_stride, double2 *data, int variant, cudaStream_t st, int num_sms) {
+static cudaError_t launch_tma(int n, int cols, const CUtensorMap &map, TmaFftArgs a, long long row_stride,
+                              long long outer_stride, double2 *data, int variant, cudaStream_t st, int num_sms,
+                              int outer0, int n_outer) {
+    a.outer0 = outer0; a.n_outer = n_outer;
     Tma1Args a1{};
+    a1.outer0 = outer0;
     a1.data = data; a1.row_stride = row_stride; a1.outer_stride = outer_stride;
     a1.n_outer = a.n_outer; a1.line_dim = a.line_dim; a1.nxh = a.nxh; a1.tw = a.tw;
     a1.lam_x = a.lam_x; a1.lam_outer = a.lam_outer; a1.lam_pos = a.lam_pos;
@@ -421,26 +472,26 @@ static cudaError_t launch_tma(int n, int cols, const CUtensorMap &map, const Tma
     return cudaErrorInvalidValue;
 }
 
-template <int N2> static cudaError_t launch_r2c_n(const flutas_plan *pl, const double *rhs, cudaStream_t st) {
+template <int N2> static cudaError_t launch_r2c_n(const flutas_plan *pl, const double *rhs, cudaStream_t st, long long tile0, long long ntiles) {
     constexpr int NT = clamp_nt(N2);
     const size_t smem = sizeof(double2) * (size_t)(N2 + 1) * 8;
     auto kern = fft_x_r2c_kernel<N2, NT>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
-    kern<<<(unsigned)((long long)pl->ny * pl->nz / 8), NT, smem, st>>>(rhs, pl->spec, pl->tw_x);
+    kern<<<(unsigned)ntiles, NT, smem, st>>>(rhs + tile0 * 8 * 2 * N2, pl->spec + tile0 * 8 * (N2 + 8), pl->tw_x);
     return cudaGetLastError();
 }
-template <int N2> static cudaError_t launch_c2r_n(const flutas_plan *pl, double *out, double scale, cudaStream_t st) {
+template <int N2> static cudaError_t launch_c2r_n(const flutas_plan *pl, double *out, double scale, cudaStream_t st, long long tile0, long long ntiles) {
     constexpr int NT = clamp_nt(N2);
     const size_t smem = sizeof(double2) * (size_t)(N2 + 1) * 8;
     auto kern = fft_x_c2r_kernel<N2, NT>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
-    kern<<<(unsigned)((long long)pl->ny * pl->nz / 8), NT, smem, st>>>(pl->spec, out, pl->tw_x, scale);
+    kern<<<(unsigned)ntiles, NT, smem, st>>>(pl->spec + tile0 * 8 * (N2 + 8), out + tile0 * 8 * 2 * N2, pl->tw_x, scale);
     return cudaGetLastError();
 }
 // persistent bulk-copy-fed x kernels (nx = 128 .. 1024)
-template <int N2> static cudaError_t launch_r2c_tma_n(const flutas_plan *pl, const double *rhs, cudaStream_t st) {
+template <int N2> static cudaError_t launch_r2c_tma_n(const flutas_plan *pl, const double *rhs, cudaStream_t st, long long tile0, long long ntiles) {
     const size_t smem = (size_t)2 * 8 * N2 * 16 + 128;
     auto kern = fft_x_r2c_tma_kernel<N2>;
     cudaError_t e = set_smem(kern, smem);
@@ -449,13 +500,12 @@ template <int N2> static cudaError_t launch_r2c_tma_n(const flutas_plan *pl, con
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, N2, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
-    const long long ntiles = (long long)pl->ny * pl->nz / 8;
     long long grid = (long long)pl->num_sms * per_sm;
     if (grid > ntiles) grid = ntiles;
-    kern<<<(unsigned)grid, N2, smem, st>>>(rhs, pl->spec, pl->tw_x, (int)ntiles);
+    kern<<<(unsigned)grid, N2, smem, st>>>(rhs + tile0 * 8 * 2 * N2, pl->spec + tile0 * 8 * (N2 + 8), pl->tw_x, (int)ntiles);
     return cudaGetLastError();
 }
-template <int N2> static cudaError_t launch_c2r_tma_n(const flutas_plan *pl, double *out, double scale, cudaStream_t st) {
+template <int N2> static cudaError_t launch_c2r_tma_n(const flutas_plan *pl, double *out, double scale, cudaStream_t st, long long tile0, long long ntiles) {
     const size_t smem = (size_t)8 * (N2 + 8) * 16 + (size_t)8 * N2 * 16 + 128;
     auto kern = fft_x_c2r_tma_kernel<N2>;
     cudaError_t e = set_smem(kern, smem);
@@ -464,37 +514,39 @@ template <int N2> static cudaError_t launch_c2r_tma_n(const flutas_plan *pl, dou
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, N2, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
-    const long long ntiles = (long long)pl->ny * pl->nz / 8;
     long long grid = (long long)pl->num_sms * per_sm;
     if (grid > ntiles) grid = ntiles;
-    kern<<<(unsigned)grid, N2, smem, st>>>(pl->spec, out, pl->tw_x, scale, (int)ntiles);
+    kern<<<(unsigned)grid, N2, smem, st>>>(pl->spec + tile0 * 8 * (N2 + 8), out + tile0 * 8 * 2 * N2, pl->tw_x, scale, (int)ntiles);
     return cudaGetLastError();
 }
 #define FOR_EACH_N2_TMA(X) X(64) X(128) X(256) X(512)
 #define FOR_EACH_N2(X) X(8) X(16) X(32) X(64) X(128) X(256) X(512) X(1024)
-static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStream_t st) {
+// planes k0 .. k1 - 1 (a tile is 8 consecutive x-lines; ny is a multiple of 8)
+static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStream_t st, int k0, int k1) {
+    const long long tile0 = (long long)k0 * pl->ny / 8, ntiles = (long long)(k1 - k0) * pl->ny / 8;
     if (pl->x_variant == 1)
         switch (pl->n2) {
-#define X(n) case n: return launch_r2c_tma_n<n>(pl, rhs, st);
+#define X(n) case n: return launch_r2c_tma_n<n>(pl, rhs, st, tile0, ntiles);
             FOR_EACH_N2_TMA(X)
 #undef X
         }
     switch (pl->n2) {
-#define X(n) case n: return launch_r2c_n<n>(pl, rhs, st);
+#define X(n) case n: return launch_r2c_n<n>(pl, rhs, st, tile0, ntiles);
         FOR_EACH_N2(X)
 #undef X
     }
     return cudaErrorInvalidValue;
 }
-static cudaError_t launch_c2r(const flutas_plan *pl, double *out, double scale, cudaStream_t st) {
+static cudaError_t launch_c2r(const flutas_plan *pl, double *out, double scale, cudaStream_t st, int k0, int k1) {
+    const long long tile0 = (long long)k0 * pl->ny / 8, ntiles = (long long)(k1 - k0) * pl->ny / 8;
     if (pl->x_variant == 1)
         switch (pl->n2) {
-#define X(n) case n: return launch_c2r_tma_n<n>(pl, out, scale, st);
+#define X(n) case n: return launch_c2r_tma_n<n>(pl, out, scale, st, tile0, ntiles);
             FOR_EACH_N2_TMA(X)
 #undef X
         }
     switch (pl->n2) {
-#define X(n) case n: return launch_c2r_n<n>(pl, out, scale, st);
+#define X(n) case n: return launch_c2r_n<n>(pl, out, scale, st, tile0, ntiles);
         FOR_EACH_N2(X)
 #undef X
     }
@@ -522,8 +574,13 @@ static int check_launch(cudaError_t e, const char *what) {
     return FLUTAS_OK;
 }
 
+// planes k0 .. k1 - 1 of rhs, u', v', w' (the bulk-copy-fed form takes any range; the older forms the whole grid)
+static bool rhs_takes_ranges(const flutas_plan *pl) {
+    return pl->rhs_variant == 3 && pl->nx % Rhs3Geom::X == 0 && pl->ny % Rhs3Geom::TY == 0;
+}
 static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
-                       const double *p, const double *po, double dt, double dt_ratio, double *rhs, cudaStream_t st) {
+                       const double *p, const double *po, double dt, double dt_ratio, double *rhs, cudaStream_t st,
+                       int k0, int k1) {
     GridParams g = pl->grid;
     g.c_pn = 1.0 + dt_ratio;    // p_hat = (1 + r) p^n - r p^(n-1)
     g.c_po = dt_ratio;
@@ -531,16 +588,18 @@ static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const 
     const int bx = pl->nx / 2 < pl->rhs_bx ? pl->nx / 2 : pl->rhs_bx;
     int ty = 256 / bx;
     if (ty > pl->ny) ty = pl->ny;
-    const int kc = pl->rhs_kc < pl->nz ? pl->rhs_kc : pl->nz;
-    dim3 block(bx, ty), grid(pl->nx / 2 / bx, pl->ny / ty, (pl->nz + kc - 1) / kc);
-    if (pl->rhs_variant == 3 && pl->nx % Rhs3Geom::X == 0 && pl->ny % Rhs3Geom::TY == 0) {
+    const int nk = k1 - k0;
+    const int kc = pl->rhs_kc < nk ? pl->rhs_kc : nk;
+    dim3 block(bx, ty), grid(pl->nx / 2 / bx, pl->ny / ty, (nk + kc - 1) / kc);
+    if (rhs_takes_ranges(pl)) {
         // bulk-copy-fed form: tile = 128 x 4 cells, three plane slabs in shared memory
-        const dim3 b3(Rhs3Geom::NTX, Rhs3Geom::TY), g3(pl->nx / Rhs3Geom::X, pl->ny / Rhs3Geom::TY, (pl->nz + kc - 1) / kc);
+        const dim3 b3(Rhs3Geom::NTX, Rhs3Geom::TY), g3(pl->nx / Rhs3Geom::X, pl->ny / Rhs3Geom::TY, (nk + kc - 1) / kc);
         auto k3 = pl->bc_z == FLUTAS_BC_Z_WALL ? splitting_rhs_kernel3<true> : splitting_rhs_kernel3<false>;
         if (set_smem(k3, Rhs3Geom::SMEM) != cudaSuccess) return check_launch(cudaGetLastError(), "splitting_rhs attr");
-        k3<<<g3, b3, Rhs3Geom::SMEM, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+        k3<<<g3, b3, Rhs3Geom::SMEM, st>>>(g, dt, kc, k0, k1, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
         return check_launch(cudaGetLastError(), "splitting_rhs");
     }
+    if (k0 != 0 || k1 != pl->nz) return fail(FLUTAS_ERR_INVALID_ARG, "this form of the RHS kernel takes the whole grid");
     if (pl->rhs_variant == 1)
         splitting_rhs_kernel<<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
     else if (pl->bc_z == FLUTAS_BC_Z_WALL)
@@ -550,51 +609,75 @@ static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const 
     return check_launch(cudaGetLastError(), "splitting_rhs");
 }
 
-// spectrum (already holding the x-transformed rhs) -> spectrum of the solution; timer marks between kernels
-static int enqueue_solve_core(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
-    const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
+// transform along y (MODE_FWD or MODE_INV) of planes k0 .. k1 - 1 of the half-spectrum
+template <int MODE> static int enqueue_y(flutas_plan *pl, cudaStream_t st, int k0, int k1) {
+    const char *what = MODE == MODE_FWD ? "fft_y_fwd" : "fft_y_inv";
+    const long long row_stride = pl->pitch, outer_stride = (long long)pl->pitch * pl->ny;
+    if (pl->use_tma) {
+        TmaFftArgs ty{};
+        ty.line_dim = 1;
+        ty.nxh = pl->nxh;
+        ty.tw = pl->tw_y;
+        return check_launch(launch_tma<MODE>(pl->ny, pl->y_cols, pl->map_y, ty, row_stride, outer_stride, pl->spec,
+                                             pl->use_tma, st, pl->num_sms, k0, k1 - k0), what);
+    }
     StridedArgs ay{};
-    ay.data = pl->spec;
-    ay.row_stride = pl->pitch;
-    ay.outer_stride = (long long)pl->pitch * pl->ny;
+    ay.data = pl->spec + (long long)k0 * outer_stride;
+    ay.row_stride = row_stride;
+    ay.outer_stride = outer_stride;
     ay.nxh = pl->nxh;
     ay.tw = pl->tw_y;
-    TmaFftArgs ty{};
-    ty.n_outer = pl->nz;
-    ty.line_dim = 1;
-    ty.nxh = pl->nxh;
-    ty.tw = pl->tw_y;
-    if (pl->use_tma) {
-        if (int rc = check_launch(launch_tma<MODE_FWD>(pl->ny, pl->y_cols, pl->map_y, ty, ay.row_stride, ay.outer_stride, pl->spec, pl->use_tma, st, pl->num_sms), "fft_y_fwd (tma)")) return rc;
-    } else if (int rc = check_launch(launch_strided<MODE_FWD>(pl->ny, pl->y_cols, ay, pl->nxh, pl->nz, st), "fft_y_fwd")) return rc;
-    if (tm) tm->mark();
+    return check_launch(launch_strided<MODE>(pl->ny, pl->y_cols, ay, pl->nxh, k1 - k0, st), what);
+}
+
+// the z stage on the whole half-spectrum (every line along z crosses all planes); timer marks between kernels
+static int enqueue_z(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
+    const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
     if (!wall) {
-        StridedArgs az{};
-        az.data = pl->spec;
-        az.row_stride = (long long)pl->pitch * pl->ny;
-        az.outer_stride = pl->pitch;
-        az.nxh = pl->nxh;
-        az.tw = pl->tw_z;
-        az.lam_x = pl->lam_x;
-        az.lam_outer = pl->lam_y;
-        az.lam_pos = pl->lam_z;
-        TmaFftArgs tz{};
-        tz.n_outer = pl->ny;
-        tz.line_dim = 2;
-        tz.nxh = pl->nxh;
-        tz.tw = pl->tw_z;
-        tz.lam_x = pl->lam_x;
-        tz.lam_outer = pl->lam_y;
-        tz.lam_pos = pl->lam_z;
+        const long long row_stride = (long long)pl->pitch * pl->ny, outer_stride = pl->pitch;
         if (pl->use_tma) {
-            if (int rc = check_launch(launch_tma<MODE_SOLVE>(pl->nz, pl->z_cols, pl->map_z, tz, az.row_stride, az.outer_stride, pl->spec, pl->use_tma, st, pl->num_sms), "z_solve (tma)")) return rc;
-        } else if (int rc = check_launch(launch_strided<MODE_SOLVE>(pl->nz, pl->z_cols, az, pl->nxh, pl->ny, st), "z_solve")) return rc;
+            TmaFftArgs tz{};
+            tz.line_dim = 2;
+            tz.nxh = pl->nxh;
+            tz.tw = pl->tw_z;
+            tz.lam_x = pl->lam_x;
+            tz.lam_outer = pl->lam_y;
+            tz.lam_pos = pl->lam_z;
+            if (int rc = check_launch(launch_tma<MODE_SOLVE>(pl->nz, pl->z_cols, pl->map_z, tz, row_stride, outer_stride, pl->spec,
+                                                             pl->use_tma, st, pl->num_sms, 0, pl->ny), "z_solve (tma)")) return rc;
+        } else {
+            StridedArgs az{};
+            az.data = pl->spec;
+            az.row_stride = row_stride;
+            az.outer_stride = outer_stride;
+            az.nxh = pl->nxh;
+            az.tw = pl->tw_z;
+            az.lam_x = pl->lam_x;
+            az.lam_outer = pl->lam_y;
+            az.lam_pos = pl->lam_z;
+            if (int rc = check_launch(launch_strided<MODE_SOLVE>(pl->nz, pl->z_cols, az, pl->nxh, pl->ny, st), "z_solve")) return rc;
+        }
         if (tm) tm->mark();
     } else {
         const long long ncol = (long long)pl->pitch * pl->ny;
         const double inv_dz2 = pl->grid.inv_dz * pl->grid.inv_dz;
-        thomas_kernel<<<(unsigned)((ncol + 127) / 128), 128, 0, st>>>(pl->spec, pl->cp, pl->pitch, pl->ny, pl->nz, pl->nxh,
-                                                                    pl->lam_x, pl->lam_y, inv_dz2);
+        if (pl->thomas_variant == 1) {
+            ThomasArgs ta{};
+            ta.tab = pl->ttab;
+            ta.n_tiles_x = (pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C;
+            ta.ny = pl->ny;
+            ta.nz = pl->nz;
+            ta.dz2 = 1.0 / inv_dz2;
+            const size_t smem_t = ThomasGeom::smem_bytes(pl->nz);
+            auto kern = pl->thomas_warps == 2 ? thomas_tma_kernel<2> : thomas_tma_kernel<1>;
+            if (set_smem(kern, smem_t) != cudaSuccess) return check_launch(cudaGetLastError(), "z_solve attr");
+            long long grid = pl->num_sms;
+            if (grid > (long long)ta.n_tiles_x * ta.ny) grid = (long long)ta.n_tiles_x * ta.ny;
+            kern<<<(unsigned)grid, 32 * pl->thomas_warps, smem_t, st>>>(pl->map_z, ta);
+        } else {
+            thomas_kernel<<<(unsigned)((ncol + 127) / 128), 128, 0, st>>>(pl->spec, pl->cp, pl->pitch, pl->ny, pl->nz, pl->nxh,
+                                                                        pl->lam_x, pl->lam_y, inv_dz2);
+        }
         if (int rc = check_launch(cudaGetLastError(), "z_solve (thomas)")) return rc;
         if (tm) tm->mark();
         const size_t smem = sizeof(double) * 3 * (size_t)pl->nz;
@@ -604,11 +687,17 @@ static int enqueue_solve_core(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
         if (int rc = check_launch(cudaGetLastError(), "z_singular")) return rc;
         if (tm) tm->mark();
     }
-    if (pl->use_tma) {
-        if (int rc = check_launch(launch_tma<MODE_INV>(pl->ny, pl->y_cols, pl->map_y, ty, ay.row_stride, ay.outer_stride, pl->spec, pl->use_tma, st, pl->num_sms), "fft_y_inv (tma)")) return rc;
-    } else if (int rc = check_launch(launch_strided<MODE_INV>(pl->ny, pl->y_cols, ay, pl->nxh, pl->nz, st), "fft_y_inv")) return rc;
-    if (tm) tm->mark();
     return FLUTAS_OK;
+}
+
+// planes k0 .. k1 - 1 of u, v, w (reads p^(n+1) of planes k0 .. k1, wrapped)
+static int enqueue_correction(flutas_plan *pl, double dt, const double *pn, double *u, double *v, double *w,
+                              cudaStream_t st, int k0, int k1) {
+    if (k1 <= k0) return FLUTAS_OK;
+    const long long plane = (long long)pl->nx * pl->ny, q0 = k0 * plane, q1 = k1 * plane;
+    const unsigned nb = (unsigned)((q1 - q0 + 255) / 256);
+    correction_kernel<<<nb, 256, 0, st>>>(pl->grid, dt, q0, q1, pn, pl->up, pl->vp, pl->wp, u, v, w);
+    return check_launch(cudaGetLastError(), "correction");
 }
 
 static double norm_scale(const flutas_plan *pl) {
@@ -630,6 +719,28 @@ static int check_fields(const flutas_plan *pl, const void *const *ptrs, int n) {
     return FLUTAS_OK;
 }
 
+// internal streams (non-blocking, priorities low / mid / high) and dependency events of the chunked launch order
+static int ensure_lanes(flutas_plan *pl, int nchunk) {
+    if (!pl->lane[0]) {
+        int lo = 0, hi = 0;
+        CUDA_TRY(cudaDeviceGetStreamPriorityRange(&lo, &hi));   // lo = least urgent (numerically largest)
+        const int mid = (lo + hi) / 2;
+        const int prio[3] = {lo, mid, hi};
+        for (int i = 0; i < 3; ++i) CUDA_TRY(cudaStreamCreateWithPriority(&pl->lane[i], cudaStreamNonBlocking, prio[i]));
+        CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
+    }
+    if (pl->n_dep < 2 * nchunk) {
+        cudaEvent_t *ev = new (std::nothrow) cudaEvent_t[2 * nchunk];
+        if (!ev) return fail(FLUTAS_ERR_ALLOC, "host allocation failed");
+        for (int i = 0; i < pl->n_dep; ++i) ev[i] = pl->ev_dep[i];
+        for (int i = pl->n_dep; i < 2 * nchunk; ++i) CUDA_TRY(cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming));
+        delete[] pl->ev_dep;
+        pl->ev_dep = ev;
+        pl->n_dep = 2 * nchunk;
+    }
+    return FLUTAS_OK;
+}
+
 // p_out may be p (in place) or p_old (ping-pong) exactly, or a seventh field; anything else must not overlap
 static int check_step_fields(const flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
                              const double *p, const double *p_old, const double *p_out) {
@@ -647,18 +758,62 @@ extern "C" int flutas_projection_step_ex(flutas_plan *pl, double *u, double *v, 
     if (int rc = check_step_fields(pl, u, v, w, phi, p, p_old, p_out)) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     StepTimer tm(pl, st);
+    const int nz = pl->nz;
+    // planes per launch group: 0 = every kernel covers the whole grid.  With a chunk of a few planes the kernels of one
+    // group run back to back on the same planes, so rhs, the x-transformed spectrum and p^(n+1) are still in L2
+    // when their consumer asks for them ("plane-chunked launch order").
+    const int chunk = (pl->chunk > 0 && pl->chunk < nz && rhs_takes_ranges(pl)) ? pl->chunk : nz;
+    const int nchunk = (nz + chunk - 1) / chunk;
+    const bool lanes = chunk != nz && pl->overlap;
+    cudaStream_t s_lo = st, s_mid = st, s_hi = st;
+    if (lanes) {
+        if (int rc = ensure_lanes(pl, nchunk)) return rc;
+        s_lo = pl->lane[0]; s_mid = pl->lane[1]; s_hi = pl->lane[2];
+        CUDA_TRY(cudaEventRecord(pl->ev_fork, st));
+        CUDA_TRY(cudaStreamWaitEvent(s_lo, pl->ev_fork, 0));
+    }
     tm.mark();
-    if (int rc = enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, dt_ratio, pl->rhs, st)) return rc;
+    for (int c = 0, k0 = 0; k0 < nz; k0 += chunk, ++c) {
+        const int k1 = k0 + chunk < nz ? k0 + chunk : nz;
+        if (int rc = enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, dt_ratio, pl->rhs, s_lo, k0, k1)) return rc;
+        if (chunk == nz) tm.mark();
+        if (lanes) { CUDA_TRY(cudaEventRecord(pl->ev_dep[2 * c], s_lo)); CUDA_TRY(cudaStreamWaitEvent(s_mid, pl->ev_dep[2 * c], 0)); }
+        if (int rc = check_launch(launch_r2c(pl, pl->rhs, s_mid, k0, k1), "fft_x_r2c")) return rc;
+        if (chunk == nz) tm.mark();
+        if (lanes) { CUDA_TRY(cudaEventRecord(pl->ev_dep[2 * c + 1], s_mid)); CUDA_TRY(cudaStreamWaitEvent(s_hi, pl->ev_dep[2 * c + 1], 0)); }
+        if (int rc = enqueue_y<MODE_FWD>(pl, s_hi, k0, k1)) return rc;
+    }
+    if (lanes) {   // the last transform along y depends on every launch of the three lanes
+        CUDA_TRY(cudaEventRecord(pl->ev_fork, s_hi));
+        CUDA_TRY(cudaStreamWaitEvent(st, pl->ev_fork, 0));
+    }
+    if (chunk != nz) { tm.mark(); tm.mark(); }   // chunked: the group's time is booked on its first kernel
     tm.mark();
-    if (int rc = check_launch(launch_r2c(pl, pl->rhs, st), "fft_x_r2c")) return rc;
-    tm.mark();
-    if (int rc = enqueue_solve_core(pl, st, &tm)) return rc;
+    if (int rc = enqueue_z(pl, st, &tm)) return rc;
+    if (lanes) {
+        CUDA_TRY(cudaEventRecord(pl->ev_fork, st));
+        CUDA_TRY(cudaStreamWaitEvent(s_lo, pl->ev_fork, 0));
+    }
     // p, p_old and phi are dead after the RHS kernel: p^(n+1) may go straight into either of them
-    if (int rc = check_launch(launch_c2r(pl, p_out, norm_scale(pl), st), "fft_x_c2r")) return rc;
-    tm.mark();
-    const unsigned nb = (unsigned)((pl->npts + 255) / 256);
-    correction_kernel<<<nb, 256, 0, st>>>(pl->grid, dt, p_out, pl->up, pl->vp, pl->wp, u, v, w);
-    if (int rc = check_launch(cudaGetLastError(), "correction")) return rc;
+    int corrected = 0;   // planes 0 .. corrected - 1 of u, v, w are final
+    for (int c = 0, k0 = 0; k0 < nz; k0 += chunk, ++c) {
+        const int k1 = k0 + chunk < nz ? k0 + chunk : nz;
+        if (int rc = enqueue_y<MODE_INV>(pl, s_lo, k0, k1)) return rc;
+        if (chunk == nz) tm.mark();
+        if (lanes) { CUDA_TRY(cudaEventRecord(pl->ev_dep[2 * c], s_lo)); CUDA_TRY(cudaStreamWaitEvent(s_mid, pl->ev_dep[2 * c], 0)); }
+        if (int rc = check_launch(launch_c2r(pl, p_out, norm_scale(pl), s_mid, k0, k1), "fft_x_c2r")) return rc;
+        if (chunk == nz) tm.mark();
+        if (lanes) { CUDA_TRY(cudaEventRecord(pl->ev_dep[2 * c + 1], s_mid)); CUDA_TRY(cudaStreamWaitEvent(s_hi, pl->ev_dep[2 * c + 1], 0)); }
+        // plane k needs p^(n+1) of plane k + 1: the last plane of a chunk waits for the next chunk
+        const int upto = k1 == nz ? nz : k1 - 1;
+        if (int rc = enqueue_correction(pl, dt, p_out, u, v, w, s_hi, corrected, upto)) return rc;
+        corrected = upto;
+    }
+    if (lanes) {
+        CUDA_TRY(cudaEventRecord(pl->ev_fork, s_hi));
+        CUDA_TRY(cudaStreamWaitEvent(st, pl->ev_fork, 0));
+    }
+    if (chunk != nz) { tm.mark(); tm.mark(); }
     tm.mark();
     tm.done();
     return FLUTAS_OK;
@@ -677,7 +832,7 @@ extern "C" int flutas_splitting_rhs_ex(flutas_plan *pl, const double *u, const d
     if (!(dt_ratio > 0.0) || !std::isfinite(dt_ratio)) return fail(FLUTAS_ERR_INVALID_ARG, "dt_ratio must be positive and finite");
     const void *ptrs[7] = {u, v, w, phi, p, p_old, rhs_out};
     if (int rc = check_fields(pl, ptrs, 7)) return rc;
-    return enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, dt_ratio, rhs_out, (cudaStream_t)stream);
+    return enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, dt_ratio, rhs_out, (cudaStream_t)stream, 0, pl->nz);
 }
 
 extern "C" int flutas_splitting_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
@@ -691,9 +846,11 @@ extern "C" int flutas_poisson_solve(flutas_plan *pl, const double *rhs, double *
     if (rhs == p_out) { if (int rc = check_fields(pl, ptrs, 1)) return rc; }
     else if (int rc = check_fields(pl, ptrs, 2)) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    if (int rc = check_launch(launch_r2c(pl, rhs, st), "fft_x_r2c")) return rc;
-    if (int rc = enqueue_solve_core(pl, st, nullptr)) return rc;
-    return check_launch(launch_c2r(pl, p_out, norm_scale(pl), st), "fft_x_c2r");
+    if (int rc = check_launch(launch_r2c(pl, rhs, st, 0, pl->nz), "fft_x_r2c")) return rc;
+    if (int rc = enqueue_y<MODE_FWD>(pl, st, 0, pl->nz)) return rc;
+    if (int rc = enqueue_z(pl, st, nullptr)) return rc;
+    if (int rc = enqueue_y<MODE_INV>(pl, st, 0, pl->nz)) return rc;
+    return check_launch(launch_c2r(pl, p_out, norm_scale(pl), st, 0, pl->nz), "fft_x_c2r");
 }
 
 extern "C" int flutas_projection_step_host(flutas_plan *pl, double *u, double *v, double *w, const double *phi, double *p,

@@ -290,12 +290,11 @@ splitting_rhs_kernel2(GridParams g, double dt, int kc, const double *__restrict_
 // a9: u = u' - dt/rho0 grad p^(n+1)   (eq. 18; p^(n+1) was already stored by a8)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-correction_kernel(GridParams g, double dt, const double *__restrict__ pn, const double *__restrict__ up,
-                  const double *__restrict__ vp, const double *__restrict__ wp, double *__restrict__ u,
-                  double *__restrict__ v, double *__restrict__ w) {
-    const long long n = (long long)g.nx * g.ny * g.nz;
-    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= n) return;
+correction_kernel(GridParams g, double dt, long long q0, long long q1, const double *__restrict__ pn,
+                  const double *__restrict__ up, const double *__restrict__ vp, const double *__restrict__ wp,
+                  double *__restrict__ u, double *__restrict__ v, double *__restrict__ w) {
+    const long long q = q0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;   // this launch covers points q0 .. q1 - 1
+    if (q >= q1) return;
     const int i = (int)(q % g.nx);
     const long long r = q / g.nx;
     const int j = (int)(r % g.ny), k = (int)(r / g.ny);

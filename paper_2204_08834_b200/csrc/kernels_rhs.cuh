@@ -32,7 +32,7 @@ enum { RHS3_LOAD_SCALARS = 1, RHS3_LOAD_UV = 2, RHS3_LOAD_W = 4, RHS3_LOAD_ALL =
 
 template <bool WALL>
 __global__ void __launch_bounds__(256, 2)
-splitting_rhs_kernel3(GridParams g, double dt, int kc, const double *__restrict__ u, const double *__restrict__ v,
+splitting_rhs_kernel3(GridParams g, double dt, int kc, int k_base, int k_end, const double *__restrict__ u, const double *__restrict__ v,
                       const double *__restrict__ w, const double *__restrict__ phi,
                       const double *__restrict__ p, const double *__restrict__ po,
                       double *__restrict__ rhs, double *__restrict__ up, double *__restrict__ vp,
@@ -46,7 +46,7 @@ splitting_rhs_kernel3(GridParams g, double dt, int kc, const double *__restrict_
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int tid = ty * G::NTX + tx;
     const int x0 = blockIdx.x * G::X, j0 = blockIdx.y * G::TY;
-    const int k0 = blockIdx.z * kc, k1 = min(k0 + kc, nz);
+    const int k0 = k_base + blockIdx.z * kc, k1 = min(k0 + kc, k_end);   // this launch covers planes k_base .. k_end - 1
     const long long plane = (long long)nx * ny;
 
     if (tid == 0) {

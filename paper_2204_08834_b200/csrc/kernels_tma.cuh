@@ -32,7 +32,8 @@ template <int FIRST, int LAST, typename F> __device__ __forceinline__ void stati
 
 struct TmaFftArgs {
     int n_tiles_x;   // tiles along kx
-    int n_outer;     // lines' outer index count: nz for the y pass, ny for the z pass
+    int n_outer;     // lines' outer index count: nz for the y pass, ny for the z pass (or the planes of one chunk)
+    int outer0;      // first outer index of this launch
     int line_dim;    // tensor dimension the transform runs along: 1 (y) or 2 (z)
     int nxh;         // valid kx columns
     const double2 *tw;                            // e^{-2 pi i m / N}
@@ -71,7 +72,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
     __syncthreads();
 
     auto issue_load = [&](int tile, int b) {
-        const int tx = tile % a.n_tiles_x, outer = tile / a.n_tiles_x;
+        const int tx = tile % a.n_tiles_x, outer = a.outer0 + tile / a.n_tiles_x;
         mbar_arrive_expect_tx(&full[b], TILE_BYTES);
 #pragma unroll
         for (int c = 0; c < NBOX; ++c) {
@@ -81,7 +82,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
         }
     };
     auto issue_store = [&](int tile, int b) {
-        const int tx = tile % a.n_tiles_x, outer = tile / a.n_tiles_x;
+        const int tx = tile % a.n_tiles_x, outer = a.outer0 + tile / a.n_tiles_x;
 #pragma unroll
         for (int c = 0; c < NBOX; ++c) {
             const double2 *src = bufs + b * TILE_ELEMS + c * ROWS * C;
@@ -130,7 +131,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma_kernel(const __grid_constant__ 
                 if (pp + 1 < P) __syncthreads();
             }
         } else {
-            const int tx = tile % a.n_tiles_x, outer = tile / a.n_tiles_x;
+            const int tx = tile % a.n_tiles_x, outer = a.outer0 + tile / a.n_tiles_x;
             const int kx = tx * C + l;
             const double lam_xy = a.lam_x[kx < a.nxh ? kx : 0] + a.lam_outer[outer];
 #pragma unroll
@@ -202,7 +203,7 @@ struct Tma1Args {
     double2 *data;           // the half-spectrum (for the direct stores of the last pass)
     long long row_stride;    // elements between positions r and r+1 of a line
     long long outer_stride;  // elements between outer indices
-    int n_tiles_x, n_outer, line_dim, nxh;
+    int n_tiles_x, n_outer, outer0, line_dim, nxh;   // outer indices outer0 .. outer0 + n_outer - 1
     const double2 *tw;
     const double *lam_x, *lam_outer, *lam_pos;
 };
@@ -276,7 +277,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
     }
 
     auto issue_load = [&](int tile, int b) {
-        const int tx = tile % a.n_tiles_x, outer = tile / a.n_tiles_x;
+        const int tx = tile % a.n_tiles_x, outer = a.outer0 + tile / a.n_tiles_x;
         mbar_arrive_expect_tx(&full[b], TILE_BYTES);
 #pragma unroll
         for (int c = 0; c < NBOX; ++c) {
@@ -333,7 +334,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
             const int nxt = tile + gridDim.x;
             if (nxt < ntiles) issue_load(nxt, b ^ 1);
         }
-        const int tx = tile % a.n_tiles_x, outer = tile / a.n_tiles_x;
+        const int tx = tile % a.n_tiles_x, outer = a.outer0 + tile / a.n_tiles_x;
         const int kx = tx * C + l;
         const bool valid = active && kx < a.nxh;
         double2 *gp = a.data + (long long)outer * a.outer_stride + kx;

@@ -64,6 +64,11 @@ __device__ __forceinline__ void bulk_store(void *gdst, const void *smem_src, uin
                  : "memory");
 }
 
+// ask for a linear range to be brought into L2 (no shared-memory destination, nothing to wait for)
+__device__ __forceinline__ void bulk_prefetch_l2(const void *gsrc, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gsrc), "r"(bytes) : "memory");
+}
+
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 // wait until at most N of this thread's bulk groups still READ their shared-memory source
 template <int N> __device__ __forceinline__ void bulk_wait_read() {
