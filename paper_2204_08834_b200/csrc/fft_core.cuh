@@ -119,6 +119,42 @@ template <int DIR> FL_HD void radix8(double2 *v) {
     v[1] = b0; v[3] = b1; v[5] = b2; v[7] = b3;
 }
 
+// a * W16^M, W16 = exp(DIR * 2 pi i / 16), for the exponents the radix-16 butterfly needs
+constexpr double kCosPi8 = 0.92387953251128675612818318939678828682;
+constexpr double kSinPi8 = 0.38268343236508977172845998403039886676;
+template <int DIR, int M> FL_HD double2 mul_w16(double2 a) {
+    // W16^M = (wr, DIR * wi) with (wr, wi) = (cos, sin)(2 pi M / 16)
+    constexpr double wr = M == 1 ? kCosPi8 : M == 2 ? kInvSqrt2 : M == 3 ? kSinPi8 : M == 4 ? 0.0 : M == 6 ? -kInvSqrt2 : -kCosPi8;
+    constexpr double wi = M == 1 ? kSinPi8 : M == 2 ? kInvSqrt2 : M == 3 ? kCosPi8 : M == 4 ? 1.0 : M == 6 ? kInvSqrt2 : -kSinPi8;
+    static_assert(M == 1 || M == 2 || M == 3 || M == 4 || M == 6 || M == 9, "exponent not used by radix16");
+    if (M == 4) return mul_dir_i<DIR>(a);
+    if (M == 2) return DIR < 0 ? make_double2((a.x + a.y) * kInvSqrt2, (a.y - a.x) * kInvSqrt2)
+                               : make_double2((a.x - a.y) * kInvSqrt2, (a.x + a.y) * kInvSqrt2);
+    if (M == 6) return DIR < 0 ? make_double2((a.y - a.x) * kInvSqrt2, (-a.x - a.y) * kInvSqrt2)
+                               : make_double2((-a.x - a.y) * kInvSqrt2, (a.x - a.y) * kInvSqrt2);
+    const double si = DIR < 0 ? -wi : wi;
+    return make_double2(a.x * wr - a.y * si, a.x * si + a.y * wr);
+}
+
+// 16-point butterfly, natural order in and out: n = 4 n1 + n0, k = k0 + 4 k1,
+//   X[k0 + 4 k1] = sum_n0 W4^(n0 k1) [ W16^(n0 k0) sum_n1 W4^(n1 k0) x[4 n1 + n0] ]
+template <int DIR> FL_HD void radix16(double2 *v) {
+    radix4<DIR>(v[0], v[4], v[8], v[12]);      // slot n0 + 4 k0
+    radix4<DIR>(v[1], v[5], v[9], v[13]);
+    radix4<DIR>(v[2], v[6], v[10], v[14]);
+    radix4<DIR>(v[3], v[7], v[11], v[15]);
+    v[5] = mul_w16<DIR, 1>(v[5]);   v[9] = mul_w16<DIR, 2>(v[9]);    v[13] = mul_w16<DIR, 3>(v[13]);
+    v[6] = mul_w16<DIR, 2>(v[6]);   v[10] = mul_w16<DIR, 4>(v[10]);  v[14] = mul_w16<DIR, 6>(v[14]);
+    v[7] = mul_w16<DIR, 3>(v[7]);   v[11] = mul_w16<DIR, 6>(v[11]);  v[15] = mul_w16<DIR, 9>(v[15]);
+    radix4<DIR>(v[0], v[1], v[2], v[3]);       // slot 4 k0 + k1 holds X[k0 + 4 k1]
+    radix4<DIR>(v[4], v[5], v[6], v[7]);
+    radix4<DIR>(v[8], v[9], v[10], v[11]);
+    radix4<DIR>(v[12], v[13], v[14], v[15]);
+    double2 t;                                   // 4 x 4 transpose of the slots -> natural order
+    t = v[1]; v[1] = v[4]; v[4] = t;    t = v[2]; v[2] = v[8]; v[8] = t;     t = v[3]; v[3] = v[12]; v[12] = t;
+    t = v[6]; v[6] = v[9]; v[9] = t;    t = v[7]; v[7] = v[13]; v[13] = t;   t = v[11]; v[11] = v[14]; v[14] = t;
+}
+
 // the small last pass: 8/R independent radix-R butterflies on contiguous groups of R
 template <int DIR, int R> FL_HD void small_groups(double2 *v) {
     if (R == 8) radix8<DIR>(v);

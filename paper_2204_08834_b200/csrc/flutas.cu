@@ -15,6 +15,7 @@
 #include "kernels_thomas.cuh"
 #include "kernels_tma.cuh"
 #include "kernels_x.cuh"
+#include "kernels_y16.cuh"
 
 using namespace flutas;
 
@@ -78,6 +79,7 @@ struct flutas_plan {
     cudaEvent_t ev_fork, *ev_dep;   // fork from the caller's stream; ev_dep[2 * chunk_index + {0, 1}]
     int n_dep;
     int rhs_variant, rhs_bx;     // 3 = bulk-copy-fed kernel (default), 2 = software-pipelined register form, 1 = first form; threads along x per block (forms 1, 2)
+    int y16;                     // ny = 1024: 1 = register-resident 16 x 8 x 8 kernel (kernels_y16.cuh), 0 = fft_tma1_kernel on 4 columns
     int use_tma;                 // strided passes: 1 = TMA prefetch + register-resident twiddles (default), 2 = generic TMA in/out, 0 = plain loads
     int num_sms;
     CUtensorMap map_y, map_z;    // boxes {2*y_cols, rows, 1} and {2*z_cols, 1, rows} over the half-spectrum
@@ -121,6 +123,30 @@ static double host_lambda(int m, int n, double d) {
     return (double)(-2.0L * (1.0L - cosl(two_pi * (long double)m / (long double)n))) / (d * d);
 }
 
+static double host_lambda(int m, int n, double d);
+static int host_freq_of_pos(int n, int pos);
+// eigenvalues along y in the storage order of the transform in use (the 16 x 8 x 8 kernel has its own digit order)
+static int upload_lam_y(flutas_plan *pl) {
+    std::vector<double> lam(pl->ny);
+    const double dy = pl->ly / pl->ny;
+    for (int pos = 0; pos < pl->ny; ++pos)
+        lam[pos] = host_lambda(pl->y16 ? y1024_freq_of_pos(pos) : host_freq_of_pos(pl->ny, pos), pl->ny, dy);
+    CUDA_TRY(cudaMemcpy(pl->lam_y, lam.data(), sizeof(double) * pl->ny, cudaMemcpyHostToDevice));
+    return FLUTAS_OK;
+}
+
+// elimination coefficients of the one-pass wall solve (they depend on lam_x + lam_y in storage order)
+static int build_thomas_table(flutas_plan *pl) {
+    const int n_tiles_x = (pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C;
+    const long long ncol = (long long)n_tiles_x * pl->ny * ThomasGeom::C;
+    const double dz = pl->lz / pl->nz;
+    thomas_table_kernel<<<(unsigned)((ncol + 127) / 128), 128>>>(pl->ttab, n_tiles_x, pl->ny, pl->nz, pl->nxh, pl->lam_x,
+                                                               pl->lam_y, 1.0 / (dz * dz));
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaDeviceSynchronize());
+    return FLUTAS_OK;
+}
+
 template <typename T> static int upload(T **dst, const std::vector<T> &src, size_t *bytes) {
     CUDA_TRY(cudaMalloc((void **)dst, src.size() * sizeof(T)));
     CUDA_TRY(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
@@ -156,7 +182,7 @@ static int make_spectrum_map(flutas_plan *pl, CUtensorMap *map, int cols, int li
 }
 
 static int plan_make_maps(flutas_plan *pl) {
-    if (int rc = make_spectrum_map(pl, &pl->map_y, pl->y_cols, 1, pl->ny)) return rc;
+    if (int rc = make_spectrum_map(pl, &pl->map_y, pl->y16 ? Y16Geom::C : pl->y_cols, 1, pl->ny)) return rc;
     if (pl->bc_z == FLUTAS_BC_Z_PERIODIC) {
         if (int rc = make_spectrum_map(pl, &pl->map_z, pl->z_cols, 2, pl->nz)) return rc;
     } else if (pl->thomas_variant == 1) {
@@ -189,9 +215,10 @@ static int plan_build(flutas_plan *pl) {
     std::vector<double> lam(pl->pitch, 1.0);
     for (int k = 0; k <= pl->n2; ++k) lam[k] = host_lambda(k, nx, dx);   // x columns are stored in natural order
     if (int rc = upload(&pl->lam_x, lam, &pl->bytes)) return rc;
-    lam.assign(ny, 0.0);
-    for (int pos = 0; pos < ny; ++pos) lam[pos] = host_lambda(host_freq_of_pos(ny, pos), ny, dy);
-    if (int rc = upload(&pl->lam_y, lam, &pl->bytes)) return rc;
+    pl->y16 = ny == Y16Geom::N ? 1 : 0;
+    CUDA_TRY(cudaMalloc((void **)&pl->lam_y, sizeof(double) * ny));
+    pl->bytes += sizeof(double) * ny;
+    if (int rc = upload_lam_y(pl)) return rc;
     if (!wall) {
         lam.assign(nz, 0.0);
         for (int pos = 0; pos < nz; ++pos) lam[pos] = host_lambda(host_freq_of_pos(nz, pos), nz, dz);
@@ -214,11 +241,7 @@ static int plan_build(flutas_plan *pl) {
             const size_t tb = sizeof(double) * ThomasGeom::tab_doubles(nz) * (size_t)n_tiles_x * ny;
             CUDA_TRY(cudaMalloc((void **)&pl->ttab, tb));
             pl->bytes += tb;
-            const long long ncol = (long long)n_tiles_x * ny * ThomasGeom::C;
-            thomas_table_kernel<<<(unsigned)((ncol + 127) / 128), 128>>>(pl->ttab, n_tiles_x, ny, nz, pl->nxh, pl->lam_x, pl->lam_y,
-                                                                       1.0 / (dz * dz));
-            CUDA_TRY(cudaGetLastError());
-            CUDA_TRY(cudaDeviceSynchronize());
+            if (int rc = build_thomas_table(pl)) return rc;
         } else {
             CUDA_TRY(cudaMalloc((void **)&pl->cp, sb / 2));
             pl->bytes += sb / 2;
@@ -348,6 +371,13 @@ extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int val
         }
         pl->thomas_variant = value;
         return FLUTAS_OK;
+    }
+    if (!strcmp(name, "y16") && (value == 0 || (value == 1 && pl->ny == Y16Geom::N))) {
+        CUDA_TRY(cudaDeviceSynchronize());
+        pl->y16 = value;                        // the storage order along y changes with the kernel
+        if (int rc = upload_lam_y(pl)) return rc;
+        if (pl->ttab) if (int rc = build_thomas_table(pl)) return rc;
+        return plan_make_maps(pl);
     }
     if (!strcmp(name, "thomas_warps") && (value == 1 || value == 2)) { pl->thomas_warps = value; return FLUTAS_OK; }
     if (!strcmp(name, "chunk") && value >= 0) { pl->chunk = value; return FLUTAS_OK; }
@@ -613,6 +643,18 @@ static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const 
 template <int MODE> static int enqueue_y(flutas_plan *pl, cudaStream_t st, int k0, int k1) {
     const char *what = MODE == MODE_FWD ? "fft_y_fwd" : "fft_y_inv";
     const long long row_stride = pl->pitch, outer_stride = (long long)pl->pitch * pl->ny;
+    if (pl->y16 && pl->use_tma) {
+        Tma1Args a1{};
+        a1.data = pl->spec; a1.row_stride = row_stride; a1.outer_stride = outer_stride;
+        a1.n_tiles_x = (pl->nxh + Y16Geom::C - 1) / Y16Geom::C;
+        a1.n_outer = k1 - k0; a1.outer0 = k0; a1.line_dim = 1; a1.nxh = pl->nxh; a1.tw = pl->tw_y;
+        auto kern = fft_y1024_kernel<MODE>;
+        if (set_smem(kern, Y16Geom::SMEM) != cudaSuccess) return check_launch(cudaGetLastError(), what);
+        long long grid = pl->num_sms;
+        if (grid > (long long)a1.n_tiles_x * a1.n_outer) grid = (long long)a1.n_tiles_x * a1.n_outer;
+        kern<<<(unsigned)grid, Y16Geom::NT, Y16Geom::SMEM, st>>>(pl->map_y, a1);
+        return check_launch(cudaGetLastError(), what);
+    }
     if (pl->use_tma) {
         TmaFftArgs ty{};
         ty.line_dim = 1;
