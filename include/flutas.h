@@ -146,8 +146,17 @@ int flutas_plan_read_timing(flutas_plan *plan, float *ms_out, int n_out, int *st
  * and write once; used by bench.py for the roofline line. */
 double flutas_plan_kernel_bytes(const flutas_plan *plan, int idx);
 
-/* Advanced tuning knob for experiments (never needed for correctness): "y_cols" / "z_cols" = 4 or 8,
- * the number of kx columns one CTA transforms in the y / z pass. */
+/* Tuning knobs for experiments (never needed for correctness; every combination is held to the same parity tests,
+ * tests/test_gpu_variants.py).  Returns FLUTAS_ERR_INVALID_ARG for an unknown name or a value the plan cannot take.
+ *   "y_cols" / "z_cols" = 4 | 8   kx columns one CTA transforms in the y / z pass (fft_tma1_kernel)
+ *   "y16" = 0 | 1                 ny = 1024 only: 1 (default) = 16 x 8 x 8 register-resident kernel, 0 = 4-column path.
+ *                                 Switching re-orders the eigenvalue tables (synchronises the device).
+ *   "thomas" = 0 | 1              wall only: 1 (default when nz <= 512) = one-pass shared-memory elimination,
+ *                                 0 = two sweeps through HBM (allocates its c' array on first use)
+ *   "thomas_warps" = 1 | 2        solving warps per CTA of the one-pass kernel (default 2)
+ *   "chunk" = n >= 0              planes per launch group of the step (0, default: every kernel covers the grid)
+ *   "overlap" = 0 | 1             chunked only: run the three kernels of a group on three internal streams
+ *   "tma", "x_variant", "rhs_variant", "rhs_kc", "rhs_bx"   older forms of the kernels, kept for A/B measurements */
 int flutas_plan_set_option(flutas_plan *plan, const char *name, int value);
 
 #ifdef __cplusplus

@@ -59,6 +59,7 @@ struct flutas_plan {
     // device workspace
     double2 *spec;
     double *rhs, *up, *vp, *wp, *cp;
+    double *sing_coef;           // wall: 1/(b_k - a c'_{k-1}) and c'_k of the singular (0,0) column, interleaved
     double *ttab;                // wall: elimination coefficients of the one-pass solve, [tile][j][8] (kernels_thomas.cuh)
     int thomas_warps;            // solving warps per CTA of the one-pass kernel (1 or 2)
     int thomas_variant;          // wall: 1 = one-pass shared-memory solve (nz <= 512), 0 = two sweeps through HBM
@@ -139,9 +140,9 @@ static int upload_lam_y(flutas_plan *pl) {
 static int build_thomas_table(flutas_plan *pl) {
     const int n_tiles_x = (pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C;
     const long long ncol = (long long)n_tiles_x * pl->ny * ThomasGeom::C;
-    const double dz = pl->lz / pl->nz;
+    const double inv_dz = 1.0 / (pl->lz / pl->nz);
     thomas_table_kernel<<<(unsigned)((ncol + 127) / 128), 128>>>(pl->ttab, n_tiles_x, pl->ny, pl->nz, pl->nxh, pl->lam_x,
-                                                               pl->lam_y, 1.0 / (dz * dz));
+                                                               pl->lam_y, inv_dz * inv_dz);
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaDeviceSynchronize());
     return FLUTAS_OK;
@@ -234,6 +235,19 @@ static int plan_build(flutas_plan *pl) {
     CUDA_TRY(cudaMalloc((void **)&pl->wp, fb));
     pl->bytes += sb + 4 * fb;
     if (wall) {
+        // the (0,0) column: lam = 0; the elimination coefficients do not depend on the data (same recurrence, same
+        // IEEE divisions as a per-step evaluation would do)
+        std::vector<double> sc(2 * (size_t)nz, 0.0);
+        const double a = (1.0 / dz) * (1.0 / dz), b_end = -a, b_in = -2.0 * a;   // as GridParams::inv_dz squared
+        double inv = 1.0 / b_end, cpv = a * inv;
+        sc[0] = inv; sc[1] = cpv;
+        for (int k = 1; k <= nz - 2; ++k) {
+            inv = 1.0 / (b_in - a * cpv);
+            cpv = a * inv;
+            sc[2 * k] = inv; sc[2 * k + 1] = cpv;
+        }
+        sc[2 * (size_t)nz - 1] = a;
+        if (int rc = upload(&pl->sing_coef, sc, &pl->bytes)) return rc;
         pl->thomas_variant = ThomasGeom::smem_bytes(nz) <= 227 * 1024 ? 1 : 0;
         pl->thomas_warps = 2;
         if (pl->thomas_variant == 1) {
@@ -316,7 +330,7 @@ extern "C" void flutas_plan_destroy(flutas_plan *pl) {
     cudaDeviceSynchronize();
     cudaFree(pl->tw_x); cudaFree(pl->tw_y); cudaFree(pl->tw_z);
     cudaFree(pl->lam_x); cudaFree(pl->lam_y); cudaFree(pl->lam_z);
-    cudaFree(pl->spec); cudaFree(pl->rhs); cudaFree(pl->up); cudaFree(pl->vp); cudaFree(pl->wp); cudaFree(pl->cp); cudaFree(pl->ttab);
+    cudaFree(pl->spec); cudaFree(pl->rhs); cudaFree(pl->up); cudaFree(pl->vp); cudaFree(pl->wp); cudaFree(pl->cp); cudaFree(pl->ttab); cudaFree(pl->sing_coef);
     for (int i = 0; i < 6; ++i) cudaFree(pl->stage[i]);
     for (int i = 0; i < 3; ++i) if (pl->lane[i]) cudaStreamDestroy(pl->lane[i]);
     if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
@@ -715,17 +729,17 @@ static int enqueue_z(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
             if (set_smem(kern, smem_t) != cudaSuccess) return check_launch(cudaGetLastError(), "z_solve attr");
             long long grid = pl->num_sms;
             if (grid > (long long)ta.n_tiles_x * ta.ny) grid = (long long)ta.n_tiles_x * ta.ny;
-            kern<<<(unsigned)grid, 32 * pl->thomas_warps, smem_t, st>>>(pl->map_z, ta);
+            kern<<<(unsigned)grid, 32 * (pl->thomas_warps + 1), smem_t, st>>>(pl->map_z, ta);
         } else {
             thomas_kernel<<<(unsigned)((ncol + 127) / 128), 128, 0, st>>>(pl->spec, pl->cp, pl->pitch, pl->ny, pl->nz, pl->nxh,
                                                                         pl->lam_x, pl->lam_y, inv_dz2);
         }
         if (int rc = check_launch(cudaGetLastError(), "z_solve (thomas)")) return rc;
         if (tm) tm->mark();
-        const size_t smem = sizeof(double) * 3 * (size_t)pl->nz;
+        const size_t smem = sizeof(double) * (4 * (size_t)pl->nz + 2);
         if (smem > 200 * 1024) return fail(FLUTAS_ERR_UNSUPPORTED_SIZE, "nz too large for the singular-column kernel");
         if (set_smem(thomas_singular_kernel, smem) != cudaSuccess) return check_launch(cudaGetLastError(), "z_singular attr");
-        thomas_singular_kernel<<<1, 256, smem, st>>>(pl->spec, ncol, pl->nz, inv_dz2);
+        thomas_singular_kernel<<<1, 256, smem, st>>>(pl->spec, ncol, pl->nz, pl->sing_coef);
         if (int rc = check_launch(cudaGetLastError(), "z_singular")) return rc;
         if (tm) tm->mark();
     }

@@ -578,40 +578,38 @@ thomas_kernel(double2 *__restrict__ spec, double *__restrict__ cp, int pitch, in
 
 // The (kx,ky) = (0,0) column: lam_xy = 0, the system is singular (pure Neumann).  Eliminate rows
 // 0..nz-2, pin x_{nz-1} = 0, back-substitute, then remove the mean over k (zero-mean gauge, R5).
-__global__ void thomas_singular_kernel(double2 *__restrict__ spec, long long col_stride, int nz, double inv_dz2) {
+__global__ void thomas_singular_kernel(double2 *__restrict__ spec, long long col_stride, int nz,
+                                       const double *__restrict__ coef /* inv_k, c'_k interleaved: 2 nz doubles */) {
     extern __shared__ double sm[];
-    double *dr = sm, *di = sm + nz, *cpv = sm + 2 * nz;
+    double *dr = sm, *di = sm + nz, *cf = sm + 2 * nz, *mean = sm + 4 * nz;
     for (int k = threadIdx.x; k < nz; k += blockDim.x) {
         const double2 d = spec[(long long)k * col_stride];
         dr[k] = d.x;
         di[k] = d.y;
+        cf[2 * k] = coef[2 * k];
+        cf[2 * k + 1] = coef[2 * k + 1];
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        const double a = inv_dz2, b_end = -inv_dz2, b_in = -2.0 * inv_dz2;
-        double inv = 1.0 / b_end;
-        cpv[0] = a * inv;
-        dr[0] *= inv;
-        di[0] *= inv;
+    if (threadIdx.x < 2) {                      // thread 0: real parts, thread 1: imaginary parts
+        double *x = threadIdx.x == 0 ? dr : di;
+        const double a = cf[2 * nz - 1];        // slot of c'_{nz-1} (never used as such) carries a = 1/dz^2
+        double prev = x[0] * cf[0];
+        x[0] = prev;
         for (int k = 1; k <= nz - 2; ++k) {
-            inv = 1.0 / (b_in - a * cpv[k - 1]);
-            cpv[k] = a * inv;
-            dr[k] = (dr[k] - a * dr[k - 1]) * inv;
-            di[k] = (di[k] - a * di[k - 1]) * inv;
+            prev = (x[k] - a * prev) * cf[2 * k];
+            x[k] = prev;
         }
-        dr[nz - 1] = 0.0;
-        di[nz - 1] = 0.0;
+        double nxt = 0.0, sum = 0.0;            // x_{nz-1} = 0 (the pinned unknown, R5)
+        x[nz - 1] = 0.0;
         for (int k = nz - 2; k >= 0; --k) {
-            dr[k] = dr[k] - cpv[k] * dr[k + 1];
-            di[k] = di[k] - cpv[k] * di[k + 1];
+            nxt = x[k] - cf[2 * k + 1] * nxt;
+            x[k] = nxt;
         }
-        double mr = 0.0, mi = 0.0;
-        for (int k = 0; k < nz; ++k) { mr += dr[k]; mi += di[k]; }
-        cpv[0] = mr / nz;
-        cpv[1] = mi / nz;     // nz >= 2
+        for (int k = 0; k < nz; ++k) sum += x[k];
+        mean[threadIdx.x] = sum / nz;
     }
     __syncthreads();
-    const double mr = cpv[0], mi = cpv[1];
+    const double mr = mean[0], mi = mean[1];
     for (int k = threadIdx.x; k < nz; k += blockDim.x)
         spec[(long long)k * col_stride] = make_double2(dr[k] - mr, di[k] - mi);
 }

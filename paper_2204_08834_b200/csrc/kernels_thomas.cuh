@@ -19,13 +19,13 @@
 // with row(j) = j for the chain from the bottom wall and nz-1-j for the chain from the top wall.  The matrix is
 // symmetric under k -> nz-1-k, so both chains of a column use the SAME coefficients c_j: they depend on the grid
 // only, not on the data, and are tabulated once per plan (thomas_table_kernel) in the order the solve reads them,
-// [tile][j][8 columns] with one more row holding 1 / (1 - c~_m c_{m-1}); a tile's table is one contiguous block
-// fetched by a linear bulk copy.
+// [tile][j / 2][8 columns][j % 2] (a lane fetches two consecutive coefficients with one 16-byte load) with one more
+// entry holding 1 / (1 - c~_m c_{m-1}); a tile's table is one contiguous block fetched by a linear bulk copy.
 //
-// CTA = NWARP (1 or 2) solving warps, persistent, one per SM.  Three data buffers and two table buffers rotate over
-// the CTA's tile sequence n = 0, 1, 2, ... (data buffer n % 3, table buffer n % 2, solved by warp n % NWARP): while
-// two tiles are being solved the third buffer drains its store and takes the load of tile n + 3, issued by whichever
-// warp just finished.  A single warp runs this loop at ~30 cycles per chain step (about 3 cycles per instruction:
+// CTA = NWARP (1 or 2) solving warps + one copy warp, persistent, one per SM.  Three data buffers and two table
+// buffers rotate over the CTA's tile sequence n = 0, 1, 2, ... (data buffer n % 3, table buffer n % 2, solved by warp
+// n % NWARP): while two tiles are being solved the third buffer drains its store and takes the load of tile n + 3,
+// both issued by the copy warp when a solving warp reports its tile done (mbarrier).  A single warp runs this loop at ~30 cycles per chain step (about 3 cycles per instruction:
 // there is nothing to switch to), so the kernel is bound by the two tiles that fit beside the one in flight, not by
 // HBM: measured 2.1 ms at 1024 x 1024 x 512 (4.6 TB/s of algorithmic bytes) against 3.75 ms for the two sweeps.
 #pragma once
@@ -40,7 +40,9 @@ struct ThomasGeom {
     static constexpr int C = 8;                     // kx columns per tile
     static constexpr int NBUF = 3, NTAB = 2, B = 8;   // data buffers, table buffers, chain steps per register batch
     __host__ __device__ static int nzh(int nz) { return nz - nz / 2; }            // steps of the longer chain
-    __host__ __device__ static size_t tab_doubles(int nz) { return (size_t)(nzh(nz) + 1) * C; }   // per tile
+    // per tile: entries j = 0 .. nzh (c_0 .. c_{nzh-1}, then f), two consecutive j packed per column so that a lane
+    // fetches c_j, c_{j+1} with one 16-byte load: [j / 2][column][j % 2]
+    __host__ __device__ static size_t tab_doubles(int nz) { return (size_t)((nzh(nz) + 2) / 2) * 2 * C; }
     __host__ __device__ static int box_rows(int nz) { return nz < 256 ? nz : 256; }
     // a buffer holds whole boxes: the last one may hang over the end of the column (zero-filled, never stored)
     __host__ __device__ static size_t data_bytes(int nz) {
@@ -48,6 +50,7 @@ struct ThomasGeom {
     }
     // a warp's table buffer, with room for the 2B rows the forward loop requests past the end
     __host__ __device__ static size_t tab_stride(int nz) { return ((tab_doubles(nz) + 2 * B * C) * 8 + 127) / 128 * 128; }
+    __host__ __device__ static int tab_index(int j, int col) { return (j >> 1) * 2 * C + col * 2 + (j & 1); }
     __host__ static size_t smem_bytes(int nz) {
         return NBUF * data_bytes(nz) + NTAB * tab_stride(nz) + 128;
     }
@@ -65,23 +68,23 @@ __global__ void thomas_table_kernel(double *__restrict__ tab, int n_tiles_x, int
     const int tx = (int)(tile % n_tiles_x), jy = (int)(tile / n_tiles_x);
     const int kx = tx * G::C + col;
     const int nzh = G::nzh(nz), m = nz / 2;
-    double *t = tab + tile * G::tab_doubles(nz) + col;
+    double *t = tab + tile * G::tab_doubles(nz);
     if (kx >= nxh || (kx == 0 && jy == 0)) {          // padding columns and the singular column: benign values
-        for (int j = 0; j < nzh; ++j) t[(long long)j * G::C] = 0.0;
-        t[(long long)nzh * G::C] = 1.0;
+        for (int j = 0; j < nzh; ++j) t[G::tab_index(j, col)] = 0.0;
+        t[G::tab_index(nzh, col)] = 1.0;
         return;
     }
     const double lam = lam_x[kx] + lam_y[jy];
     const double a = inv_dz2, b_end = -inv_dz2 + lam, b_in = -2.0 * inv_dz2 + lam;
     double cj = a / b_end, c_m1 = 0.0;                // c_m1 = c_{m-1}
-    t[0] = cj;
+    t[G::tab_index(0, col)] = cj;
     if (m == 1) c_m1 = cj;
     for (int j = 1; j < nzh; ++j) {
         cj = a / (b_in - a * cj);
-        t[(long long)j * G::C] = cj;
+        t[G::tab_index(j, col)] = cj;
         if (j == m - 1) c_m1 = cj;
     }
-    t[(long long)nzh * G::C] = 1.0 / (1.0 - cj * c_m1);   // cj = c_{nzh-1} = c~_m
+    t[G::tab_index(nzh, col)] = 1.0 / (1.0 - cj * c_m1);   // cj = c_{nzh-1} = c~_m
 }
 
 struct ThomasArgs {
@@ -91,10 +94,10 @@ struct ThomasArgs {
 };
 
 template <int NWARP>
-__global__ void __launch_bounds__(32 * NWARP, 1) thomas_tma_kernel(const __grid_constant__ CUtensorMap tmap, ThomasArgs a) {
+__global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const __grid_constant__ CUtensorMap tmap, ThomasArgs a) {
     using G = ThomasGeom;
     extern __shared__ unsigned char smem_raw[];
-    __shared__ uint64_t full_d[G::NBUF], full_c[G::NTAB];
+    __shared__ uint64_t full_d[G::NBUF], full_c[G::NTAB], done[G::NBUF];
 
     const int nz = a.nz, nzh = G::nzh(nz), m = nz / 2;
     const int rows = G::box_rows(nz), nbox = (nz + rows - 1) / rows;
@@ -114,6 +117,7 @@ __global__ void __launch_bounds__(32 * NWARP, 1) thomas_tma_kernel(const __grid_
     if (threadIdx.x == 0) {
         for (int b = 0; b < G::NBUF; ++b) mbar_init(&full_d[b], 1);
         for (int w = 0; w < G::NTAB; ++w) mbar_init(&full_c[w], 1);
+        for (int b = 0; b < G::NBUF; ++b) mbar_init(&done[b], 1);
         fence_barrier_init();
         fence_proxy_async();
     }
@@ -150,12 +154,31 @@ __global__ void __launch_bounds__(32 * NWARP, 1) thomas_tma_kernel(const __grid_
 
     const int cnt = top ? nzh : m;                     // steps of this lane's chain
     const double dz2 = a.dz2;
+    if (warp == NWARP) {
+        // ---- the copy warp: as tiles are reported solved (in order), write them back, refill the table buffer at
+        //      once and the data buffer as soon as the store has drained it.  The solving warps never wait for a drain.
+        if (lane == 0) {
+            for (long long n = 0; n < my_tiles; ++n) {
+                mbar_wait(&done[n % G::NBUF], (uint32_t)(n / G::NBUF) & 1);
+                issue_store(n);
+                if (n + G::NTAB < my_tiles) issue_table(n + G::NTAB);
+                if (n + G::NBUF < my_tiles) {
+                    bulk_wait_read<0>();
+                    issue_data(n + G::NBUF);
+                }
+            }
+            bulk_wait_all<0>();
+        }
+        return;
+    }
     for (long long n = warp; n < my_tiles; n += NWARP) {
         const int b = (int)(n % G::NBUF);
         const int tb = (int)(n % G::NTAB);
         const uint32_t it_c = (uint32_t)(n / G::NTAB), it_d = (uint32_t)(n / G::NBUF);
         double *s = reinterpret_cast<double *>(base + b * buf_stride) + col * 2 + comp;   // element (row, col): s[row * 16]
-        const double *ct = reinterpret_cast<const double *>(tab_base + tb * tab_stride) + col;   // c_j: ct[j * 8]
+        const double *ctab = reinterpret_cast<const double *>(tab_base + tb * tab_stride);
+        const double2 *ct2 = reinterpret_cast<const double2 *>(ctab) + col;      // (c_2q, c_2q+1): ct2[q * 8]
+        auto c_at = [&](int j) { return ctab[G::tab_index(j, col)]; };
         const bool nostore = tile_of(n) == 0 && col == 0;   // the (0,0) column is left as it is (thomas_singular_kernel)
         if (lane == 0 && n + G::NTAB < my_tiles)       // the table that takes this buffer next: on its way to L2 meanwhile
             bulk_prefetch_l2(a.tab + tile_of(n + G::NTAB) * G::tab_doubles(nz), tab_bytes);
@@ -173,32 +196,46 @@ __global__ void __launch_bounds__(32 * NWARP, 1) thomas_tma_kernel(const __grid_
         const int nfull = m >= 4 * G::B ? m / G::B : 0;    // m <= cnt: the same trip count in every lane
         if (nfull > 0) {
             double *sp = s + row_of(0) * 16;
-            const double *cp = ct;
-            double ec[G::B], cc[G::B], dn[G::B], cn[G::B];
+            const double2 *cp = ct2;
+            double ec[G::B], cc[G::B], dn[G::B];
+            double2 cn[G::B / 2];
 #pragma unroll
-            for (int e = 0; e < G::B; ++e) { cc[e] = cp[e * 8]; ec[e] = sp[e * ds] * (cc[e] * dz2); }
+            for (int q = 0; q < G::B / 2; ++q) {
+                const double2 c2 = cp[q * 8];
+                cc[2 * q] = c2.x; cc[2 * q + 1] = c2.y;
+                ec[2 * q] = sp[(2 * q) * ds] * (c2.x * dz2);
+                ec[2 * q + 1] = sp[(2 * q + 1) * ds] * (c2.y * dz2);
+            }
 #pragma unroll
-            for (int e = 0; e < G::B; ++e) { dn[e] = sp[(G::B + e) * ds]; cn[e] = cp[(G::B + e) * 8]; }
+            for (int e = 0; e < G::B; ++e) dn[e] = sp[(G::B + e) * ds];
+#pragma unroll
+            for (int q = 0; q < G::B / 2; ++q) cn[q] = cp[(G::B / 2 + q) * 8];
 #pragma unroll 2
             for (int bt = 0; bt < nfull; ++bt) {
-                double d2[G::B], c2[G::B], gv[G::B];
+                double d2[G::B], gv[G::B];
+                double2 c2[G::B / 2];
 #pragma unroll
-                for (int e = 0; e < G::B; ++e) { d2[e] = sp[(2 * G::B + e) * ds]; c2[e] = cp[(2 * G::B + e) * 8]; }
+                for (int e = 0; e < G::B; ++e) d2[e] = sp[(2 * G::B + e) * ds];
+#pragma unroll
+                for (int q = 0; q < G::B / 2; ++q) c2[q] = cp[(G::B + q) * 8];
 #pragma unroll
                 for (int e = 0; e < G::B; ++e) {
                     g = fma(-cc[e], g, ec[e]);             // the only dependent operation of a step
                     gv[e] = g;
-                    cc[e] = cn[e];
-                    ec[e] = dn[e] * (cn[e] * dz2);
+                    const double cnx = (e & 1) ? cn[e >> 1].y : cn[e >> 1].x;
+                    cc[e] = cnx;
+                    ec[e] = dn[e] * (cnx * dz2);
                 }
                 if (!nostore) {
 #pragma unroll
                     for (int e = 0; e < G::B; ++e) sp[e * ds] = gv[e];
                 }
 #pragma unroll
-                for (int e = 0; e < G::B; ++e) { dn[e] = d2[e]; cn[e] = c2[e]; }
+                for (int e = 0; e < G::B; ++e) dn[e] = d2[e];
+#pragma unroll
+                for (int q = 0; q < G::B / 2; ++q) cn[q] = c2[q];
                 sp += G::B * ds;
-                cp += G::B * 8;
+                cp += (G::B / 2) * 8;
             }
         }
         for (int j0 = nfull * G::B; j0 < nzh; j0 += G::B) {
@@ -207,7 +244,7 @@ __global__ void __launch_bounds__(32 * NWARP, 1) thomas_tma_kernel(const __grid_
             for (int e = 0; e < G::B; ++e) {
                 const bool ok = j0 + e < cnt;              // a masked step is the identity map: d = 0, c = -1
                 d[e] = ok ? s[row_of(j0 + e) * 16] : 0.0;
-                c[e] = ok ? ct[(j0 + e) * 8] : -1.0;
+                c[e] = ok ? c_at(j0 + e) : -1.0;
             }
 #pragma unroll
             for (int e = 0; e < G::B; ++e) {
@@ -223,30 +260,45 @@ __global__ void __launch_bounds__(32 * NWARP, 1) thomas_tma_kernel(const __grid_
         // ---- the 2 x 2 system where the two chains meet: g = g_{m-1} (bottom chain) or h_m (top chain)
         const double other = __shfl_xor_sync(0xffffffffu, g, 16);
         const double g_lo = top ? other : g, h_hi = top ? g : other;
-        const double c_hi = ct[(nzh - 1) * 8], c_lo = ct[(m - 1) * 8], f = ct[nzh * 8];
+        const double c_hi = c_at(nzh - 1), c_lo = c_at(m - 1), f = c_at(nzh);
         const double x_m = (h_hi - c_hi * g_lo) * f;
         double x = top ? x_m : fma(-c_lo, x_m, g_lo);      // x_{cnt-1} of this chain
         if (!nostore) s[row_of(cnt - 1) * 16] = x;
-        // ---- back-substitution outwards: j = cnt-2 .. 0, full batches first (operands requested one batch ahead;
-        //      the last full batch requests nothing)
-        const int nfull_b = m >= 4 * G::B ? (m - 1) / G::B : 0;
+        // ---- back-substitution outwards: j = cnt-2 .. 0.  One step alone if that makes the next j odd (coefficient
+        //      pairs are (c_2q, c_2q+1)), then full batches (operands requested one batch ahead; the last full batch
+        //      requests nothing), then the predicated remainder
+        int jb = cnt - 2;
+        if (jb >= 0 && (jb & 1) == 0) {
+            x = fma(-c_at(jb), x, s[row_of(jb) * 16]);
+            if (!nostore) s[row_of(jb) * 16] = x;
+            --jb;
+        }
+        const int nfull_b = m >= 4 * G::B ? (m - 2) / G::B : 0;   // every lane has at least m - 2 steps left
         if (nfull_b > 0) {
-            double *sp = s + row_of(cnt - 2) * 16;
-            const double *cp = ct + (cnt - 2) * 8;
-            double dn[G::B], cn[G::B];
+            double *sp = s + row_of(jb) * 16;
+            const double2 *cp = ct2 + (jb >> 1) * 8;   // jb is odd: the pair (c_{jb-1}, c_jb)
+            double dn[G::B];
+            double2 cn[G::B / 2];
 #pragma unroll
-            for (int e = 0; e < G::B; ++e) { dn[e] = sp[-e * ds]; cn[e] = cp[-e * 8]; }
+            for (int e = 0; e < G::B; ++e) dn[e] = sp[-e * ds];
+#pragma unroll
+            for (int q = 0; q < G::B / 2; ++q) cn[q] = cp[-q * 8];
             auto batch = [&](auto request_next) {
-                double d[G::B], c[G::B];
+                double d[G::B];
+                double2 c[G::B / 2];
 #pragma unroll
-                for (int e = 0; e < G::B; ++e) { d[e] = dn[e]; c[e] = cn[e]; }
+                for (int e = 0; e < G::B; ++e) d[e] = dn[e];
+#pragma unroll
+                for (int q = 0; q < G::B / 2; ++q) c[q] = cn[q];
                 if (decltype(request_next)::value) {
 #pragma unroll
-                    for (int e = 0; e < G::B; ++e) { dn[e] = sp[-(G::B + e) * ds]; cn[e] = cp[-(G::B + e) * 8]; }
+                    for (int e = 0; e < G::B; ++e) dn[e] = sp[-(G::B + e) * ds];
+#pragma unroll
+                    for (int q = 0; q < G::B / 2; ++q) cn[q] = cp[-(G::B / 2 + q) * 8];
                 }
 #pragma unroll
-                for (int e = 0; e < G::B; ++e) {
-                    x = fma(-c[e], x, d[e]);
+                for (int e = 0; e < G::B; ++e) {           // step e: j = jb - e, odd j first
+                    x = fma(-((e & 1) ? c[e >> 1].x : c[e >> 1].y), x, d[e]);
                     d[e] = x;
                 }
                 if (!nostore) {
@@ -254,19 +306,19 @@ __global__ void __launch_bounds__(32 * NWARP, 1) thomas_tma_kernel(const __grid_
                     for (int e = 0; e < G::B; ++e) sp[-e * ds] = d[e];
                 }
                 sp -= G::B * ds;
-                cp -= G::B * 8;
+                cp -= (G::B / 2) * 8;
             };
 #pragma unroll 2
             for (int bt = 0; bt + 1 < nfull_b; ++bt) batch(std::true_type{});
             batch(std::false_type{});
         }
-        for (int j0 = cnt - 2 - nfull_b * G::B; j0 >= 0; j0 -= G::B) {
+        for (int j0 = jb - nfull_b * G::B; j0 >= 0; j0 -= G::B) {
             double d[G::B], c[G::B];
 #pragma unroll
             for (int e = 0; e < G::B; ++e) {
                 const bool ok = j0 - e >= 0;
                 d[e] = ok ? s[row_of(j0 - e) * 16] : 0.0;
-                c[e] = ok ? ct[(j0 - e) * 8] : -1.0;
+                c[e] = ok ? c_at(j0 - e) : -1.0;
             }
 #pragma unroll
             for (int e = 0; e < G::B; ++e) {
@@ -279,20 +331,11 @@ __global__ void __launch_bounds__(32 * NWARP, 1) thomas_tma_kernel(const __grid_
                     if (j0 - e >= 0) s[row_of(j0 - e) * 16] = d[e];
             }
         }
-        // ---- write the tile back; its buffer then takes tile n + NBUF, its table buffer tile n + NTAB
+        // ---- report the tile solved (the copy warp writes it back and refills the buffers)
         fence_proxy_async();
         __syncwarp();
-        if (lane == 0) {
-            issue_store(n);
-            if (n + G::NTAB < my_tiles) issue_table(n + G::NTAB);
-            if (n + G::NBUF < my_tiles) {
-                bulk_wait_read<0>();
-                issue_data(n + G::NBUF);
-            }
-        }
-        __syncwarp();
+        if (lane == 0) mbar_arrive(&done[b]);
     }
-    if (lane == 0) bulk_wait_all<0>();
 }
 
 }  // namespace flutas
