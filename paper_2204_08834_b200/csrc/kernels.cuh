@@ -18,6 +18,17 @@
 
 namespace flutas {
 
+// Where the x transforms find the rows of the half-spectrum: row (j, k) starts at k * plane + j * pitch (a plane holds
+// ny rows + padding); a launch covers lines line0, line0 + 1, ... of the real field (line = j + ny k).
+struct SpecRows {
+    int ny;
+    long long plane, line0;
+};
+__device__ __forceinline__ long long spec_row_offset(const SpecRows &r, long long line, int pitch) {
+    const long long g = r.line0 + line;
+    return (g / r.ny) * r.plane + (g % r.ny) * pitch;
+}
+
 struct GridParams {
     int nx, ny, nz, wall;
     double inv_dx, inv_dy, inv_dz;
@@ -480,7 +491,7 @@ __device__ __forceinline__ void batched_copy(int tid, Load load, Store store) {
 template <int N2, int NT>
 __global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1)
 fft_x_r2c_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec,
-                 const double2 *__restrict__ tw /* e^{-2 pi i m / nx} */) {
+                 const double2 *__restrict__ tw /* e^{-2 pi i m / nx} */, SpecRows sr) {
     extern __shared__ double2 smem[];
     double2 *s = smem;
     constexpr int PITCH = N2 + 8;
@@ -495,7 +506,7 @@ fft_x_r2c_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec,
     __syncthreads();
     for (int item = tid; item < 8 * (N2 / 2 + 1); item += NT) r2c_post_item<N2, 8, true>(s, item / 8, item % 8, tw);
     __syncthreads();
-    double2 *dst = spec + line0 * PITCH;
+    double2 *dst = spec + spec_row_offset(sr, line0, PITCH);
     for (int idx = tid; idx < 8 * PITCH; idx += NT) {
         const int l = idx / PITCH, k = idx % PITCH;     // spectrum rows are stored in natural kx order
         if (k <= N2) dst[idx] = s[tile_index<8, true>(k == N2 ? N2 : pos_of_freq<N2>(k), l)];
@@ -508,13 +519,13 @@ fft_x_r2c_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec,
 template <int N2, int NT>
 __global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1)
 fft_x_c2r_kernel(const double2 *__restrict__ spec, double *__restrict__ out,
-                 const double2 *__restrict__ tw, double scale) {
+                 const double2 *__restrict__ tw, double scale, SpecRows sr) {
     extern __shared__ double2 smem[];
     double2 *s = smem;
     constexpr int PITCH = N2 + 8;
     const int tid = threadIdx.x;
     const long long line0 = (long long)blockIdx.x * 8;
-    const double2 *src = spec + line0 * PITCH;
+    const double2 *src = spec + spec_row_offset(sr, line0, PITCH);
     batched_copy<8 * PITCH, NT, 9, double2>(
         tid, [&](int idx) { return src[idx]; },
         [&](int idx, double2 val) {
@@ -540,7 +551,7 @@ fft_x_c2r_kernel(const double2 *__restrict__ spec, double *__restrict__ out,
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128)
 thomas_kernel(double2 *__restrict__ spec, double *__restrict__ cp, int pitch, int ny, int nz, int nxh,
-              const double *__restrict__ lam_x, const double *__restrict__ lam_y, double inv_dz2) {
+              const double *__restrict__ lam_x, const double *__restrict__ lam_y, double inv_dz2, long long plane) {
     const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long ncol = (long long)pitch * ny;
     if (c >= ncol || c == 0) return;
@@ -556,7 +567,7 @@ thomas_kernel(double2 *__restrict__ spec, double *__restrict__ cp, int pitch, in
     cp[c] = cpv;
 #pragma unroll 4
     for (int k = 1; k < nz; ++k) {
-        const long long q = c + (long long)k * ncol;
+        const long long q = c + (long long)k * plane;
         d = spec[q];
         const double b = (k == nz - 1) ? b_end : b_in;
         inv = 1.0 / (b - a * cpv);
@@ -568,7 +579,7 @@ thomas_kernel(double2 *__restrict__ spec, double *__restrict__ cp, int pitch, in
     double2 x = dp;  // x_{nz-1} = d'_{nz-1}
 #pragma unroll 4
     for (int k = nz - 2; k >= 0; --k) {
-        const long long q = c + (long long)k * ncol;
+        const long long q = c + (long long)k * plane;
         const double2 dk = spec[q];
         const double ck = cp[q];
         x = make_double2(dk.x - ck * x.x, dk.y - ck * x.y);

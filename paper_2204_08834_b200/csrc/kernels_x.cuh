@@ -67,7 +67,8 @@ __device__ __forceinline__ void xpass_b(double2 *X, int lb, int tb, const double
 // ------------------------------------------------------------------------------------------------
 template <int N2>
 __global__ void __launch_bounds__(N2, N2 <= 256 ? 2 : 1)
-fft_x_r2c_tma_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec, const double2 *__restrict__ tw, int ntiles) {
+fft_x_r2c_tma_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec, const double2 *__restrict__ tw, int ntiles,
+                     SpecRows sr) {
     using XG = XGeom<N2>;
     constexpr int P = XG::P, B = XG::B, PITCH = XG::PITCH;
     static_assert(P <= 3, "nx <= 1024");
@@ -121,7 +122,7 @@ fft_x_r2c_tma_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec,
         }
         __syncthreads();
         {   // split: Z -> X[q], X[N2 - q], written to the global row in natural kx order
-            double2 *dst = spec + ((long long)tile * 8 + la) * PITCH;
+            double2 *dst = spec + spec_row_offset(sr, (long long)tile * 8, PITCH) + la * PITCH;
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
                 const int q = ta + r * B;                    // 0 .. N2/2 - 1
@@ -149,7 +150,7 @@ fft_x_r2c_tma_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec,
 template <int N2>
 __global__ void __launch_bounds__(N2, N2 <= 256 ? 2 : 1)
 fft_x_c2r_tma_kernel(const double2 *__restrict__ spec, double *__restrict__ out, const double2 *__restrict__ tw,
-                     double scale, int ntiles) {
+                     double scale, int ntiles, SpecRows sr) {
     using XG = XGeom<N2>;
     constexpr int P = XG::P, B = XG::B, PITCH = XG::PITCH;
     static_assert(P <= 3, "nx <= 1024");
@@ -173,7 +174,7 @@ fft_x_c2r_tma_kernel(const double2 *__restrict__ spec, double *__restrict__ out,
 
     auto issue_load = [&](int tile) {
         mbar_arrive_expect_tx(&full, TILE_BYTES);
-        bulk_load(land, spec + (long long)tile * 8 * PITCH, TILE_BYTES, &full);
+        bulk_load(land, spec + spec_row_offset(sr, (long long)tile * 8, PITCH), TILE_BYTES, &full);
     };
     if (tid == 0 && (int)blockIdx.x < ntiles) issue_load(blockIdx.x);
 
