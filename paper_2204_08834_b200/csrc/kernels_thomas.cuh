@@ -25,9 +25,10 @@
 // CTA = NWARP (1 or 2) solving warps + one copy warp, persistent, one per SM.  Three data buffers and two table
 // buffers rotate over the CTA's tile sequence n = 0, 1, 2, ... (data buffer n % 3, table buffer n % 2, solved by warp
 // n % NWARP): while two tiles are being solved the third buffer drains its store and takes the load of tile n + 3,
-// both issued by the copy warp when a solving warp reports its tile done (mbarrier).  A single warp runs this loop at ~30 cycles per chain step (about 3 cycles per instruction:
-// there is nothing to switch to), so the kernel is bound by the two tiles that fit beside the one in flight, not by
-// HBM: measured 2.1 ms at 1024 x 1024 x 512 (4.6 TB/s of algorithmic bytes) against 3.75 ms for the two sweeps.
+// both issued by the copy warp when a solving warp reports its tile done (mbarrier).  A single warp runs this loop at
+// ~30 cycles per chain step (about 3 cycles per instruction: there is nothing to switch to), so the kernel is bound
+// by the two tiles that fit beside the one in flight, not by HBM: measured 2.1-2.2 ms at 1024 x 1024 x 512
+// (4.3-4.6 TB/s of algorithmic bytes) against 3.75 ms for the two sweeps.
 #pragma once
 #include "kernels.cuh"
 #include "tma.cuh"

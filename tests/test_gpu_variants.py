@@ -100,3 +100,36 @@ def test_chunked_launch_order_is_bitwise_the_plain_order(maker):
         for g, r in zip(got, ref):
             assert np.array_equal(g, r), (W.name, chunk, overlap)
     plan.destroy()
+
+
+def test_chunked_multi_stream_step_replays_from_a_cuda_graph():
+    """the fork / join over the plan's internal streams is capturable: one graph launch = one step, bit for bit"""
+    W = wl.random_case(128, 16, 32, PER, 10.0, 23)
+    plan = plan_for(W)
+    pristine = [to_dev(a) for a in W.fields()]
+    d = [t.clone() for t in pristine]
+    plan.projection_step(*d, W.dt)
+    torch.cuda.synchronize()
+    want = [d[i].cpu().numpy() for i in (0, 1, 2, 4)]
+    plan.set_option("chunk", 8)
+    plan.set_option("overlap", 1)
+    for t, src in zip(d, pristine):
+        t.copy_(src)
+    plan.projection_step(*d, W.dt)                            # creates the internal streams and events outside capture
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        s.synchronize()
+        g.capture_begin()
+        plan.projection_step_ex(*d, d[4], W.dt, 1.0, stream=s.cuda_stream)
+        g.capture_end()
+    torch.cuda.synchronize()
+    for rep in range(2):
+        for t, src in zip(d, pristine):
+            t.copy_(src)
+        g.replay()
+        torch.cuda.synchronize()
+        for i, ref in zip((0, 1, 2, 4), want):
+            assert np.array_equal(d[i].cpu().numpy(), ref), rep
+    plan.destroy()
