@@ -126,8 +126,6 @@ static double host_lambda(int m, int n, double d) {
     return (double)(-2.0L * (1.0L - cosl(two_pi * (long double)m / (long double)n))) / (d * d);
 }
 
-static double host_lambda(int m, int n, double d);
-static int host_freq_of_pos(int n, int pos);
 // eigenvalues along y in the storage order of the transform in use (the 16 x 8 x 8 kernel has its own digit order)
 static int upload_lam_y(flutas_plan *pl) {
     std::vector<double> lam(pl->ny);
