@@ -133,3 +133,29 @@ def test_chunked_multi_stream_step_replays_from_a_cuda_graph():
         for i, ref in zip((0, 1, 2, 4), want):
             assert np.array_equal(d[i].cpu().numpy(), ref), rep
     plan.destroy()
+
+
+def test_plans_release_their_device_memory():
+    """create / use / destroy in a loop (every variant that allocates lazily touched once): free device memory returns"""
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free0, _ = torch.cuda.mem_get_info()
+    for rep in range(6):
+        for bc, nz in ((PER, 64), (WALL, 50)):
+            W = wl.random_case(128, 64, nz, bc, 3.0, 30 + rep)
+            plan = plan_for(W)
+            if bc == WALL:
+                plan.set_option("thomas", rep % 2)          # the two-sweep form allocates c' on first use
+            plan.set_option("chunk", 8 * (rep % 2))
+            plan.set_option("overlap", rep % 2)             # internal streams and events
+            plan.set_timing(rep % 2 == 0)
+            d = [to_dev(x) for x in W.fields()]
+            plan.projection_step(*d, W.dt)
+            torch.cuda.synchronize()
+            assert torch.isfinite(d[4]).all()
+            plan.destroy()
+            del d
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free0 - free1 < 64 * 2**20, (free0, free1)
