@@ -189,6 +189,14 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
         "workspace_gib": round(plan.workspace_bytes / 2**30, 2),
     }
 
+    if not args.no_compare_torch and not args.no_e2e and W.bc_z == 0 and world == 1 and with_e2e:
+        fresh = [torch.from_numpy(a).cuda() for a in host]
+        plan.projection_step(*fresh, W.dt)
+        torch.cuda.synchronize()
+        out["comparison"] = torch_comparison(W, [fresh[i] for i in (0, 1, 2, 4)])
+        del fresh
+        torch.cuda.empty_cache()
+
     if with_e2e:
         # end to end through the host entry point of the C ABI: pinned host buffers, H2D of the six inputs
         # and D2H of u, v, w, p inside the timed region, every step
@@ -213,6 +221,69 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     del dev
     torch.cuda.empty_cache()
     return out
+
+
+def torch_cufft_step(u, v, w, phi, p, po, box, rho1, rho2, dt):
+    """COMPARISON ONLY (never on the product path, not the oracle): the same triply periodic projection step written
+    the obvious way with library calls -- torch.roll stencils + torch.fft.rfftn / irfftn (cuFFT).  Returns u, v, w, p."""
+    import math
+    import torch
+    nz, ny, nx = u.shape
+    dx, dy, dz = box[0] / nx, box[1] / ny, box[2] / nz
+    rho0 = min(rho1, rho2)
+    rc = rho1 * phi + rho2 * (1.0 - phi)
+    ph = 2.0 * p - po
+    fx = (1.0 - rho0 / (0.5 * (rc + torch.roll(rc, -1, 2)))) * (torch.roll(ph, -1, 2) - ph) / dx
+    fy = (1.0 - rho0 / (0.5 * (rc + torch.roll(rc, -1, 1)))) * (torch.roll(ph, -1, 1) - ph) / dy
+    fz = (1.0 - rho0 / (0.5 * (rc + torch.roll(rc, -1, 0)))) * (torch.roll(ph, -1, 0) - ph) / dz
+    del rc, ph
+    up, vp, wp = u + (dt / rho0) * fx, v + (dt / rho0) * fy, w + (dt / rho0) * fz
+    del fx, fy, fz
+    rhs = (rho0 / dt) * ((up - torch.roll(up, 1, 2)) / dx + (vp - torch.roll(vp, 1, 1)) / dy + (wp - torch.roll(wp, 1, 0)) / dz)
+    lam = lambda n, d, m: -2.0 * (1.0 - torch.cos(2.0 * math.pi * torch.arange(m, device=u.device, dtype=torch.float64) / n)) / (d * d)
+    den = lam(nz, dz, nz)[:, None, None] + lam(ny, dy, ny)[None, :, None] + lam(nx, dx, nx // 2 + 1)[None, None, :]
+    den[0, 0, 0] = 1.0
+    spec = torch.fft.rfftn(rhs) / den
+    spec[0, 0, 0] = 0.0
+    del rhs, den
+    pn = torch.fft.irfftn(spec, s=(nz, ny, nx))
+    del spec
+    c = dt / rho0
+    return (up - c * (torch.roll(pn, -1, 2) - pn) / dx, vp - c * (torch.roll(pn, -1, 1) - pn) / dy,
+            wp - c * (torch.roll(pn, -1, 0) - pn) / dz, pn)
+
+
+def torch_comparison(W, ours, steps=5):
+    """times torch_cufft_step on the same device-resident inputs and reports how far its result is from ours"""
+    import torch
+    d = [torch.from_numpy(a).cuda() for a in W.fields()]
+    args = (*d, W.box, W.rho1, W.rho2, W.dt)
+    ref = torch_cufft_step(*args)
+    errs = {n: float((a - b).norm() / b.norm()) for n, a, b in zip("uvwp", ours, ref)}
+    del ref
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        out = torch_cufft_step(*args)
+        del out
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    # the transforms alone: rfftn + irfftn of one field (our five transform kernels do this plus the division)
+    nz, ny, nx = d[0].shape
+    e0.record()
+    for _ in range(steps):
+        sp = torch.fft.rfftn(d[0])
+        back = torch.fft.irfftn(sp, s=(nz, ny, nx))
+        del sp, back
+    e1.record()
+    torch.cuda.synchronize()
+    ms_fft = e0.elapsed_time(e1) / steps
+    return {"cufft_rfftn_irfftn_ms": round(ms_fft, 3), "kind": "COMPARISON ONLY: the same periodic step with torch.roll stencils + torch.fft.rfftn/irfftn (cuFFT), "
+                    "inputs resident, out of place", "ms_per_step": round(ms, 3),
+            "value": round(W.npts / (ms * 1e-3) / 1e6, 1), "unit": UNIT, "steps": steps,
+            "rel_l2_ours_vs_it": {k: float("%.2e" % v) for k, v in errs.items()}}
 
 
 def oracle_sample(threads=0):
@@ -286,6 +357,7 @@ def main():
     ap.add_argument("--e2e-all", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    ap.add_argument("--no-compare-torch", action="store_true", help="skip the torch/cuFFT statement of the periodic step (comparison only)")
     ap.add_argument("--opt", action="append", help="plan tuning knob name=value (experiments)")
     args = ap.parse_args()
     if args.impl == "reference":
