@@ -642,7 +642,7 @@ static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const 
     const int kc = pl->rhs_kc < nk ? pl->rhs_kc : nk;
     dim3 block(bx, ty), grid(pl->nx / 2 / bx, pl->ny / ty, (nk + kc - 1) / kc);
     if (rhs_takes_ranges(pl)) {
-        // bulk-copy-fed form: tile = 128 x 4 cells, three plane slabs in shared memory
+        // bulk-copy-fed form: tile = 128 x 8 cells, three plane slabs in shared memory
         const dim3 b3(Rhs3Geom::NTX, Rhs3Geom::TY), g3(pl->nx / Rhs3Geom::X, pl->ny / Rhs3Geom::TY, (nk + kc - 1) / kc);
         auto k3 = pl->bc_z == FLUTAS_BC_Z_WALL ? splitting_rhs_kernel3<true> : splitting_rhs_kernel3<false>;
         if (set_smem(k3, Rhs3Geom::SMEM) != cudaSuccess) return check_launch(cudaGetLastError(), "splitting_rhs attr");
