@@ -757,7 +757,7 @@ static int enqueue_correction(flutas_plan *pl, double dt, const double *pn, doub
                               cudaStream_t st, int k0, int k1) {
     if (k1 <= k0) return FLUTAS_OK;
     const long long plane = (long long)pl->nx * pl->ny, q0 = k0 * plane, q1 = k1 * plane;
-    const unsigned nb = (unsigned)((q1 - q0 + 255) / 256);
+    const unsigned nb = (unsigned)(((q1 - q0) / 2 + 255) / 256);   // two points per thread
     correction_kernel<<<nb, 256, 0, st>>>(pl->grid, dt, q0, q1, pn, pl->up, pl->vp, pl->wp, u, v, w);
     return check_launch(cudaGetLastError(), "correction");
 }

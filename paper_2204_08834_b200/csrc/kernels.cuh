@@ -304,21 +304,25 @@ __global__ void __launch_bounds__(256)
 correction_kernel(GridParams g, double dt, long long q0, long long q1, const double *__restrict__ pn,
                   const double *__restrict__ up, const double *__restrict__ vp, const double *__restrict__ wp,
                   double *__restrict__ u, double *__restrict__ v, double *__restrict__ w) {
-    const long long q = q0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;   // this launch covers points q0 .. q1 - 1
+    // two consecutive x points per thread (nx is even and q0 a multiple of nx): 16-byte loads and streaming stores
+    const long long q = q0 + 2 * ((long long)blockIdx.x * blockDim.x + threadIdx.x);   // this launch covers points q0 .. q1 - 1
     if (q >= q1) return;
     const int i = (int)(q % g.nx);
     const long long r = q / g.nx;
     const int j = (int)(r % g.ny), k = (int)(r / g.ny);
     const long long sy = g.nx, sz = (long long)g.nx * g.ny;
-    const long long qip = (i + 1 == g.nx) ? q - (g.nx - 1) : q + 1;
+    const long long qip = (i + 2 == g.nx) ? q - (g.nx - 2) : q + 2;
     const long long qjp = (j + 1 == g.ny) ? q - (g.ny - 1) * sy : q + sy;
     const long long qkp = (k + 1 == g.nz) ? q - (g.nz - 1) * sz : q + sz;
     const bool top = g.wall && (k + 1 == g.nz);
     const double c = dt / g.rho0;
-    const double pc = pn[q];
-    u[q] = up[q] - c * ((pn[qip] - pc) * g.inv_dx);
-    v[q] = vp[q] - c * ((pn[qjp] - pc) * g.inv_dy);
-    w[q] = top ? wp[q] : wp[q] - c * ((pn[qkp] - pc) * g.inv_dz);
+    auto ld2 = [](const double *f, long long a) { return *reinterpret_cast<const double2 *>(f + a); };
+    const double2 pc = ld2(pn, q), pj = ld2(pn, qjp), pk = ld2(pn, qkp);
+    const double pe = pn[qip];
+    const double2 a = ld2(up, q), b = ld2(vp, q), d = ld2(wp, q);
+    stcs2(u, q, make_double2(a.x - c * ((pc.y - pc.x) * g.inv_dx), a.y - c * ((pe - pc.y) * g.inv_dx)));
+    stcs2(v, q, make_double2(b.x - c * ((pj.x - pc.x) * g.inv_dy), b.y - c * ((pj.y - pc.y) * g.inv_dy)));
+    stcs2(w, q, top ? d : make_double2(d.x - c * ((pk.x - pc.x) * g.inv_dz), d.y - c * ((pk.y - pc.y) * g.inv_dz)));
 }
 
 // ------------------------------------------------------------------------------------------------
