@@ -28,6 +28,11 @@
  * All functions are extern "C", never throw and never call exit().  Unless a parameter says HOST,
  * pointers are DEVICE pointers.  The library never prints, reads no environment variable and has no
  * CPU fallback: without a CUDA device every call below fails with FLUTAS_ERR_CUDA / NULL.
+ *
+ * Arithmetic: fp64 throughout, no --use_fast_math.  The two reciprocals on the path -- 1/(rho_a + rho_b) of a face and
+ * 1/(lambda_x + lambda_y + lambda_z) of a mode -- are the hardware seed (rcp.approx.ftz.f64) refined by two Newton
+ * steps: relative error <= ~1 ulp, not the correctly rounded IEEE quotient (measured against the divide-based
+ * CPU definition: <= 1e-14 relative L2 on every field).  The seed flushes subnormals, hence the density range below.
  */
 #ifndef FLUTAS_H
 #define FLUTAS_H
@@ -41,6 +46,11 @@ extern "C" {
 typedef struct flutas_plan flutas_plan;
 
 enum { FLUTAS_BC_Z_PERIODIC = 0, FLUTAS_BC_Z_WALL = 1 };
+/* boundary conditions (the same values, for any direction) */
+enum { FLUTAS_BC_PERIODIC = 0, FLUTAS_BC_NEUMANN = 1 };
+
+/* flags of flutas_plan_create_ex */
+enum { FLUTAS_PLAN_CALLER_WORKSPACE = 1 };   /* do not allocate the workspace: flutas_plan_set_workspace supplies it */
 
 enum {
     FLUTAS_OK = 0,
@@ -52,16 +62,40 @@ enum {
 };
 
 /* Create a plan for an nx x ny x nz grid on a box lx x ly x lz, on the CURRENT CUDA device.
- *   sizes:  nx, ny powers of two, 16 <= nx <= 2048, 8 <= ny <= 2048;
- *           bc_z periodic: nz a power of two, 8 <= nz <= 2048;  bc_z wall: any nz >= 2.
- *   rho1, rho2 > 0: densities of phase 1 (phi = 1) and phase 2 (phi = 0); rho0 = min(rho1, rho2)
- *           (R3, R11).
- * The plan owns, on the device: twiddle and (permuted) eigenvalue tables, and a workspace of
- * flutas_plan_workspace_bytes() (one padded half-spectrum + the intermediate fields).
+ *   sizes:  nx, ny powers of two, 8 <= nx, ny <= 2048;
+ *           bc_z periodic: nz a power of two, 8 <= nz <= 2048;  bc_z wall: any 2 <= nz <= 4096.
+ *   rho1, rho2 in [1e-100, 1e100]: densities of phase 1 (phi = 1) and phase 2 (phi = 0);
+ *           rho0 = min(rho1, rho2) (R3, R11).  With rho1 == rho2 the splitting
+ *           coefficient (1 - rho0/rho_f) is exactly 0 (the classical constant-density projection).
+ * The plan owns, on the device: twiddle and (permuted) eigenvalue tables (kilobytes), and -- unless
+ * flutas_plan_create_ex was told FLUTAS_PLAN_CALLER_WORKSPACE -- a workspace of flutas_plan_workspace_bytes()
+ * (one padded half-spectrum, four intermediate fields and, with walls, the elimination-coefficient table).
  * Returns NULL on failure; flutas_last_error() / flutas_last_error_code() say why.
  * A plan may be reused for any number of steps; one step in flight per plan (shared workspace). */
 flutas_plan *flutas_plan_create(int nx, int ny, int nz, double lx, double ly, double lz,
                                 int bc_z, double rho1, double rho2);
+
+/* flutas_plan_create with boundary conditions along x and y and flags (same problem).
+ *   bc_x, bc_y: FLUTAS_BC_PERIODIC (what flutas_plan_create passes); see "boundary conditions" above.
+ *   FLUTAS_PLAN_CALLER_WORKSPACE: the plan allocates its small tables only; before the first step the caller hands it
+ *   a device buffer with flutas_plan_set_workspace (e.g. one torch tensor, so that the framework's allocator
+ *   accounts for every large byte).  A step on a plan without a workspace fails with FLUTAS_ERR_INVALID_ARG. */
+flutas_plan *flutas_plan_create_ex(int nx, int ny, int nz, double lx, double ly, double lz,
+                                   int bc_x, int bc_y, int bc_z, double rho1, double rho2, unsigned flags);
+
+/* Bytes of workspace a plan for this grid needs (no plan, no device needed; 0 for an unsupported grid):
+ * the number flutas_plan_workspace_bytes returns for such a plan.  PAPER.md:146-163 (sizes the solve of eq. 17). */
+size_t flutas_workspace_bytes(int nx, int ny, int nz, int bc_x, int bc_y, int bc_z);
+
+/* Make the plan use the caller's device buffer [dev_ptr, dev_ptr + bytes) as its workspace (the
+ * intermediate arrays of eqs. 16-18 and of the solver steps 1-9).
+ *   dev_ptr: device memory, 256-byte aligned, bytes >= flutas_plan_workspace_bytes(plan); the caller keeps
+ *            ownership and must keep it alive and otherwise unused while the plan may run; contents need not be
+ *            preserved between steps by the caller, but are (the coefficient table of the wall solve lives there).
+ *   dev_ptr == NULL: go back to a plan-owned workspace (allocated here).
+ * Synchronises the device, releases a plan-owned workspace, rebuilds the tensor maps and the wall coefficient
+ * table.  FLUTAS_ERR_INVALID_ARG for a misaligned or too small buffer. */
+int flutas_plan_set_workspace(flutas_plan *plan, void *dev_ptr, size_t bytes);
 
 /* One projection step, enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy
  * default stream).  Returns without synchronising; no device<->host copy is made.
@@ -125,13 +159,17 @@ int flutas_poisson_solve(flutas_plan *plan, const double *rhs, double *p_out, vo
 const char *flutas_last_error(void);
 int flutas_last_error_code(void);
 
-/* Device bytes owned by the plan (tables + workspace; staging buffers of the _host entry excluded). */
+/* Bytes of workspace the plan needs (== flutas_workspace_bytes of its grid), whoever owns it; the plan's tables
+ * (kilobytes) and the staging buffers of the _host entry are not included. */
 size_t flutas_plan_workspace_bytes(const flutas_plan *plan);
 
 /* Number of kernel launches one flutas_projection_step enqueues, and their names
  * (idx in [0, launches); returns NULL outside). */
 int flutas_plan_kernel_launches(const flutas_plan *plan);
 const char *flutas_plan_kernel_name(const flutas_plan *plan, int idx);
+/* The device function launch idx runs with the plan as it is configured now (the name a profiler shows, without
+ * template arguments), so that stored profiler captures can be matched to the code that is running. */
+const char *flutas_plan_kernel_symbol(const flutas_plan *plan, int idx);
 
 /* Per-kernel device timing.  flutas_plan_set_timing(plan, 1) makes every following step record a
  * CUDA event before and after each of its kernels on the step's stream (events only; no
@@ -146,17 +184,17 @@ int flutas_plan_read_timing(flutas_plan *plan, float *ms_out, int n_out, int *st
  * and write once; used by bench.py for the roofline line. */
 double flutas_plan_kernel_bytes(const flutas_plan *plan, int idx);
 
-/* Tuning knobs for experiments (never needed for correctness; every combination is held to the same parity tests,
- * tests/test_gpu_variants.py).  Returns FLUTAS_ERR_INVALID_ARG for an unknown name or a value the plan cannot take.
- *   "y_cols" / "z_cols" = 4 | 8   kx columns one CTA transforms in the y / z pass (fft_tma1_kernel)
+/* Kernel variants a plan can switch between (never needed for correctness; every value of every option is held to
+ * the same parity tests in tests/test_gpu_variants.py).  FLUTAS_ERR_INVALID_ARG for an unknown name or a value the plan
+ * cannot take.
  *   "y16" = 0 | 1                 ny = 1024 only: 1 (default) = 16 x 8 x 8 register-resident kernel, 0 = 4-column path.
  *                                 Switching re-orders the eigenvalue tables (synchronises the device).
  *   "thomas" = 0 | 1              wall only: 1 (default when nz <= 512) = one-pass shared-memory elimination,
- *                                 0 = two sweeps through HBM (allocates its c' array on first use)
+ *                                 0 = two sweeps through HBM (allocates its c' array, half a spectrum, on first use;
+ *                                 plan-owned, outside the workspace)
  *   "thomas_warps" = 1 | 2        solving warps per CTA of the one-pass kernel (default 2)
  *   "chunk" = n >= 0              planes per launch group of the step (0, default: every kernel covers the grid)
- *   "overlap" = 0 | 1             chunked only: run the three kernels of a group on three internal streams
- *   "tma", "x_variant", "rhs_variant", "rhs_kc", "rhs_bx"   older forms of the kernels, kept for A/B measurements */
+ *   "overlap" = 0 | 1             chunked only: run the three kernels of a group on three internal streams */
 int flutas_plan_set_option(flutas_plan *plan, const char *name, int value);
 
 #ifdef __cplusplus

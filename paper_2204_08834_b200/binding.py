@@ -10,12 +10,23 @@ from .build import build as _build
 
 BC_Z_PERIODIC = 0
 BC_Z_WALL = 1
+BC_PERIODIC = 0
+BC_NEUMANN = 1
+PLAN_CALLER_WORKSPACE = 1
 
 _vp, _ci, _cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
 lib = ctypes.CDLL(_build())
 
 lib.flutas_plan_create.argtypes = [_ci, _ci, _ci, _cd, _cd, _cd, _ci, _cd, _cd]
 lib.flutas_plan_create.restype = _vp
+lib.flutas_plan_create_ex.argtypes = [_ci, _ci, _ci, _cd, _cd, _cd, _ci, _ci, _ci, _cd, _cd, ctypes.c_uint]
+lib.flutas_plan_create_ex.restype = _vp
+lib.flutas_workspace_bytes.argtypes = [_ci] * 6
+lib.flutas_workspace_bytes.restype = ctypes.c_size_t
+lib.flutas_plan_set_workspace.argtypes = [_vp, _vp, ctypes.c_size_t]
+lib.flutas_plan_set_workspace.restype = _ci
+lib.flutas_plan_kernel_symbol.argtypes = [_vp, _ci]
+lib.flutas_plan_kernel_symbol.restype = ctypes.c_char_p
 lib.flutas_plan_destroy.argtypes = [_vp]
 lib.flutas_plan_destroy.restype = None
 lib.flutas_projection_step.argtypes = [_vp] * 7 + [_cd, _vp]
@@ -55,6 +66,7 @@ EXPORTS = [
     "flutas_plan_workspace_bytes", "flutas_plan_kernel_launches", "flutas_plan_kernel_name",
     "flutas_plan_set_timing", "flutas_plan_read_timing", "flutas_plan_kernel_bytes", "flutas_plan_set_option",
     "flutas_projection_step_ex", "flutas_splitting_rhs_ex",
+    "flutas_plan_create_ex", "flutas_workspace_bytes", "flutas_plan_set_workspace", "flutas_plan_kernel_symbol",
 ]
 
 
@@ -86,23 +98,54 @@ def _stream():
     return torch.cuda.current_stream().cuda_stream
 
 
-class Plan:
-    """flutas_plan_create / flutas_projection_step / flutas_plan_destroy with the same argument order."""
+def workspace_bytes(nx, ny, nz, bc_z, bc_x=BC_PERIODIC, bc_y=BC_PERIODIC):
+    """flutas_workspace_bytes: what a plan for this grid needs (0 = unsupported grid); no device needed"""
+    return lib.flutas_workspace_bytes(int(nx), int(ny), int(nz), int(bc_x), int(bc_y), int(bc_z))
 
-    def __init__(self, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2):
+
+class Plan:
+    """flutas_plan_create / flutas_projection_step / flutas_plan_destroy with the same argument order.
+
+    workspace="torch" (default): the plan is created with FLUTAS_PLAN_CALLER_WORKSPACE and handed one uint8 torch
+    tensor (flutas_plan_set_workspace), so that every large device byte goes through torch's allocator;
+    workspace="library": flutas_plan_create allocates it with cudaMalloc (what a C caller of the three north-star
+    calls gets); workspace=<uint8 CUDA tensor>: that buffer."""
+
+    def __init__(self, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, bc_x=BC_PERIODIC, bc_y=BC_PERIODIC, workspace="torch"):
         self._h = None
-        h = lib.flutas_plan_create(int(nx), int(ny), int(nz), float(lx), float(ly), float(lz), int(bc_z),
-                                   float(rho1), float(rho2))
+        self._ws = None
+        args = (int(nx), int(ny), int(nz), float(lx), float(ly), float(lz))
+        if isinstance(workspace, str) and workspace == "library":
+            if bc_x == BC_PERIODIC and bc_y == BC_PERIODIC:
+                h = lib.flutas_plan_create(*args, int(bc_z), float(rho1), float(rho2))
+            else:
+                h = lib.flutas_plan_create_ex(*args, int(bc_x), int(bc_y), int(bc_z), float(rho1), float(rho2), 0)
+        else:
+            h = lib.flutas_plan_create_ex(*args, int(bc_x), int(bc_y), int(bc_z), float(rho1), float(rho2),
+                                          PLAN_CALLER_WORKSPACE)
         if not h:
             _raise_last()
         self._h = h
         self.nx, self.ny, self.nz, self.bc_z = int(nx), int(ny), int(nz), int(bc_z)
         self.npts = self.nx * self.ny * self.nz
+        if not (isinstance(workspace, str) and workspace == "library"):
+            import torch
+            ws = torch.empty(self.workspace_bytes, dtype=torch.uint8, device="cuda") if isinstance(workspace, str) else workspace
+            self.set_workspace(ws)
+
+    def set_workspace(self, ws):
+        """ws: a contiguous uint8 CUDA tensor of at least workspace_bytes (kept alive by the plan), or None = library-owned"""
+        if ws is None:
+            _check(lib.flutas_plan_set_workspace(self._h, None, 0))
+        else:
+            _check(lib.flutas_plan_set_workspace(self._h, ws.data_ptr(), ws.numel() * ws.element_size()))
+        self._ws = ws
 
     def destroy(self):
         if self._h:
             lib.flutas_plan_destroy(self._h)
             self._h = None
+            self._ws = None
 
     def __del__(self):
         try:
@@ -149,6 +192,11 @@ class Plan:
     def kernel_names(self):
         n = lib.flutas_plan_kernel_launches(self._h)
         return [lib.flutas_plan_kernel_name(self._h, i).decode() for i in range(n)]
+
+    @property
+    def kernel_symbols(self):
+        n = lib.flutas_plan_kernel_launches(self._h)
+        return [lib.flutas_plan_kernel_symbol(self._h, i).decode() for i in range(n)]
 
     @property
     def kernel_bytes(self):

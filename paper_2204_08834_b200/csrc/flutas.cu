@@ -1,7 +1,9 @@
 // flutas.cu -- plan, launch sequence and C ABI of libflutas_b200.so (see include/flutas.h).
 //
-// build: nvcc -O3 -std=c++17 -gencode arch=compute_100a,code=sm_100a -lineinfo -Xcompiler -fPIC
-//        -shared (no --use_fast_math: fp64 division / reciprocal stay IEEE)  -- see ../build.py
+// build: nvcc -O3 -std=c++17 -gencode arch=compute_100a,code=sm_100a -lineinfo -Xcompiler -fPIC -shared -- see ../build.py
+//        No --use_fast_math.  Host-side tables use IEEE divisions; on the device the face-density and eigenvalue
+//        reciprocals are rcp.approx.ftz.f64 + two Newton steps (<= ~1 ulp; rcp_density, rcp_normal), everything else
+//        is plain fp64 add / mul / fma.
 #include "flutas.h"
 
 #include <cmath>
@@ -65,25 +67,25 @@ struct flutas_plan {
     double *ttab;                // wall: elimination coefficients of the one-pass solve, [tile][j][8] (kernels_thomas.cuh)
     int thomas_warps;            // solving warps per CTA of the one-pass kernel (1 or 2)
     int thomas_variant;          // wall: 1 = one-pass shared-memory solve (nz <= 512), 0 = two sweeps through HBM
-    size_t bytes;
+    size_t bytes;                // workspace bytes this plan needs (layout: plan_carve)
+    void *ws_base;               // start of the workspace in use (plan-owned or the caller's), nullptr = none yet
+    bool ws_owned;               // true: ws_base came from cudaMalloc here and is freed by the plan
+    bool cp_owned;               // the c' array of the two-sweep option was allocated on demand (outside the workspace)
     // staging for the host entry point
     double *stage[6];
     // launch list
     int n_launch;
     int launch_ids[K_MAX];
     // tuning
-    int y_cols, z_cols;          // tile width (columns of kx) of the strided passes
+    int y_cols, z_cols;          // tile width (columns of kx) of the strided passes: 8, or 4 for lines of >= 1024
     int rhs_kc;                  // planes one thread of the RHS kernel marches through
-    int x_variant;               // x transforms: 1 = persistent bulk-copy-fed kernels (nx = 128..1024), 0 = staged kernels
     int chunk;                   // planes per launch group of the step (0 = whole grid per kernel)
     int overlap;                 // chunked only: 1 = the three kernels of a group run on three internal streams (low, mid, high
                                  // priority; producer -> consumer), so groups overlap and tails are filled
     cudaStream_t lane[3];        // internal streams, created on first use
     cudaEvent_t ev_fork, *ev_dep;   // fork from the caller's stream; ev_dep[2 * chunk_index + {0, 1}]
     int n_dep;
-    int rhs_variant, rhs_bx;     // 3 = bulk-copy-fed kernel (default), 2 = software-pipelined register form, 1 = first form; threads along x per block (forms 1, 2)
     int y16;                     // ny = 1024: 1 = register-resident 16 x 8 x 8 kernel (kernels_y16.cuh), 0 = fft_tma1_kernel on 4 columns
-    int use_tma;                 // strided passes: 1 = TMA prefetch + register-resident twiddles (default), 2 = generic TMA in/out, 0 = plain loads
     int num_sms;
     CUtensorMap map_y, map_z;    // boxes {2*y_cols, rows, 1} and {2*z_cols, 1, rows} over the half-spectrum
     // timing
@@ -192,12 +194,45 @@ static int plan_make_maps(flutas_plan *pl) {
     return FLUTAS_OK;
 }
 
-static int plan_build(flutas_plan *pl) {
+// ---- sizes: everything that follows from (nx, ny, nz, bc_z) alone, no device needed
+static bool sizes_supported(int nx, int ny, int nz, int bc_x, int bc_y, int bc_z) {
+    if (bc_x != FLUTAS_BC_PERIODIC || bc_y != FLUTAS_BC_PERIODIC) return false;
+    if (bc_z != FLUTAS_BC_Z_PERIODIC && bc_z != FLUTAS_BC_Z_WALL) return false;
+    if (!is_pow2(nx) || nx < 8 || nx > 2048 || !is_pow2(ny) || ny < 8 || ny > 2048) return false;
+    if (bc_z == FLUTAS_BC_Z_WALL) return nz >= 2 && nz <= 4096;
+    return is_pow2(nz) && nz >= 8 && nz <= 2048;
+}
+
+static size_t align_up(size_t x) { return (x + 1023) / 1024 * 1024; }
+
+// Workspace layout, in this order, every part 1024-byte aligned:  spec | rhs | u' | v' | w' | wall: table or c'
+struct WsLayout {
+    size_t spec, rhs, up, vp, wp, zaux, total;
+};
+static WsLayout plan_layout(const flutas_plan *pl) {
+    const size_t fb = sizeof(double) * (size_t)pl->npts, sb = sizeof(double2) * (size_t)pl->nspec;
+    WsLayout w{};
+    size_t o = 0;
+    w.spec = o; o += align_up(sb);
+    w.rhs = o; o += align_up(fb);
+    w.up = o; o += align_up(fb);
+    w.vp = o; o += align_up(fb);
+    w.wp = o; o += align_up(fb);
+    w.zaux = o;
+    if (pl->bc_z == FLUTAS_BC_Z_WALL) {
+        if (ThomasGeom::smem_bytes(pl->nz) <= 227 * 1024) {   // coefficient table of the one-pass solve
+            const int n_tiles_x = (pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C;
+            o += align_up(sizeof(double) * ThomasGeom::tab_doubles(pl->nz) * (size_t)n_tiles_x * pl->ny);
+        } else {                                              // c' of the two sweeps
+            o += align_up(sb / 2);
+        }
+    }
+    w.total = o;
+    return w;
+}
+
+static void plan_geometry(flutas_plan *pl) {
     const int nx = pl->nx, ny = pl->ny, nz = pl->nz;
-    const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
-    const double dx = pl->lx / nx, dy = pl->ly / ny, dz = pl->lz / nz;
-    pl->grid = GridParams{nx, ny, nz, wall ? 1 : 0, 1.0 / dx, 1.0 / dy, 1.0 / dz, pl->rho1, pl->rho2,
-                          pl->rho1 < pl->rho2 ? pl->rho1 : pl->rho2, 2.0, 1.0};
     pl->n2 = nx / 2;
     pl->nxh = nx / 2 + 1;
     pl->pitch = nx / 2 + 8;
@@ -205,41 +240,76 @@ static int plan_build(flutas_plan *pl) {
     // One unused row per plane, so that the stride of a line along z is an odd multiple of the row size instead of
     // (nx/2 + 8) * 16 bytes times a power of two.  Measured effect on the z stage: +3-5 % at 512^3, none at
     // 1024 x 1024 x 512 (the memory system's own address hashing already spreads such strides); kept because it is free.
-    int pad_rows = 1;
-    if (const char *e = getenv("FLUTAS_PLANE_PAD_ROWS")) pad_rows = atoi(e) < 0 ? 0 : atoi(e);   // experiments
-    pl->plane = (long long)pl->pitch * (ny + pad_rows);
+    pl->plane = (long long)pl->pitch * (ny + 1);
     pl->nspec = pl->plane * nz;
+    pl->bytes = plan_layout(pl).total;
+}
 
+// point the plan at a workspace (device memory of at least pl->bytes) and (re)build what lives in it or refers to it
+static int plan_attach_workspace(flutas_plan *pl, void *base, bool owned) {
+    const WsLayout w = plan_layout(pl);
+    char *b = (char *)base;
+    pl->ws_base = base;
+    pl->ws_owned = owned;
+    pl->spec = (double2 *)(b + w.spec);
+    pl->rhs = (double *)(b + w.rhs);
+    pl->up = (double *)(b + w.up);
+    pl->vp = (double *)(b + w.vp);
+    pl->wp = (double *)(b + w.wp);
+    if (!pl->cp_owned) pl->cp = nullptr;
+    pl->ttab = nullptr;
+    // padding columns / the pad row of the spectrum are read (never used) by the strided kernels: keep them finite
+    CUDA_TRY(cudaMemset(pl->spec, 0, sizeof(double2) * (size_t)pl->nspec));
+    if (pl->bc_z == FLUTAS_BC_Z_WALL) {
+        if (ThomasGeom::smem_bytes(pl->nz) <= 227 * 1024) {
+            pl->ttab = (double *)(b + w.zaux);
+            if (int rc = build_thomas_table(pl)) return rc;
+        } else if (!pl->cp_owned) {
+            pl->cp = (double *)(b + w.zaux);
+        }
+    }
+    return plan_make_maps(pl);
+}
+
+static void plan_detach_workspace(flutas_plan *pl) {
+    if (pl->ws_owned && pl->ws_base) cudaFree(pl->ws_base);
+    pl->ws_base = nullptr;
+    pl->ws_owned = false;
+    pl->spec = nullptr;
+    pl->rhs = pl->up = pl->vp = pl->wp = pl->ttab = nullptr;
+    if (!pl->cp_owned) pl->cp = nullptr;
+}
+
+static int plan_build(flutas_plan *pl, unsigned flags) {
+    const int nx = pl->nx, ny = pl->ny, nz = pl->nz;
+    const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
+    const double dx = pl->lx / nx, dy = pl->ly / ny, dz = pl->lz / nz;
+    const bool same_rho = pl->rho1 == pl->rho2;    // (1 - rho0/rho_f) is then exactly 0 (flux_coef)
+    pl->grid = GridParams{nx, ny, nz, wall ? 1 : 0, 1.0 / dx, 1.0 / dy, 1.0 / dz, pl->rho1, pl->rho2,
+                          pl->rho1 < pl->rho2 ? pl->rho1 : pl->rho2, 2.0, 1.0, same_rho ? 0.0 : 1.0};
+    plan_geometry(pl);
+
+    size_t tb = 0;   // table bytes (not part of the workspace)
     std::vector<double2> t;
     host_twiddles(nx, t);
-    if (int rc = upload(&pl->tw_x, t, &pl->bytes)) return rc;
+    if (int rc = upload(&pl->tw_x, t, &tb)) return rc;
     host_twiddles(ny, t);
-    if (int rc = upload(&pl->tw_y, t, &pl->bytes)) return rc;
+    if (int rc = upload(&pl->tw_y, t, &tb)) return rc;
     if (!wall) {
         host_twiddles(nz, t);
-        if (int rc = upload(&pl->tw_z, t, &pl->bytes)) return rc;
+        if (int rc = upload(&pl->tw_z, t, &tb)) return rc;
     }
     std::vector<double> lam(pl->pitch, 1.0);
     for (int k = 0; k <= pl->n2; ++k) lam[k] = host_lambda(k, nx, dx);   // x columns are stored in natural order
-    if (int rc = upload(&pl->lam_x, lam, &pl->bytes)) return rc;
+    if (int rc = upload(&pl->lam_x, lam, &tb)) return rc;
     pl->y16 = ny == Y16Geom::N ? 1 : 0;
     CUDA_TRY(cudaMalloc((void **)&pl->lam_y, sizeof(double) * ny));
-    pl->bytes += sizeof(double) * ny;
     if (int rc = upload_lam_y(pl)) return rc;
     if (!wall) {
         lam.assign(nz, 0.0);
         for (int pos = 0; pos < nz; ++pos) lam[pos] = host_lambda(host_freq_of_pos(nz, pos), nz, dz);
-        if (int rc = upload(&pl->lam_z, lam, &pl->bytes)) return rc;
+        if (int rc = upload(&pl->lam_z, lam, &tb)) return rc;
     }
-
-    const size_t fb = sizeof(double) * (size_t)pl->npts, sb = sizeof(double2) * (size_t)pl->nspec;
-    CUDA_TRY(cudaMalloc((void **)&pl->spec, sb));
-    CUDA_TRY(cudaMemset(pl->spec, 0, sb));
-    CUDA_TRY(cudaMalloc((void **)&pl->rhs, fb));
-    CUDA_TRY(cudaMalloc((void **)&pl->up, fb));
-    CUDA_TRY(cudaMalloc((void **)&pl->vp, fb));
-    CUDA_TRY(cudaMalloc((void **)&pl->wp, fb));
-    pl->bytes += sb + 4 * fb;
     if (wall) {
         // the (0,0) column: lam = 0; the elimination coefficients do not depend on the data (same recurrence, same
         // IEEE divisions as a per-step evaluation would do)
@@ -253,19 +323,9 @@ static int plan_build(flutas_plan *pl) {
             sc[2 * k] = inv; sc[2 * k + 1] = cpv;
         }
         sc[2 * (size_t)nz - 1] = a;
-        if (int rc = upload(&pl->sing_coef, sc, &pl->bytes)) return rc;
+        if (int rc = upload(&pl->sing_coef, sc, &tb)) return rc;
         pl->thomas_variant = ThomasGeom::smem_bytes(nz) <= 227 * 1024 ? 1 : 0;
         pl->thomas_warps = 2;
-        if (pl->thomas_variant == 1) {
-            const int n_tiles_x = (pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C;
-            const size_t tb = sizeof(double) * ThomasGeom::tab_doubles(nz) * (size_t)n_tiles_x * ny;
-            CUDA_TRY(cudaMalloc((void **)&pl->ttab, tb));
-            pl->bytes += tb;
-            if (int rc = build_thomas_table(pl)) return rc;
-        } else {
-            CUDA_TRY(cudaMalloc((void **)&pl->cp, sb / 2));
-            pl->bytes += sb / 2;
-        }
     }
 
     int n = 0;
@@ -281,33 +341,38 @@ static int plan_build(flutas_plan *pl) {
     pl->y_cols = ny >= 1024 ? 4 : 8;
     pl->z_cols = nz >= 1024 ? 4 : 8;
     pl->rhs_kc = 32;
-    pl->rhs_variant = 3;   // falls back to the second form when nx % 128 or ny % 4 is non-zero
-    pl->x_variant = 1;
-    pl->rhs_bx = 64;
-    pl->use_tma = 1;
     int dev = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&pl->num_sms, cudaDevAttrMultiProcessorCount, dev));
-    if (int rc = plan_make_maps(pl)) return rc;
+    if (flags & FLUTAS_PLAN_CALLER_WORKSPACE) return FLUTAS_OK;   // flutas_plan_set_workspace supplies it
+    void *base = nullptr;
+    CUDA_TRY(cudaMalloc(&base, pl->bytes));
+    if (int rc = plan_attach_workspace(pl, base, true)) return rc;
     return FLUTAS_OK;
 }
 
-extern "C" flutas_plan *flutas_plan_create(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
-                                           double rho1, double rho2) {
+extern "C" flutas_plan *flutas_plan_create_ex(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y,
+                                              int bc_z, double rho1, double rho2, unsigned flags) {
     if (bc_z != FLUTAS_BC_Z_PERIODIC && bc_z != FLUTAS_BC_Z_WALL) {
         fail(FLUTAS_ERR_INVALID_ARG, "bc_z must be FLUTAS_BC_Z_PERIODIC or FLUTAS_BC_Z_WALL");
         return nullptr;
     }
-    if (!(lx > 0.0) || !(ly > 0.0) || !(lz > 0.0) || !(rho1 > 0.0) || !(rho2 > 0.0) || !std::isfinite(lx + ly + lz + rho1 + rho2)) {
-        fail(FLUTAS_ERR_INVALID_ARG, "box lengths and densities must be positive and finite");
+    if (flags & ~(unsigned)FLUTAS_PLAN_CALLER_WORKSPACE) {
+        fail(FLUTAS_ERR_INVALID_ARG, "unknown flag bits 0x%x", flags);
         return nullptr;
     }
-    const bool wall = bc_z == FLUTAS_BC_Z_WALL;
-    if (!is_pow2(nx) || nx < 16 || nx > 2048 || !is_pow2(ny) || ny < 8 || ny > 2048 ||
-        (wall ? (nz < 2) : (!is_pow2(nz) || nz < 8 || nz > 2048))) {
+    if (!(lx > 0.0) || !(ly > 0.0) || !(lz > 0.0) || !std::isfinite(lx + ly + lz)) {
+        fail(FLUTAS_ERR_INVALID_ARG, "box lengths must be positive and finite");
+        return nullptr;
+    }
+    if (!(rho1 >= 1e-100 && rho1 <= 1e100) || !(rho2 >= 1e-100 && rho2 <= 1e100)) {
+        fail(FLUTAS_ERR_INVALID_ARG, "densities must lie in [1e-100, 1e100]");
+        return nullptr;
+    }
+    if (!sizes_supported(nx, ny, nz, bc_x, bc_y, bc_z)) {
         fail(FLUTAS_ERR_UNSUPPORTED_SIZE,
-             "unsupported grid %d x %d x %d: nx in [16,2048], ny in [8,2048] powers of two; nz power of two in "
-             "[8,2048] (periodic) or >= 2 (wall)", nx, ny, nz);
+             "unsupported grid %d x %d x %d: nx, ny powers of two in [8,2048]; nz a power of two in [8,2048] (periodic) "
+             "or any value in [2,4096] (wall); bc_x, bc_y periodic", nx, ny, nz);
         return nullptr;
     }
     int ndev = 0;
@@ -324,11 +389,42 @@ extern "C" flutas_plan *flutas_plan_create(int nx, int ny, int nz, double lx, do
     memset(pl, 0, sizeof(*pl));
     pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->bc_z = bc_z;
     pl->lx = lx; pl->ly = ly; pl->lz = lz; pl->rho1 = rho1; pl->rho2 = rho2;
-    if (plan_build(pl) != FLUTAS_OK) {
+    if (plan_build(pl, flags) != FLUTAS_OK) {
         flutas_plan_destroy(pl);   // keeps g_err of the failure
         return nullptr;
     }
     return pl;
+}
+
+extern "C" flutas_plan *flutas_plan_create(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                                           double rho1, double rho2) {
+    return flutas_plan_create_ex(nx, ny, nz, lx, ly, lz, FLUTAS_BC_PERIODIC, FLUTAS_BC_PERIODIC, bc_z, rho1, rho2, 0u);
+}
+
+extern "C" size_t flutas_workspace_bytes(int nx, int ny, int nz, int bc_x, int bc_y, int bc_z) {
+    if (!sizes_supported(nx, ny, nz, bc_x, bc_y, bc_z)) return 0;
+    flutas_plan tmp;
+    memset(&tmp, 0, sizeof(tmp));
+    tmp.nx = nx; tmp.ny = ny; tmp.nz = nz; tmp.bc_z = bc_z;
+    plan_geometry(&tmp);
+    return tmp.bytes;
+}
+
+extern "C" int flutas_plan_set_workspace(flutas_plan *pl, void *dev_ptr, size_t bytes) {
+    if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
+    if (dev_ptr) {
+        if (((size_t)dev_ptr) & 255) return fail(FLUTAS_ERR_INVALID_ARG, "the workspace must be 256-byte aligned");
+        if (bytes < pl->bytes)
+            return fail(FLUTAS_ERR_INVALID_ARG, "the workspace is too small: %zu bytes given, %zu needed", bytes, pl->bytes);
+    }
+    CUDA_TRY(cudaDeviceSynchronize());
+    plan_detach_workspace(pl);
+    if (!dev_ptr) {
+        void *base = nullptr;
+        CUDA_TRY(cudaMalloc(&base, pl->bytes));
+        return plan_attach_workspace(pl, base, true);
+    }
+    return plan_attach_workspace(pl, dev_ptr, false);
 }
 
 extern "C" void flutas_plan_destroy(flutas_plan *pl) {
@@ -336,7 +432,9 @@ extern "C" void flutas_plan_destroy(flutas_plan *pl) {
     cudaDeviceSynchronize();
     cudaFree(pl->tw_x); cudaFree(pl->tw_y); cudaFree(pl->tw_z);
     cudaFree(pl->lam_x); cudaFree(pl->lam_y); cudaFree(pl->lam_z);
-    cudaFree(pl->spec); cudaFree(pl->rhs); cudaFree(pl->up); cudaFree(pl->vp); cudaFree(pl->wp); cudaFree(pl->cp); cudaFree(pl->ttab); cudaFree(pl->sing_coef);
+    cudaFree(pl->sing_coef);
+    if (pl->cp_owned) cudaFree(pl->cp);
+    plan_detach_workspace(pl);
     for (int i = 0; i < 6; ++i) cudaFree(pl->stage[i]);
     for (int i = 0; i < 3; ++i) if (pl->lane[i]) cudaStreamDestroy(pl->lane[i]);
     if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
@@ -351,6 +449,9 @@ extern "C" void flutas_plan_destroy(flutas_plan *pl) {
     cudaGetLastError();
     delete pl;
 }
+
+static bool rhs_takes_ranges(const flutas_plan *pl);
+static bool x_is_persistent(const flutas_plan *pl) { return pl->n2 >= 64 && pl->n2 <= 512; }   // nx = 128 .. 1024
 
 extern "C" size_t flutas_plan_workspace_bytes(const flutas_plan *pl) { return pl ? pl->bytes : 0; }
 extern "C" int flutas_plan_kernel_launches(const flutas_plan *pl) { return pl ? pl->n_launch : 0; }
@@ -379,33 +480,44 @@ extern "C" double flutas_plan_kernel_bytes(const flutas_plan *pl, int idx) {
     return 0.0;
 }
 
+extern "C" const char *flutas_plan_kernel_symbol(const flutas_plan *pl, int idx) {
+    if (!pl || idx < 0 || idx >= pl->n_launch) return nullptr;
+    const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
+    switch (pl->launch_ids[idx]) {
+        case K_RHS: return rhs_takes_ranges(pl) ? "splitting_rhs_kernel3" : "splitting_rhs_kernel2";
+        case K_FFTX: return pl->nx == 8 ? "fft_x8_r2c_kernel" : (x_is_persistent(pl) ? "fft_x_r2c_tma_kernel" : "fft_x_r2c_kernel");
+        case K_IFFTX: return pl->nx == 8 ? "fft_x8_c2r_kernel" : (x_is_persistent(pl) ? "fft_x_c2r_tma_kernel" : "fft_x_c2r_kernel");
+        case K_FFTY: case K_IFFTY:
+            return pl->y16 ? "fft_y1024_kernel" : (pl->ny * pl->y_cols / 8 <= 512 ? "fft_tma1_kernel" : "fft_tma_kernel");
+        case K_Z:
+            if (wall) return pl->thomas_variant == 1 ? "thomas_tma_kernel" : "thomas_kernel";
+            return pl->nz * pl->z_cols / 8 <= 512 ? "fft_tma1_kernel" : "fft_tma_kernel";
+        case K_ZS: return "thomas_singular_kernel";
+        case K_CORR: return "correction_kernel";
+    }
+    return nullptr;
+}
+
 extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int value) {
     if (!pl || !name) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan or option name");
-    if (!strcmp(name, "y_cols") && (value == 4 || (value == 8 && pl->ny < 2048))) { pl->y_cols = value; return plan_make_maps(pl); }
-    if (!strcmp(name, "z_cols") && (value == 4 || (value == 8 && pl->nz < 2048))) { pl->z_cols = value; return plan_make_maps(pl); }
-    if (!strcmp(name, "tma") && value >= 0 && value <= 2) { pl->use_tma = value; return FLUTAS_OK; }
-    if (!strcmp(name, "thomas") && pl->bc_z == FLUTAS_BC_Z_WALL && (value == 0 || (value == 1 && pl->ttab))) {
-        if (value == 0 && !pl->cp) {   // the two-sweep kernel keeps c' in a half-spectrum of its own
+    if (!strcmp(name, "thomas") && pl->bc_z == FLUTAS_BC_Z_WALL && (value == 0 || (value == 1 && ThomasGeom::smem_bytes(pl->nz) <= 227 * 1024))) {
+        if (value == 0 && !pl->cp) {   // the two-sweep kernel keeps c' in half a spectrum of its own
             CUDA_TRY(cudaMalloc((void **)&pl->cp, sizeof(double) * (size_t)pl->nspec));
-            pl->bytes += sizeof(double) * (size_t)pl->nspec;
+            pl->cp_owned = true;
         }
         pl->thomas_variant = value;
-        return FLUTAS_OK;
+        return pl->ws_base ? plan_make_maps(pl) : FLUTAS_OK;
     }
     if (!strcmp(name, "y16") && (value == 0 || (value == 1 && pl->ny == Y16Geom::N))) {
         CUDA_TRY(cudaDeviceSynchronize());
         pl->y16 = value;                        // the storage order along y changes with the kernel
         if (int rc = upload_lam_y(pl)) return rc;
         if (pl->ttab) if (int rc = build_thomas_table(pl)) return rc;
-        return plan_make_maps(pl);
+        return pl->ws_base ? plan_make_maps(pl) : FLUTAS_OK;
     }
     if (!strcmp(name, "thomas_warps") && (value == 1 || value == 2)) { pl->thomas_warps = value; return FLUTAS_OK; }
     if (!strcmp(name, "chunk") && value >= 0) { pl->chunk = value; return FLUTAS_OK; }
     if (!strcmp(name, "overlap") && (value == 0 || value == 1)) { pl->overlap = value; return FLUTAS_OK; }
-    if (!strcmp(name, "rhs_kc") && value >= 1) { pl->rhs_kc = value; return FLUTAS_OK; }
-    if (!strcmp(name, "x_variant") && (value == 0 || value == 1)) { pl->x_variant = value; return FLUTAS_OK; }
-    if (!strcmp(name, "rhs_variant") && value >= 1 && value <= 3) { pl->rhs_variant = value; return FLUTAS_OK; }
-    if (!strcmp(name, "rhs_bx") && (value == 8 || value == 16 || value == 32 || value == 64 || value == 128)) { pl->rhs_bx = value; return FLUTAS_OK; }
     return fail(FLUTAS_ERR_INVALID_ARG, "unknown option or value: %s = %d", name, value);
 }
 
@@ -417,48 +529,16 @@ template <typename K> static cudaError_t set_smem(K kernel, size_t bytes) {
 
 constexpr int clamp_nt(int n) { return n < 32 ? 32 : (n > 256 ? 256 : n); }
 
-template <int N, int C, int MODE> static cudaError_t launch_strided_nc(const StridedArgs &a, int n_outer, cudaStream_t st) {
-    constexpr int NT = clamp_nt(N * C / 8);
-    const size_t smem = sizeof(double2) * (size_t)N * C;
-    auto kern = fft_strided_kernel<N, C, MODE, NT>;
-    cudaError_t e = set_smem(kern, smem);
-    if (e != cudaSuccess) return e;
-    kern<<<(unsigned)(a.n_tiles_x * n_outer), NT, smem, st>>>(a);
-    return cudaGetLastError();
-}
-
-template <int N, int MODE> static cudaError_t launch_strided_n(int cols, StridedArgs a, int nxh, int n_outer, cudaStream_t st) {
-    a.n_tiles_x = (nxh + cols - 1) / cols;
-    if (cols == 4) return launch_strided_nc<N, 4, MODE>(a, n_outer, st);
-    if constexpr (N >= 2048) return cudaErrorInvalidValue;   // 8 columns of 2048 do not fit in shared memory
-    else return launch_strided_nc<N, 8, MODE>(a, n_outer, st);
-}
-
-template <int MODE> static cudaError_t launch_strided(int n, int cols, const StridedArgs &a, int nxh, int n_outer, cudaStream_t st) {
-    switch (n) {
-        case 8: return launch_strided_n<8, MODE>(cols, a, nxh, n_outer, st);
-        case 16: return launch_strided_n<16, MODE>(cols, a, nxh, n_outer, st);
-        case 32: return launch_strided_n<32, MODE>(cols, a, nxh, n_outer, st);
-        case 64: return launch_strided_n<64, MODE>(cols, a, nxh, n_outer, st);
-        case 128: return launch_strided_n<128, MODE>(cols, a, nxh, n_outer, st);
-        case 256: return launch_strided_n<256, MODE>(cols, a, nxh, n_outer, st);
-        case 512: return launch_strided_n<512, MODE>(cols, a, nxh, n_outer, st);
-        case 1024: return launch_strided_n<1024, MODE>(cols, a, nxh, n_outer, st);
-        case 2048: return launch_strided_n<2048, MODE>(4, a, nxh, n_outer, st);
-    }
-    return cudaErrorInvalidValue;
-}
-
 // ---- persistent TMA-fed strided passes
 constexpr int tma_nt(int n, int c) { return n * c / 8 < 32 ? 32 : (n * c / 8 > 512 ? 512 : n * c / 8); }
 constexpr int tma_nbuf(int n, int c) { return 2 * n * c * 16 + 4096 <= 227 * 1024 ? 2 : 1; }
 
 template <int N, int C, int MODE>
-static cudaError_t launch_tma_nc(const CUtensorMap &map, const TmaFftArgs &a, const Tma1Args &a1, int variant, int num_sms,
+static cudaError_t launch_tma_nc(const CUtensorMap &map, const TmaFftArgs &a, const Tma1Args &a1, int num_sms,
                                  cudaStream_t st) {
     const long long ntiles = (long long)a.n_tiles_x * a.n_outer;
     if constexpr (N * C / 8 <= 512) {
-        if (variant == 1) {
+        {
             // one butterfly per thread: register-cached twiddles, direct stores, TMA prefetch only
             constexpr int NT = N * C / 8 < 32 ? 32 : N * C / 8;
             constexpr int P = Fact<N>::P, NCACHE = P - 1 < 2 ? P - 1 : 2;
@@ -476,6 +556,7 @@ static cudaError_t launch_tma_nc(const CUtensorMap &map, const TmaFftArgs &a, co
             return cudaGetLastError();
         }
     }
+    // lines of 2048 (1024 butterflies per tile): the generic kernel, several butterflies per thread
     constexpr int NT = tma_nt(N, C), NBUF = tma_nbuf(N, C);
     const size_t smem = (size_t)NBUF * N * C * 16 + 128;
     auto kern = fft_tma_kernel<N, C, MODE, NT, NBUF>;
@@ -491,16 +572,16 @@ static cudaError_t launch_tma_nc(const CUtensorMap &map, const TmaFftArgs &a, co
     return cudaGetLastError();
 }
 template <int N, int MODE>
-static cudaError_t launch_tma_n(int cols, const CUtensorMap &map, TmaFftArgs a, Tma1Args a1, int variant, cudaStream_t st,
+static cudaError_t launch_tma_n(int cols, const CUtensorMap &map, TmaFftArgs a, Tma1Args a1, cudaStream_t st,
                                 int num_sms) {
     a.n_tiles_x = a1.n_tiles_x = (a.nxh + cols - 1) / cols;
-    if (cols == 4) return launch_tma_nc<N, 4, MODE>(map, a, a1, variant, num_sms, st);
+    if (cols == 4) return launch_tma_nc<N, 4, MODE>(map, a, a1, num_sms, st);
     if constexpr (N >= 2048) return cudaErrorInvalidValue;
-    else return launch_tma_nc<N, 8, MODE>(map, a, a1, variant, num_sms, st);
+    else return launch_tma_nc<N, 8, MODE>(map, a, a1, num_sms, st);
 }
 template <int MODE>
 static cudaError_t launch_tma(int n, int cols, const CUtensorMap &map, TmaFftArgs a, long long row_stride,
-                              long long outer_stride, double2 *data, int variant, cudaStream_t st, int num_sms,
+                              long long outer_stride, double2 *data, cudaStream_t st, int num_sms,
                               int outer0, int n_outer) {
     a.outer0 = outer0; a.n_outer = n_outer;
     Tma1Args a1{};
@@ -509,15 +590,15 @@ static cudaError_t launch_tma(int n, int cols, const CUtensorMap &map, TmaFftArg
     a1.n_outer = a.n_outer; a1.line_dim = a.line_dim; a1.nxh = a.nxh; a1.tw = a.tw;
     a1.lam_x = a.lam_x; a1.lam_outer = a.lam_outer; a1.lam_pos = a.lam_pos;
     switch (n) {
-        case 8: return launch_tma_n<8, MODE>(cols, map, a, a1, variant, st, num_sms);
-        case 16: return launch_tma_n<16, MODE>(cols, map, a, a1, variant, st, num_sms);
-        case 32: return launch_tma_n<32, MODE>(cols, map, a, a1, variant, st, num_sms);
-        case 64: return launch_tma_n<64, MODE>(cols, map, a, a1, variant, st, num_sms);
-        case 128: return launch_tma_n<128, MODE>(cols, map, a, a1, variant, st, num_sms);
-        case 256: return launch_tma_n<256, MODE>(cols, map, a, a1, variant, st, num_sms);
-        case 512: return launch_tma_n<512, MODE>(cols, map, a, a1, variant, st, num_sms);
-        case 1024: return launch_tma_n<1024, MODE>(cols, map, a, a1, variant, st, num_sms);
-        case 2048: return launch_tma_n<2048, MODE>(4, map, a, a1, variant, st, num_sms);
+        case 8: return launch_tma_n<8, MODE>(cols, map, a, a1, st, num_sms);
+        case 16: return launch_tma_n<16, MODE>(cols, map, a, a1, st, num_sms);
+        case 32: return launch_tma_n<32, MODE>(cols, map, a, a1, st, num_sms);
+        case 64: return launch_tma_n<64, MODE>(cols, map, a, a1, st, num_sms);
+        case 128: return launch_tma_n<128, MODE>(cols, map, a, a1, st, num_sms);
+        case 256: return launch_tma_n<256, MODE>(cols, map, a, a1, st, num_sms);
+        case 512: return launch_tma_n<512, MODE>(cols, map, a, a1, st, num_sms);
+        case 1024: return launch_tma_n<1024, MODE>(cols, map, a, a1, st, num_sms);
+        case 2048: return launch_tma_n<2048, MODE>(4, map, a, a1, st, num_sms);
     }
     return cudaErrorInvalidValue;
 }
@@ -574,7 +655,12 @@ template <int N2> static cudaError_t launch_c2r_tma_n(const flutas_plan *pl, dou
 // planes k0 .. k1 - 1 (a tile is 8 consecutive x-lines; ny is a multiple of 8)
 static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStream_t st, int k0, int k1) {
     const long long tile0 = (long long)k0 * pl->ny / 8, ntiles = (long long)(k1 - k0) * pl->ny / 8;
-    if (pl->x_variant == 1)
+    if (pl->nx == 8) {   // the degenerate length: one thread per line
+        const long long nlines = ntiles * 8;
+        fft_x8_r2c_kernel<<<(unsigned)((nlines + 127) / 128), 128, 0, st>>>(rhs + tile0 * 64, pl->spec, nlines, SpecRows{pl->ny, pl->plane, tile0 * 8});
+        return cudaGetLastError();
+    }
+    if (x_is_persistent(pl))
         switch (pl->n2) {
 #define X(n) case n: return launch_r2c_tma_n<n>(pl, rhs, st, tile0, ntiles);
             FOR_EACH_N2_TMA(X)
@@ -589,7 +675,12 @@ static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStre
 }
 static cudaError_t launch_c2r(const flutas_plan *pl, double *out, double scale, cudaStream_t st, int k0, int k1) {
     const long long tile0 = (long long)k0 * pl->ny / 8, ntiles = (long long)(k1 - k0) * pl->ny / 8;
-    if (pl->x_variant == 1)
+    if (pl->nx == 8) {
+        const long long nlines = ntiles * 8;
+        fft_x8_c2r_kernel<<<(unsigned)((nlines + 127) / 128), 128, 0, st>>>(pl->spec, out + tile0 * 64, scale, nlines, SpecRows{pl->ny, pl->plane, tile0 * 8});
+        return cudaGetLastError();
+    }
+    if (x_is_persistent(pl))
         switch (pl->n2) {
 #define X(n) case n: return launch_c2r_tma_n<n>(pl, out, scale, st, tile0, ntiles);
             FOR_EACH_N2_TMA(X)
@@ -624,9 +715,9 @@ static int check_launch(cudaError_t e, const char *what) {
     return FLUTAS_OK;
 }
 
-// planes k0 .. k1 - 1 of rhs, u', v', w' (the bulk-copy-fed form takes any range; the older forms the whole grid)
+// planes k0 .. k1 - 1 of rhs, u', v', w' (the bulk-copy-fed form takes any range; the register form the whole grid)
 static bool rhs_takes_ranges(const flutas_plan *pl) {
-    return pl->rhs_variant == 3 && pl->nx % Rhs3Geom::X == 0 && pl->ny % Rhs3Geom::TY == 0;
+    return pl->nx % Rhs3Geom::X == 0 && pl->ny % Rhs3Geom::TY == 0;
 }
 static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
                        const double *p, const double *po, double dt, double dt_ratio, double *rhs, cudaStream_t st,
@@ -634,13 +725,8 @@ static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const 
     GridParams g = pl->grid;
     g.c_pn = 1.0 + dt_ratio;    // p_hat = (1 + r) p^n - r p^(n-1)
     g.c_po = dt_ratio;
-    // block = (bx threads x 2 points) x ty rows; nx/2 and ny are powers of two, so the grid divides evenly
-    const int bx = pl->nx / 2 < pl->rhs_bx ? pl->nx / 2 : pl->rhs_bx;
-    int ty = 256 / bx;
-    if (ty > pl->ny) ty = pl->ny;
     const int nk = k1 - k0;
     const int kc = pl->rhs_kc < nk ? pl->rhs_kc : nk;
-    dim3 block(bx, ty), grid(pl->nx / 2 / bx, pl->ny / ty, (nk + kc - 1) / kc);
     if (rhs_takes_ranges(pl)) {
         // bulk-copy-fed form: tile = 128 x 8 cells, three plane slabs in shared memory
         const dim3 b3(Rhs3Geom::NTX, Rhs3Geom::TY), g3(pl->nx / Rhs3Geom::X, pl->ny / Rhs3Geom::TY, (nk + kc - 1) / kc);
@@ -649,10 +735,14 @@ static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const 
         k3<<<g3, b3, Rhs3Geom::SMEM, st>>>(g, dt, kc, k0, k1, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
         return check_launch(cudaGetLastError(), "splitting_rhs");
     }
+    // small grids (nx < 128 or ny < 8 rows per tile): the register-marching form.
+    // block = (bx threads x 2 points) x ty rows; nx/2 and ny are powers of two, so the grid divides evenly
     if (k0 != 0 || k1 != pl->nz) return fail(FLUTAS_ERR_INVALID_ARG, "this form of the RHS kernel takes the whole grid");
-    if (pl->rhs_variant == 1)
-        splitting_rhs_kernel<<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
-    else if (pl->bc_z == FLUTAS_BC_Z_WALL)
+    const int bx = pl->nx / 2 < 64 ? pl->nx / 2 : 64;
+    int ty = 256 / bx;
+    if (ty > pl->ny) ty = pl->ny;
+    dim3 block(bx, ty), grid(pl->nx / 2 / bx, pl->ny / ty, (nk + kc - 1) / kc);
+    if (pl->bc_z == FLUTAS_BC_Z_WALL)
         splitting_rhs_kernel2<true><<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
     else
         splitting_rhs_kernel2<false><<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
@@ -663,7 +753,7 @@ static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const 
 template <int MODE> static int enqueue_y(flutas_plan *pl, cudaStream_t st, int k0, int k1) {
     const char *what = MODE == MODE_FWD ? "fft_y_fwd" : "fft_y_inv";
     const long long row_stride = pl->pitch, outer_stride = pl->plane;
-    if (pl->y16 && pl->use_tma) {
+    if (pl->y16) {
         Tma1Args a1{};
         a1.data = pl->spec; a1.row_stride = row_stride; a1.outer_stride = outer_stride;
         a1.n_tiles_x = (pl->nxh + Y16Geom::C - 1) / Y16Geom::C;
@@ -675,21 +765,12 @@ template <int MODE> static int enqueue_y(flutas_plan *pl, cudaStream_t st, int k
         kern<<<(unsigned)grid, Y16Geom::NT, Y16Geom::SMEM, st>>>(pl->map_y, a1);
         return check_launch(cudaGetLastError(), what);
     }
-    if (pl->use_tma) {
-        TmaFftArgs ty{};
-        ty.line_dim = 1;
-        ty.nxh = pl->nxh;
-        ty.tw = pl->tw_y;
-        return check_launch(launch_tma<MODE>(pl->ny, pl->y_cols, pl->map_y, ty, row_stride, outer_stride, pl->spec,
-                                             pl->use_tma, st, pl->num_sms, k0, k1 - k0), what);
-    }
-    StridedArgs ay{};
-    ay.data = pl->spec + (long long)k0 * outer_stride;
-    ay.row_stride = row_stride;
-    ay.outer_stride = outer_stride;
-    ay.nxh = pl->nxh;
-    ay.tw = pl->tw_y;
-    return check_launch(launch_strided<MODE>(pl->ny, pl->y_cols, ay, pl->nxh, k1 - k0, st), what);
+    TmaFftArgs ty{};
+    ty.line_dim = 1;
+    ty.nxh = pl->nxh;
+    ty.tw = pl->tw_y;
+    return check_launch(launch_tma<MODE>(pl->ny, pl->y_cols, pl->map_y, ty, row_stride, outer_stride, pl->spec,
+                                         st, pl->num_sms, k0, k1 - k0), what);
 }
 
 // the z stage on the whole half-spectrum (every line along z crosses all planes); timer marks between kernels
@@ -697,28 +778,15 @@ static int enqueue_z(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
     const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
     if (!wall) {
         const long long row_stride = pl->plane, outer_stride = pl->pitch;
-        if (pl->use_tma) {
-            TmaFftArgs tz{};
-            tz.line_dim = 2;
-            tz.nxh = pl->nxh;
-            tz.tw = pl->tw_z;
-            tz.lam_x = pl->lam_x;
-            tz.lam_outer = pl->lam_y;
-            tz.lam_pos = pl->lam_z;
-            if (int rc = check_launch(launch_tma<MODE_SOLVE>(pl->nz, pl->z_cols, pl->map_z, tz, row_stride, outer_stride, pl->spec,
-                                                             pl->use_tma, st, pl->num_sms, 0, pl->ny), "z_solve (tma)")) return rc;
-        } else {
-            StridedArgs az{};
-            az.data = pl->spec;
-            az.row_stride = row_stride;
-            az.outer_stride = outer_stride;
-            az.nxh = pl->nxh;
-            az.tw = pl->tw_z;
-            az.lam_x = pl->lam_x;
-            az.lam_outer = pl->lam_y;
-            az.lam_pos = pl->lam_z;
-            if (int rc = check_launch(launch_strided<MODE_SOLVE>(pl->nz, pl->z_cols, az, pl->nxh, pl->ny, st), "z_solve")) return rc;
-        }
+        TmaFftArgs tz{};
+        tz.line_dim = 2;
+        tz.nxh = pl->nxh;
+        tz.tw = pl->tw_z;
+        tz.lam_x = pl->lam_x;
+        tz.lam_outer = pl->lam_y;
+        tz.lam_pos = pl->lam_z;
+        if (int rc = check_launch(launch_tma<MODE_SOLVE>(pl->nz, pl->z_cols, pl->map_z, tz, row_stride, outer_stride, pl->spec,
+                                                         st, pl->num_sms, 0, pl->ny), "z_solve")) return rc;
         if (tm) tm->mark();
     } else {
         const long long ncol = (long long)pl->pitch * pl->ny;
@@ -743,7 +811,7 @@ static int enqueue_z(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
         if (int rc = check_launch(cudaGetLastError(), "z_solve (thomas)")) return rc;
         if (tm) tm->mark();
         const size_t smem = sizeof(double) * (4 * (size_t)pl->nz + 2);
-        if (smem > 200 * 1024) return fail(FLUTAS_ERR_UNSUPPORTED_SIZE, "nz too large for the singular-column kernel");
+        // nz <= 4096 (checked at plan creation): at most 128 KB
         if (set_smem(thomas_singular_kernel, smem) != cudaSuccess) return check_launch(cudaGetLastError(), "z_singular attr");
         thomas_singular_kernel<<<1, 256, smem, st>>>(pl->spec, pl->plane, pl->nz, pl->sing_coef);
         if (int rc = check_launch(cudaGetLastError(), "z_singular")) return rc;
@@ -818,6 +886,7 @@ extern "C" int flutas_projection_step_ex(flutas_plan *pl, double *u, double *v, 
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail(FLUTAS_ERR_INVALID_ARG, "dt must be positive and finite");
     if (!(dt_ratio > 0.0) || !std::isfinite(dt_ratio)) return fail(FLUTAS_ERR_INVALID_ARG, "dt_ratio must be positive and finite");
     if (int rc = check_step_fields(pl, u, v, w, phi, p, p_old, p_out)) return rc;
+    if (!pl->ws_base) return fail(FLUTAS_ERR_INVALID_ARG, "the plan has no workspace (flutas_plan_set_workspace)");
     cudaStream_t st = (cudaStream_t)stream;
     StepTimer tm(pl, st);
     const int nz = pl->nz;
@@ -894,6 +963,7 @@ extern "C" int flutas_splitting_rhs_ex(flutas_plan *pl, const double *u, const d
     if (!(dt_ratio > 0.0) || !std::isfinite(dt_ratio)) return fail(FLUTAS_ERR_INVALID_ARG, "dt_ratio must be positive and finite");
     const void *ptrs[7] = {u, v, w, phi, p, p_old, rhs_out};
     if (int rc = check_fields(pl, ptrs, 7)) return rc;
+    if (!pl->ws_base) return fail(FLUTAS_ERR_INVALID_ARG, "the plan has no workspace (flutas_plan_set_workspace)");
     return enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, dt_ratio, rhs_out, (cudaStream_t)stream, 0, pl->nz);
 }
 
@@ -907,6 +977,7 @@ extern "C" int flutas_poisson_solve(flutas_plan *pl, const double *rhs, double *
     const void *ptrs[2] = {rhs, p_out};
     if (rhs == p_out) { if (int rc = check_fields(pl, ptrs, 1)) return rc; }
     else if (int rc = check_fields(pl, ptrs, 2)) return rc;
+    if (!pl->ws_base) return fail(FLUTAS_ERR_INVALID_ARG, "the plan has no workspace (flutas_plan_set_workspace)");
     cudaStream_t st = (cudaStream_t)stream;
     if (int rc = check_launch(launch_r2c(pl, rhs, st, 0, pl->nz), "fft_x_r2c")) return rc;
     if (int rc = enqueue_y<MODE_FWD>(pl, st, 0, pl->nz)) return rc;

@@ -1,11 +1,11 @@
 // kernels.cuh -- the device kernels of the projection step (sm_100a, fp64).
 //
-//   splitting_rhs_kernel   a1-a3  density from colour, p_hat, splitting RHS; also stores the
+//   splitting_rhs_kernel2  a1-a3  density from colour, p_hat, splitting RHS; also stores the
 //                                 half-corrected velocity u' = u* - dt (1/rho_f - 1/rho0) grad p_hat
-//   fft_x_r2c_kernel       a4     real-to-complex transform along x (8 contiguous lines per CTA)
-//   fft_strided_kernel     a5/a7  complex transform along y (tile = C columns of kx x all j)
-//                          a6p    and, in SOLVE mode, forward-z / divide by eigenvalues / inverse-z
-//   thomas_kernel          a6w    tridiagonal solve along z per (kx,ky), one thread per column
+//                                 (register-marching form for small grids; kernels_rhs.cuh holds the production form)
+//   fft_x_r2c_kernel       a4     real-to-complex transform along x (8 contiguous lines per CTA; nx outside 128..1024)
+//   fft_x8_r2c/c2r_kernel  a4/a8  the degenerate length nx = 8
+//   thomas_kernel          a6w    tridiagonal solve along z per (kx,ky), one thread per column (two sweeps; nz > 512)
 //   thomas_singular_kernel a6w    the (0,0) column: pin the last unknown, remove the mean
 //   fft_x_c2r_kernel       a8     complex-to-real transform along x, normalisation, writes p^(n+1)
 //   correction_kernel      a9     u = u' - dt/rho0 grad p^(n+1)
@@ -34,17 +34,12 @@ struct GridParams {
     double inv_dx, inv_dy, inv_dz;
     double rho1, rho2, rho0;
     double c_pn, c_po;   // p_hat = c_pn p^n - c_po p^(n-1); (2, 1) for constant dt, (1 + r, r) in general
+    double flux_one;     // 1, or 0 when rho1 == rho2: the splitting coefficient 1 - rho0/rho_f is then exactly 0
 };
 
 // ------------------------------------------------------------------------------------------------
 // a1-a3: fused density + splitting right-hand side (eqs. 2, 16, 17).
 // Reads u*, v*, w*, phi, p, p_old once; writes rhs and the half-corrected velocity u', v', w'.
-//
-// 2.5-D register-marching stencil: a block is (bx threads along x, 2 points each) x (ty rows of j); each
-// thread marches over `kc` planes in z carrying, in registers, the centre and top values of rho_c and p_hat,
-// the bottom-face flux (= the previous plane's top-face flux) and w below.  x neighbours come from warp
-// shuffles (edge lanes load them), y neighbours from L1/L2 (the rows were loaded one iteration earlier by
-// the neighbouring threads).  Per point: 4 reciprocals, no integer division, 32-bit index arithmetic.
 // ------------------------------------------------------------------------------------------------
 // Reciprocal of a normal, positive double: hardware seed (MUFU.RCP64H, ~2^-23) + two Newton steps
 // (relative error <= ~1 ulp, branch-free, 5 instructions instead of the ~30 of an IEEE division).
@@ -57,124 +52,11 @@ __device__ __forceinline__ double rcp_density(double x) {
     return r;
 }
 
-struct Flux { double f, r; };   // f = (1 - rho0/rho_f) * g,  r = 1/rho_f
-__device__ __forceinline__ Flux face_flux(double rc_a, double rc_b, double g, double rho0) {
-    Flux o;
-    o.r = rcp_density(0.5 * (rc_a + rc_b));
-    o.f = (1.0 - rho0 * o.r) * g;
-    return o;
-}
-
-__global__ void __launch_bounds__(256, 2)
-splitting_rhs_kernel(GridParams g, double dt, int kc, const double *__restrict__ u, const double *__restrict__ v,
-                     const double *__restrict__ w, const double *__restrict__ phi,
-                     const double *__restrict__ p, const double *__restrict__ po,
-                     double *__restrict__ rhs, double *__restrict__ up, double *__restrict__ vp,
-                     double *__restrict__ wp) {
-    const int nx = g.nx, ny = g.ny, nz = g.nz;
-    const int i0 = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
-    const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    const int k0 = blockIdx.z * kc, k1 = min(k0 + kc, nz);
-    const int jn = (j + 1 == ny) ? 0 : j + 1, js = (j == 0) ? ny - 1 : j - 1;
-    const int iw = (i0 == 0) ? nx - 1 : i0 - 1, ie = (i0 + 2 == nx) ? 0 : i0 + 2;
-    // shuffle neighbourhood: a "row" of lanes is min(32, blockDim.x) wide
-    const int lane = (threadIdx.x + threadIdx.y * blockDim.x) & 31;
-    const int rw = blockDim.x < 32 ? blockDim.x : 32;
-    const bool edge_l = (lane % rw) == 0, edge_r = (lane % rw) == rw - 1;
-    const long long plane = (long long)nx * ny;
-    const long long col = (long long)j * nx + i0, col_n = (long long)jn * nx + i0, col_s = (long long)js * nx + i0;
-    const long long row_j = (long long)j * nx;
-    const double rho1 = g.rho1, rho2 = g.rho2, rho0 = g.rho0, inv_rho0 = 1.0 / g.rho0;
-    const double c_div = g.rho0 / dt;
-
-    auto ld2 = [](const double *f, long long q) { return *reinterpret_cast<const double2 *>(f + q); };
-    auto rho_of = [&](double f) { return rho1 * f + rho2 * (1.0 - f); };
-    auto rho2_of = [&](double2 f) { return make_double2(rho_of(f.x), rho_of(f.y)); };
-    const double c_pn = g.c_pn, c_po = g.c_po;
-    auto phat2 = [&](double2 a, double2 b) { return make_double2(fma(c_pn, a.x, -(c_po * b.x)), fma(c_pn, a.y, -(c_po * b.y))); };
-
-    // prologue: centre plane k0, bottom flux and w below
-    long long qk = (long long)k0 * plane;
-    double2 rc_c = rho2_of(ld2(phi, qk + col)), ph_c = phat2(ld2(p, qk + col), ld2(po, qk + col));
-    double2 fb = make_double2(0.0, 0.0), wb = make_double2(0.0, 0.0);
-    if (!(g.wall && k0 == 0)) {
-        const long long qb = (long long)((k0 == 0) ? nz - 1 : k0 - 1) * plane + col;
-        const double2 rc_b = rho2_of(ld2(phi, qb)), ph_b = phat2(ld2(p, qb), ld2(po, qb));
-        fb.x = face_flux(rc_b.x, rc_c.x, (ph_c.x - ph_b.x) * g.inv_dz, rho0).f;
-        fb.y = face_flux(rc_b.y, rc_c.y, (ph_c.y - ph_b.y) * g.inv_dz, rho0).f;
-        wb = ld2(w, qb);
-    }
-
-    for (int k = k0; k < k1; ++k, qk += plane) {
-        const bool top = g.wall && (k + 1 == nz);
-        // next plane (becomes the centre of the next iteration)
-        double2 rc_t = rc_c, ph_t = ph_c;
-        if (!top) {
-            const long long qt = (long long)((k + 1 == nz) ? 0 : k + 1) * plane + col;
-            rc_t = rho2_of(ld2(phi, qt));
-            ph_t = phat2(ld2(p, qt), ld2(po, qt));
-        }
-        // y neighbours of the centre plane
-        const double2 rc_n = rho2_of(ld2(phi, qk + col_n)), ph_n = phat2(ld2(p, qk + col_n), ld2(po, qk + col_n));
-        const double2 rc_s = rho2_of(ld2(phi, qk + col_s)), ph_s = phat2(ld2(p, qk + col_s), ld2(po, qk + col_s));
-        const double2 uc = ld2(u, qk + col), vc = ld2(v, qk + col), wc = ld2(w, qk + col), vs = ld2(v, qk + col_s);
-
-        // x faces: m between (i0, i0+1), e between (i0+1, i0+2), wf between (i0-1, i0)
-        double rc_e = __shfl_down_sync(0xffffffffu, rc_c.x, 1), ph_e = __shfl_down_sync(0xffffffffu, ph_c.x, 1);
-        if (edge_r) {
-            const long long qe = qk + row_j + ie;
-            rc_e = rho_of(phi[qe]);
-            ph_e = fma(c_pn, p[qe], -(c_po * po[qe]));
-        }
-        const Flux fm = face_flux(rc_c.x, rc_c.y, (ph_c.y - ph_c.x) * g.inv_dx, rho0);
-        const Flux fe = face_flux(rc_c.y, rc_e, (ph_e - ph_c.y) * g.inv_dx, rho0);
-        double f_w = __shfl_up_sync(0xffffffffu, fe.f, 1), u_w = __shfl_up_sync(0xffffffffu, uc.y, 1);
-        if (edge_l) {
-            const long long qw = qk + row_j + iw;
-            f_w = face_flux(rho_of(phi[qw]), rc_c.x, (ph_c.x - fma(c_pn, p[qw], -(c_po * po[qw]))) * g.inv_dx, rho0).f;
-            u_w = u[qw];
-        }
-        // y faces
-        const Flux fn0 = face_flux(rc_c.x, rc_n.x, (ph_n.x - ph_c.x) * g.inv_dy, rho0);
-        const Flux fn1 = face_flux(rc_c.y, rc_n.y, (ph_n.y - ph_c.y) * g.inv_dy, rho0);
-        const double fs0 = face_flux(rc_s.x, rc_c.x, (ph_c.x - ph_s.x) * g.inv_dy, rho0).f;
-        const double fs1 = face_flux(rc_s.y, rc_c.y, (ph_c.y - ph_s.y) * g.inv_dy, rho0).f;
-        // z faces (wall faces carry zero flux)
-        Flux ft0{0.0, 0.0}, ft1{0.0, 0.0};
-        double gz0 = 0.0, gz1 = 0.0;
-        if (!top) {
-            gz0 = (ph_t.x - ph_c.x) * g.inv_dz;
-            gz1 = (ph_t.y - ph_c.y) * g.inv_dz;
-            ft0 = face_flux(rc_c.x, rc_t.x, gz0, rho0);
-            ft1 = face_flux(rc_c.y, rc_t.y, gz1, rho0);
-        }
-
-        double2 out;
-        out.x = c_div * ((uc.x - u_w) * g.inv_dx + (vc.x - vs.x) * g.inv_dy + (wc.x - wb.x) * g.inv_dz) +
-                ((fm.f - f_w) * g.inv_dx + (fn0.f - fs0) * g.inv_dy + (ft0.f - fb.x) * g.inv_dz);
-        out.y = c_div * ((uc.y - uc.x) * g.inv_dx + (vc.y - vs.y) * g.inv_dy + (wc.y - wb.y) * g.inv_dz) +
-                ((fe.f - fm.f) * g.inv_dx + (fn1.f - fs1) * g.inv_dy + (ft1.f - fb.y) * g.inv_dz);
-        *reinterpret_cast<double2 *>(rhs + qk + col) = out;
-
-        out.x = uc.x - dt * ((fm.r - inv_rho0) * ((ph_c.y - ph_c.x) * g.inv_dx));
-        out.y = uc.y - dt * ((fe.r - inv_rho0) * ((ph_e - ph_c.y) * g.inv_dx));
-        *reinterpret_cast<double2 *>(up + qk + col) = out;
-        out.x = vc.x - dt * ((fn0.r - inv_rho0) * ((ph_n.x - ph_c.x) * g.inv_dy));
-        out.y = vc.y - dt * ((fn1.r - inv_rho0) * ((ph_n.y - ph_c.y) * g.inv_dy));
-        *reinterpret_cast<double2 *>(vp + qk + col) = out;
-        out.x = top ? wc.x : wc.x - dt * ((ft0.r - inv_rho0) * gz0);
-        out.y = top ? wc.y : wc.y - dt * ((ft1.r - inv_rho0) * gz1);
-        *reinterpret_cast<double2 *>(wp + qk + col) = out;
-
-        fb = make_double2(ft0.f, ft1.f);
-        wb = wc;
-        rc_c = rc_t;
-        ph_c = ph_t;
-    }
-}
-
 // ------------------------------------------------------------------------------------------------
-// Second form of the same kernel: identical decomposition (thread = 2 x-points, marching in z), but
+// Register-marching form (small grids: nx < 128 or ny < 8).  2.5-D stencil: a block is (bx threads along x, 2 points
+// each) x (ty rows of j); each thread marches over `kc` planes in z carrying, in registers, the centre and top values of
+// rho_c and p_hat, the bottom-face flux and w below.  x neighbours come from warp shuffles (edge lanes load them),
+// y neighbours from L1/L2.
 //  * software-pipelined: the operands that miss in cache (phi, p, p_old of plane k+2 and u*, v*, w* of plane
 //    k+1) are requested one iteration before they are used, so a warp waits on DRAM once per kernel instead
 //    of once per plane; the row / edge neighbours of the current plane (L1 / L2 hits) are requested at the top
@@ -189,9 +71,10 @@ __device__ __forceinline__ double2 ldg2(const double *f, long long q) {
 __device__ __forceinline__ void stcs2(double *f, long long q, double2 v) {
     __stcs(reinterpret_cast<double2 *>(f + q), v);
 }
-// (1 - rho0/rho_f) for the face between cells of density ra and rb
-__device__ __forceinline__ double flux_coef(double ra, double rb, double m2rho0) {
-    return fma(m2rho0, rcp_density(ra + rb), 1.0);
+// (1 - rho0/rho_f) for the face between cells of density ra and rb: one = 1, m2rho0 = -2 rho0
+// (one = m2rho0 = 0 when rho1 == rho2: exactly 0, the constant-density projection)
+__device__ __forceinline__ double flux_coef(double ra, double rb, double m2rho0, double one) {
+    return fma(m2rho0, rcp_density(ra + rb), one);
 }
 
 template <bool WALL>
@@ -213,7 +96,7 @@ splitting_rhs_kernel2(GridParams g, double dt, int kc, const double *__restrict_
     const long long plane = (long long)nx * ny;
     const long long col = (long long)j * nx + i0, col_n = (long long)jn * nx + i0, col_s = (long long)js * nx + i0;
     const long long q_e = (long long)j * nx + ie, q_w = (long long)j * nx + iw;
-    const double drho = g.rho1 - g.rho2, rho2 = g.rho2, m2rho0 = -2.0 * g.rho0;
+    const double drho = g.rho1 - g.rho2, rho2 = g.rho2, one = g.flux_one, m2rho0 = -2.0 * g.rho0 * g.flux_one;
     const double c_div = g.rho0 / dt, c_up = dt / g.rho0;
     const double idx = g.inv_dx, idy = g.inv_dy, idz = g.inv_dz;
 
@@ -230,8 +113,8 @@ splitting_rhs_kernel2(GridParams g, double dt, int kc, const double *__restrict_
     if (!(WALL && k0 == 0)) {
         const long long qb = (long long)((k0 == 0) ? nz - 1 : k0 - 1) * plane + col;
         const double2 rc_b = rho2_of(ldg2(phi, qb)), ph_b = phat2(ldg2(p, qb), ldg2(po, qb));
-        fb.x = flux_coef(rc_b.x, rc_c.x, m2rho0) * ((ph_c.x - ph_b.x) * idz);
-        fb.y = flux_coef(rc_b.y, rc_c.y, m2rho0) * ((ph_c.y - ph_b.y) * idz);
+        fb.x = flux_coef(rc_b.x, rc_c.x, m2rho0, one) * ((ph_c.x - ph_b.x) * idz);
+        fb.y = flux_coef(rc_b.y, rc_c.y, m2rho0, one) * ((ph_c.y - ph_b.y) * idz);
         wb = ldg2(w, qb);
     }
     // pipeline registers: plane k+1 (phi, p, p_old at the centre column) and plane k (u*, v*, w*, v* south)
@@ -261,26 +144,26 @@ splitting_rhs_kernel2(GridParams g, double dt, int kc, const double *__restrict_
         if (!top) {
             rc_t = rho2_of(a_phi);
             ph_t = phat2(a_p, a_po);
-            ft.x = flux_coef(rc_c.x, rc_t.x, m2rho0) * ((ph_t.x - ph_c.x) * idz);
-            ft.y = flux_coef(rc_c.y, rc_t.y, m2rho0) * ((ph_t.y - ph_c.y) * idz);
+            ft.x = flux_coef(rc_c.x, rc_t.x, m2rho0, one) * ((ph_t.x - ph_c.x) * idz);
+            ft.y = flux_coef(rc_c.y, rc_t.y, m2rho0, one) * ((ph_t.y - ph_c.y) * idz);
         }
         // ---- x faces: m between (i0, i0+1), e between (i0+1, i0+2), west face from the left lane
         double rc_e = __shfl_down_sync(0xffffffffu, rc_c.x, 1), ph_e = __shfl_down_sync(0xffffffffu, ph_c.x, 1);
         if (edge_r) { rc_e = rho_of(e_phi); ph_e = phat(e_p, e_po); }
-        const double fm = flux_coef(rc_c.x, rc_c.y, m2rho0) * ((ph_c.y - ph_c.x) * idx);
-        const double fe = flux_coef(rc_c.y, rc_e, m2rho0) * ((ph_e - ph_c.y) * idx);
+        const double fm = flux_coef(rc_c.x, rc_c.y, m2rho0, one) * ((ph_c.y - ph_c.x) * idx);
+        const double fe = flux_coef(rc_c.y, rc_e, m2rho0, one) * ((ph_e - ph_c.y) * idx);
         double f_w = __shfl_up_sync(0xffffffffu, fe, 1), u_w = __shfl_up_sync(0xffffffffu, uc.y, 1);
         if (edge_l) {
-            f_w = flux_coef(rho_of(w_phi), rc_c.x, m2rho0) * ((ph_c.x - phat(w_p, w_po)) * idx);
+            f_w = flux_coef(rho_of(w_phi), rc_c.x, m2rho0, one) * ((ph_c.x - phat(w_p, w_po)) * idx);
             u_w = w_u;
         }
         // ---- y faces
         const double2 rc_n = rho2_of(r_nphi), ph_n = phat2(r_np, r_npo);
         const double2 rc_s = rho2_of(r_sphi), ph_s = phat2(r_sp, r_spo);
-        const double fn0 = flux_coef(rc_c.x, rc_n.x, m2rho0) * ((ph_n.x - ph_c.x) * idy);
-        const double fn1 = flux_coef(rc_c.y, rc_n.y, m2rho0) * ((ph_n.y - ph_c.y) * idy);
-        const double fs0 = flux_coef(rc_s.x, rc_c.x, m2rho0) * ((ph_c.x - ph_s.x) * idy);
-        const double fs1 = flux_coef(rc_s.y, rc_c.y, m2rho0) * ((ph_c.y - ph_s.y) * idy);
+        const double fn0 = flux_coef(rc_c.x, rc_n.x, m2rho0, one) * ((ph_n.x - ph_c.x) * idy);
+        const double fn1 = flux_coef(rc_c.y, rc_n.y, m2rho0, one) * ((ph_n.y - ph_c.y) * idy);
+        const double fs0 = flux_coef(rc_s.x, rc_c.x, m2rho0, one) * ((ph_c.x - ph_s.x) * idy);
+        const double fs1 = flux_coef(rc_s.y, rc_c.y, m2rho0, one) * ((ph_c.y - ph_s.y) * idy);
 
         double2 out;
         out.x = c_div * ((uc.x - u_w) * idx + (vc.x - vs.x) * idy + (wc.x - wb.x) * idz) +
@@ -351,120 +234,8 @@ __device__ __forceinline__ void tile_fft(double2 *s, const double2 *__restrict__
     }
 }
 
-// ------------------------------------------------------------------------------------------------
-// a5 / a7 / a6p: transform along a strided direction.  A tile is C consecutive kx columns x the whole
-// line (N positions, `row_stride` elements apart); blockIdx.x = tx + n_tiles_x * outer.
-// ------------------------------------------------------------------------------------------------
+// modes of the strided transform kernels (kernels_tma.cuh, kernels_y16.cuh)
 enum { MODE_FWD = 0, MODE_INV = 1, MODE_SOLVE = 2 };
-
-struct StridedArgs {
-    double2 *data;
-    long long row_stride;    // elements between line positions r and r+1
-    long long outer_stride;  // elements between outer indices (k for the y pass, j for the z pass)
-    int n_tiles_x;           // tiles along kx
-    int nxh;                 // valid kx columns (nx/2 + 1)
-    const double2 *tw;       // e^{-2 pi i m / N}
-    // SOLVE only: eigenvalues in storage (permuted) order
-    const double *lam_x, *lam_outer, *lam_pos;
-};
-
-// The first pass reads its 8 elements straight from global memory into registers and the last pass
-// writes them straight back (the permuted order makes every pass in place), so shared memory is only
-// the exchange buffer between passes: P-1 exchanges, P-1 barriers, no staging copies.
-template <int N, int C, int MODE, int NT>
-__global__ void __launch_bounds__(NT, (N * C * 16 <= 72 * 1024 && NT == 256) ? 3 : 1) fft_strided_kernel(StridedArgs a) {
-    extern __shared__ double2 smem[];
-    double2 *s = smem;
-    constexpr int P = Fact<N>::P;
-    const int tid = threadIdx.x;
-    const int tx = blockIdx.x % a.n_tiles_x, outer = blockIdx.x / a.n_tiles_x;
-    const int l = tid % C;
-    const int kx = tx * C + l;
-    const bool valid = kx < a.nxh;
-    double2 *gp = a.data + (long long)outer * a.outer_stride + kx;
-    const long long rs = a.row_stride;
-
-    auto load8 = [&](bool from_global, const int *pos, double2 *v) {
-        if (from_global) {
-#pragma unroll
-            for (int e = 0; e < 8; ++e) v[e] = valid ? gp[(long long)pos[e] * rs] : make_double2(0.0, 0.0);
-        } else {
-#pragma unroll
-            for (int e = 0; e < 8; ++e) v[e] = s[pos[e] * C + l];
-        }
-    };
-    auto store8 = [&](bool to_global, const int *pos, const double2 *v) {
-        if (to_global) {
-            if (valid) {
-#pragma unroll
-                for (int e = 0; e < 8; ++e) gp[(long long)pos[e] * rs] = v[e];
-            }
-        } else {
-#pragma unroll
-            for (int e = 0; e < 8; ++e) s[pos[e] * C + l] = v[e];
-        }
-    };
-
-    if (MODE == MODE_FWD || MODE == MODE_INV) {
-#pragma unroll
-        for (int pp = 0; pp < P; ++pp) {
-            const int p = (MODE == MODE_FWD) ? pp + 1 : P - pp;
-            for (int t = tid / C; t < N / 8; t += NT / C) {
-                int pos[8], n2;
-                double2 v[8];
-                pass_positions<N>(p, t, pos, n2);
-                load8(pp == 0, pos, v);
-                if (MODE == MODE_FWD) fwd_pass_regs<N>(p, n2, v, a.tw, 1);
-                else inv_pass_regs<N>(p, n2, v, a.tw, 1);
-                store8(pp == P - 1, pos, v);
-            }
-            if (pp + 1 < P) __syncthreads();
-        }
-    } else {
-        // forward passes 1..P-1
-#pragma unroll
-        for (int p = 1; p < P; ++p) {
-            for (int t = tid / C; t < N / 8; t += NT / C) {
-                int pos[8], n2;
-                double2 v[8];
-                pass_positions<N>(p, t, pos, n2);
-                load8(p == 1, pos, v);
-                fwd_pass_regs<N>(p, n2, v, a.tw, 1);
-                store8(false, pos, v);
-            }
-            __syncthreads();
-        }
-        // last forward pass, division by the eigenvalue sum, first inverse pass: all in registers
-        const double lam_xy = a.lam_x[valid ? kx : 0] + a.lam_outer[outer];
-        for (int t = tid / C; t < N / 8; t += NT / C) {
-            int pos[8], n2;
-            double2 v[8];
-            pass_positions<N>(P, t, pos, n2);
-            load8(P == 1, pos, v);
-            fwd_pass_regs<N>(P, n2, v, a.tw, 1);
-#pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                const double den = lam_xy + a.lam_pos[pos[e]];
-                const double inv = (den == 0.0) ? 0.0 : 1.0 / den;     // the (0,0,0) mode is dropped (zero-mean gauge)
-                v[e] = cscale(v[e], inv);
-            }
-            inv_pass_regs<N>(P, n2, v, a.tw, 1);
-            store8(P == 1, pos, v);
-        }
-#pragma unroll
-        for (int p = P - 1; p >= 1; --p) {
-            __syncthreads();
-            for (int t = tid / C; t < N / 8; t += NT / C) {
-                int pos[8], n2;
-                double2 v[8];
-                pass_positions<N>(p, t, pos, n2);
-                load8(false, pos, v);
-                inv_pass_regs<N>(p, n2, v, a.tw, 1);
-                store8(p == 1, pos, v);
-            }
-        }
-    }
-}
 
 // ------------------------------------------------------------------------------------------------
 // Cooperative copy of TOT contiguous elements with B loads in flight per thread: all loads of a batch are
@@ -544,6 +315,43 @@ fft_x_c2r_kernel(const double2 *__restrict__ spec, double *__restrict__ out,
     double2 *dst = reinterpret_cast<double2 *>(out) + line0 * N2;
     for (int idx = tid; idx < 8 * N2; idx += NT)
         dst[idx] = cscale(s[tile_index<8, true>(idx % N2, idx / N2)], scale);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4 / a8 for the degenerate length nx = 8: one thread per line, the 8-point transform in registers (a complex radix-8
+// butterfly on real input: natural order in and out), rows written / read in natural kx order (kx = 0..4).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+fft_x8_r2c_kernel(const double *__restrict__ rhs, double2 *__restrict__ spec, long long nlines, SpecRows sr) {
+    const long long line = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (line >= nlines) return;
+    double2 v[8];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const double2 x = reinterpret_cast<const double2 *>(rhs + line * 8)[e];
+        v[2 * e] = make_double2(x.x, 0.0);
+        v[2 * e + 1] = make_double2(x.y, 0.0);
+    }
+    radix8<-1>(v);
+    double2 *dst = spec + spec_row_offset(sr, line, 4 + 8);
+#pragma unroll
+    for (int k = 0; k <= 4; ++k) dst[k] = (k == 0 || k == 4) ? make_double2(v[k].x, 0.0) : v[k];
+}
+
+__global__ void __launch_bounds__(128)
+fft_x8_c2r_kernel(const double2 *__restrict__ spec, double *__restrict__ out, double scale, long long nlines, SpecRows sr) {
+    const long long line = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (line >= nlines) return;
+    const double2 *src = spec + spec_row_offset(sr, line, 4 + 8);
+    double2 v[8];
+    v[0] = make_double2(src[0].x, 0.0);          // the imaginary parts of the DC and Nyquist columns do not enter
+    v[4] = make_double2(src[4].x, 0.0);
+#pragma unroll
+    for (int k = 1; k < 4; ++k) { v[k] = src[k]; v[8 - k] = cconj(src[k]); }
+    radix8<+1>(v);
+#pragma unroll
+    for (int e = 0; e < 4; ++e)
+        reinterpret_cast<double2 *>(out + line * 8)[e] = make_double2(v[2 * e].x * scale, v[2 * e + 1].x * scale);
 }
 
 // ------------------------------------------------------------------------------------------------

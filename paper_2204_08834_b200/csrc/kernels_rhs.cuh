@@ -1,7 +1,7 @@
 // kernels_rhs.cuh -- third form of the fused density + splitting right-hand side kernel (rows a1-a3 of the step;
 // eqs. 2, 16, 17: PAPER.md:76, 153-155, 161), fed by the bulk-copy engine.
 //
-// Same decomposition as splitting_rhs_kernel2 (block = 64 x-threads x 2 points x TY rows of j, marching in z; TY = 8: 57 KB per slab,
+// Same decomposition as splitting_rhs_kernel2 in kernels.cuh (block = 64 x-threads x 2 points x TY rows of j, marching in z; TY = 8: 57 KB per slab,
 // one CTA of 512 threads per SM, 25 % less halo traffic from L2 than TY = 4 and 3 % faster), but
 // the operands no longer travel through registers: one warp asks the copy engine (cp.async.bulk -> mbarrier
 // complete_tx) for whole row segments of the plane two steps ahead, which land in a three-slot ring of plane
@@ -122,7 +122,7 @@ splitting_rhs_kernel3(GridParams g, double dt, int kc, int k_base, int k_end, co
     for (int m = 0; m < G::NSLOT; ++m)
         if (m <= m_last) issue_slab(k0 - 1 + m, m, mask_of(m));
 
-    const double drho = g.rho1 - g.rho2, rho2 = g.rho2, m2rho0 = -2.0 * g.rho0;
+    const double drho = g.rho1 - g.rho2, rho2 = g.rho2, one = g.flux_one, m2rho0 = -2.0 * g.rho0 * g.flux_one;
     const double c_div = g.rho0 / dt, c_up = dt / g.rho0;
     const double idx = g.inv_dx, idy = g.inv_dy, idz = g.inv_dz;
     const double c_pn = g.c_pn, c_po = g.c_po;
@@ -151,8 +151,8 @@ splitting_rhs_kernel3(GridParams g, double dt, int kc, int k_base, int k_end, co
         // z face between planes q-1 and q (wall faces carry zero flux)
         double2 fz = make_double2(0.0, 0.0);
         if (m >= 1 && !(WALL && (q == 0 || q == nz))) {
-            fz.x = flux_coef(rc_b.x, rc.x, m2rho0) * ((ph.x - ph_b.x) * idz);
-            fz.y = flux_coef(rc_b.y, rc.y, m2rho0) * ((ph.y - ph_b.y) * idz);
+            fz.x = flux_coef(rc_b.x, rc.x, m2rho0, one) * ((ph.x - ph_b.x) * idz);
+            fz.y = flux_coef(rc_b.y, rc.y, m2rho0, one) * ((ph.y - ph_b.y) * idz);
         }
         if (m >= 2) {   // plane q-1 is complete: its top-face flux is fz, its bottom-face flux fb
             const long long o = (long long)(q - 1) * plane + out0;
@@ -173,15 +173,15 @@ splitting_rhs_kernel3(GridParams g, double dt, int kc, int k_base, int k_end, co
             const double2 vc = ld2s(S + G::O_V + (ty + 1) * G::X + 2 * tx), vs = ld2s(S + G::O_V + ty * G::X + 2 * tx);
             const double2 wc = ld2s(S + G::O_W + ty * G::X + 2 * tx);
 
-            const double fm = flux_coef(rc.x, rc.y, m2rho0) * ((ph.y - ph.x) * idx);
-            const double fe = flux_coef(rc.y, rho_of(e_phi), m2rho0) * ((phat(e_p, e_po) - ph.y) * idx);
-            const double fw = flux_coef(rho_of(w_phi), rc.x, m2rho0) * ((ph.x - phat(w_p, w_po)) * idx);
+            const double fm = flux_coef(rc.x, rc.y, m2rho0, one) * ((ph.y - ph.x) * idx);
+            const double fe = flux_coef(rc.y, rho_of(e_phi), m2rho0, one) * ((phat(e_p, e_po) - ph.y) * idx);
+            const double fw = flux_coef(rho_of(w_phi), rc.x, m2rho0, one) * ((ph.x - phat(w_p, w_po)) * idx);
             const double2 rc_n = make_double2(rho_of(n_phi.x), rho_of(n_phi.y)), ph_n = make_double2(phat(n_p.x, n_po.x), phat(n_p.y, n_po.y));
             const double2 rc_s = make_double2(rho_of(s_phi.x), rho_of(s_phi.y)), ph_s = make_double2(phat(s_p.x, s_po.x), phat(s_p.y, s_po.y));
-            const double fn0 = flux_coef(rc.x, rc_n.x, m2rho0) * ((ph_n.x - ph.x) * idy);
-            const double fn1 = flux_coef(rc.y, rc_n.y, m2rho0) * ((ph_n.y - ph.y) * idy);
-            const double fs0 = flux_coef(rc_s.x, rc.x, m2rho0) * ((ph.x - ph_s.x) * idy);
-            const double fs1 = flux_coef(rc_s.y, rc.y, m2rho0) * ((ph.y - ph_s.y) * idy);
+            const double fn0 = flux_coef(rc.x, rc_n.x, m2rho0, one) * ((ph_n.x - ph.x) * idy);
+            const double fn1 = flux_coef(rc.y, rc_n.y, m2rho0, one) * ((ph_n.y - ph.y) * idy);
+            const double fs0 = flux_coef(rc_s.x, rc.x, m2rho0, one) * ((ph.x - ph_s.x) * idy);
+            const double fs1 = flux_coef(rc_s.y, rc.y, m2rho0, one) * ((ph.y - ph_s.y) * idy);
 
             part.x = c_div * ((uc.x - u_w) * idx + (vc.x - vs.x) * idy + (wc.x - wb.x) * idz) +
                      ((fm - fw) * idx + (fn0 - fs0) * idy);

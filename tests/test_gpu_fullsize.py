@@ -1,37 +1,26 @@
 """-m gpu: parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (default plan).
 
-The oracle's solve (naive DFT) cannot run at 512^3 / 1024x1024x512 in minutes, so at full size:
-  * the splitting right-hand side is compared ELEMENT BY ELEMENT with oracle.rhs (a plain O(N) stencil);
-  * the velocity correction is compared ELEMENT BY ELEMENT with oracle.correction applied to the GPU pressure;
-  * the pressure is checked through what is unique about it:
-      - SAMPLED spectral outputs computed one by one from the definition: for sampled wavenumbers the
-        Fourier coefficient of rhs (a plain sum over all points) divided by the eigenvalue (periodic), or fed
-        through an independent banded solve along z (walls), must equal the same coefficient of the GPU p;
-      - residual  ||L p - (rhs - mean rhs)|| / ||rhs||  with oracle.laplacian, zero mean, and
-        ||div u_new|| / ||div u*|| with oracle.divergence.
+Every stored entry of u, v, w and p after one flutas_projection_step is compared with oracle.projection_step (the plain
+definition: literal stencils, naive O(n^2) DFT per line, textbook Thomas) on the same seeded inputs, relative
+L2 <= 1e-10 per field -- north_star's bar, SURVEY.md sec. 8(c) "Parity metric".  The oracle needs about 40 s
+(512^3) and 4 minutes (1024 x 1024 x 512, ~45 GB of host memory) on the GPU box's 16 host cores.
+Beside the element-wise comparison, what is unique about the result is checked through independent operators:
+the right-hand side element by element (oracle.rhs, <= 1e-13), the residual || L p - (rhs - mean rhs) || / || rhs ||,
+the zero-mean gauge, || div u_new || / || div u* ||, and the wall face passing through.
+Run with -s to print the table row of BASELINE.md sec. 4.
 """
+import time
+
 import numpy as np
 import pytest
 import torch
 
-from paper_2204_08834_b200 import workloads as wl
+import workloads as wl
 from tests.gpu_util import plan_for, rel_l2, to_dev
 
 pytestmark = pytest.mark.gpu
+TOL = 1e-10
 PER, WALL = 0, 1
-
-
-def _lam(m, n, d):
-    return -2.0 * (1.0 - np.cos(2.0 * np.pi * m / n)) / d ** 2
-
-
-def _coef_xy(f, kx, ky):
-    """sum_{i,j} f[k,j,i] exp(-2 pi i (kx i / nx + ky j / ny)) for every k -> (nz,) complex"""
-    nz, ny, nx = f.shape
-    ex = np.exp(-2j * np.pi * kx * np.arange(nx) / nx)
-    ey = np.exp(-2j * np.pi * ky * np.arange(ny) / ny)
-    g = (f @ ex.real) + 1j * (f @ ex.imag)          # (nz, ny): two real matrix-vector products, no complex copy of f
-    return g @ ey
 
 
 def _run_step(W):
@@ -51,62 +40,40 @@ def _run_step(W):
     return rhs_gpu, out
 
 
-def _check_full_size(oracle, W, modes, tol_coef):
-    rhs_gpu, (u, v, w, p) = _run_step(W)
-    shape, box, wall = W.shape, W.box, W.bc_z == WALL
-    nz, ny, nx = shape
-    dx, dy, dz = box[0] / nx, box[1] / ny, box[2] / nz
-
-    # (a) right-hand side, element by element
-    rhs = oracle.rhs(*W.fields(), box, W.bc_z, W.rho1, W.rho2, W.dt)
+def _check_full_size(oracle, W):
+    rhs_gpu, got = _run_step(W)
+    box, wall = W.box, W.bc_z == WALL
+    t0 = time.perf_counter()
+    *want, rhs = oracle.projection_step(*W.fields(), box, W.bc_z, W.rho1, W.rho2, W.dt, return_rhs=True)
+    osec = time.perf_counter() - t0
     e_rhs = rel_l2(rhs_gpu, rhs)
     del rhs_gpu
-    # (b) correction, element by element, given the GPU pressure
-    uo, vo, wo = oracle.correction(*W.fields(), p, box, W.bc_z, W.rho1, W.rho2, W.dt)
-    e_u, e_v, e_w = rel_l2(u, uo), rel_l2(v, vo), rel_l2(w, wo)
-    del uo, vo, wo
-    # (c) residual, gauge, divergence
+    errs = {n: rel_l2(g, w_) for n, g, w_ in zip("uvwp", got, want)}
+    mx = {n: float(np.max(np.abs(g - w_))) for n, g, w_ in zip("uvwp", got, want)}
+    del want
+    u, v, w, p = got
     rn = np.linalg.norm(rhs)
     res = np.linalg.norm(oracle.laplacian(p, box, W.bc_z) - (rhs - rhs.mean())) / rn
+    del rhs
     mean_p = abs(p.mean()) / np.sqrt(np.mean(p * p))
     dn = np.linalg.norm(oracle.divergence(u, v, w, box, W.bc_z)) / np.linalg.norm(oracle.divergence(W.u, W.v, W.w, box, W.bc_z))
-    # (d) sampled spectral coefficients of p against the definition
-    e_coef = []
-    for (kx, ky, kz) in modes:
-        r_k, p_k = _coef_xy(rhs, kx, ky), _coef_xy(p, kx, ky)
-        lxy = _lam(kx, nx, dx) + _lam(ky, ny, dy)
-        if not wall:
-            ez = np.exp(-2j * np.pi * kz * np.arange(nz) / nz)
-            want, got = (r_k @ ez) / (lxy + _lam(kz, nz, dz)), p_k @ ez
-            e_coef.append(abs(got - want) / abs(want))
-        else:
-            from scipy.linalg import solve_banded
-            ab = np.zeros((3, nz))
-            ab[0, 1:] = 1.0 / dz ** 2
-            ab[2, :-1] = 1.0 / dz ** 2
-            ab[1, :] = -2.0 / dz ** 2 + lxy
-            ab[1, 0] = ab[1, -1] = -1.0 / dz ** 2 + lxy
-            want = solve_banded((1, 1), ab, r_k)
-            e_coef.append(np.linalg.norm(p_k - want) / np.linalg.norm(want))
-    print(W.name, f"rhs {e_rhs:.2e} u {e_u:.2e} v {e_v:.2e} w {e_w:.2e} residual {res:.2e} mean {mean_p:.2e} "
-                  f"div {dn:.2e} coef {max(e_coef):.2e}")
+    print(f"\n{W.name}: rel L2 vs the full oracle  u {errs['u']:.1e}  v {errs['v']:.1e}  w {errs['w']:.1e}  p {errs['p']:.1e}"
+          f"  (max abs p {mx['p']:.1e});  rhs {e_rhs:.1e}  residual {res:.1e}  mean {mean_p:.1e}  div {dn:.1e};"
+          f"  oracle {osec:.1f} s on {oracle.threads(0)} threads")
     assert e_rhs <= 1e-13
-    assert max(e_u, e_v, e_w) <= 1e-12
+    for n, e in errs.items():
+        assert e <= TOL, (W.name, n, e)
     assert res <= 1e-11 and mean_p <= 1e-10 and dn <= 1e-11
-    assert max(e_coef) <= tol_coef
     if wall:
         assert np.array_equal(w[-1], W.w[-1])
 
 
-def test_config4_full_size(oracle_mod):
-    """512^3 triply periodic, rho2/rho1 = 50 (bench.py's primary workload)"""
-    W = wl.config4(512, 50.0)
-    modes = [(1, 0, 0), (0, 3, 0), (0, 0, 5), (7, 11, 13), (100, 200, 255), (256, 256, 256), (256, 1, 300), (33, 500, 2)]
-    _check_full_size(oracle_mod, W, modes, 1e-9)
+@pytest.mark.parametrize("ratio", [1.0, 50.0])
+def test_config4_full_size(oracle_mod, ratio):
+    """512^3 triply periodic, the density-ratio sweep {1, 50} (rho2/rho1 = 50 is bench.py's primary workload)"""
+    _check_full_size(oracle_mod, wl.config4(512, ratio))
 
 
 def test_config5_full_size(oracle_mod):
     """1024 x 1024 x 512 wall-bounded, rho2/rho1 = 1000 (bench.py's second workload)"""
-    W = wl.config5()
-    modes = [(1, 0, 0), (0, 2, 0), (37, 411, 0), (512, 512, 0)]
-    _check_full_size(oracle_mod, W, modes, 1e-8)
+    _check_full_size(oracle_mod, wl.config5())

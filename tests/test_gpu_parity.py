@@ -5,7 +5,7 @@ import pytest
 import torch
 
 import paper_2204_08834_b200 as fl
-from paper_2204_08834_b200 import workloads as wl
+import workloads as wl
 from tests import np_ops as ops
 from tests.gpu_util import gpu_step, plan_for, rel_l2, to_dev
 
@@ -50,7 +50,8 @@ def test_splitting_rhs_matches_oracle(oracle_mod, maker):
 
 @pytest.mark.parametrize("shape,bc", [
     ((32, 32, 32), PER), ((8, 8, 16), PER), ((16, 64, 128), PER), ((64, 16, 256), PER), ((128, 32, 32), PER),
-    ((512, 8, 16), PER), ((8, 512, 16), PER), ((8, 8, 1024), PER),
+    ((512, 8, 16), PER), ((8, 512, 16), PER), ((8, 8, 1024), PER), ((1024, 8, 16), PER), ((8, 16, 8), PER),
+    ((16, 64, 2048), PER), ((9, 8, 8), WALL),
     ((2, 8, 16), WALL), ((3, 16, 32), WALL), ((20, 32, 64), WALL), ((37, 64, 16), WALL), ((128, 8, 512), WALL)])
 def test_poisson_solve_matches_oracle(oracle_mod, shape, bc):
     """sizes span: minimum sizes, every radix tail (r = 1, 2, 4), non-power-of-two nz for walls,
@@ -111,7 +112,11 @@ def test_step_config5_shape_small(oracle_mod):
 
 
 @pytest.mark.parametrize("maker", [
-    lambda: wl.random_case(16, 8, 8, PER, 10.0, 11),          # smallest supported periodic grid
+    lambda: wl.random_case(8, 8, 8, PER, 10.0, 10),           # smallest supported periodic grid (nx = 8: degenerate x kernels)
+    lambda: wl.random_case(8, 16, 5, WALL, 100.0, 9),
+    lambda: wl.random_case(16, 8, 8, PER, 10.0, 11),
+    lambda: wl.random_case(32, 64, 1024, PER, 20.0, 18),      # periodic z of 1024: the 4-column one-butterfly z kernel
+    lambda: wl.random_case(2048, 32, 16, WALL, 20.0, 19),     # maximum nx with more than one tile of rows
     lambda: wl.random_case(16, 8, 2, WALL, 10.0, 12),         # smallest wall grid
     lambda: wl.random_case(2048, 8, 8, PER, 5.0, 13),         # maximum nx
     lambda: wl.random_case(16, 2048, 8, WALL, 5.0, 14),       # maximum ny (4-column tiles)
@@ -121,6 +126,57 @@ def test_step_config5_shape_small(oracle_mod):
 ])
 def test_step_edge_sizes(oracle_mod, maker):
     _assert_step_parity(oracle_mod, maker())
+
+
+def test_equal_densities_make_the_step_independent_of_the_pressure_history_bit_for_bit():
+    """rho1 == rho2: the splitting coefficient is exactly 0 on the GPU too (P6), so p and p_old
+    cannot influence the result at all"""
+    W = wl.random_case(128, 32, 16, WALL, 1.0, 24)
+    a = gpu_step(W)
+    rng = np.random.default_rng(5)
+    W.p, W.p_old = rng.standard_normal(W.shape), rng.standard_normal(W.shape)
+    b = gpu_step(W)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+
+
+def test_workspace_is_the_callers_torch_memory(oracle_mod):
+    """flutas_plan_set_workspace: the default binding hands the plan ONE torch tensor; torch's allocator accounts for
+    it; the same step on a library-owned workspace, on a second caller buffer and after switching back and forth gives
+    the same bits; a buffer that is too small or misaligned is refused"""
+    W = wl.random_case(128, 32, 20, WALL, 10.0, 25)
+    need = fl.binding.workspace_bytes(W.nx, W.ny, W.nz, W.bc_z)
+    torch.cuda.synchronize()
+    before = torch.cuda.memory_allocated()
+    plan = plan_for(W)
+    assert plan.workspace_bytes == need
+    assert torch.cuda.memory_allocated() - before >= need                 # the workspace is torch's
+    want = gpu_step(W, plan)
+    ref = _oracle_step(oracle_mod, W)
+    for g, r in zip(want, ref):
+        assert rel_l2(g, r) <= TOL
+    lib_plan = fl.Plan(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2, workspace="library")
+    for g, r in zip(gpu_step(W, lib_plan), want):
+        assert np.array_equal(g, r)
+    lib_plan.destroy()
+    other = torch.empty(need + 4096, dtype=torch.uint8, device="cuda")
+    plan.set_workspace(other[256:])                                        # any 256-byte aligned view will do
+    for g, r in zip(gpu_step(W, plan), want):
+        assert np.array_equal(g, r)
+    with pytest.raises(fl.FlutasError):
+        plan.set_workspace(other[8:])                                      # misaligned
+    with pytest.raises(fl.FlutasError):
+        plan.set_workspace(other[:need - 1024])                            # too small
+    plan.set_workspace(None)                                               # back to a library-owned one
+    for g, r in zip(gpu_step(W, plan), want):
+        assert np.array_equal(g, r)
+    plan.destroy()
+    # a plan created for a caller workspace refuses to step without one
+    h = fl.lib.flutas_plan_create_ex(W.nx, W.ny, W.nz, *W.box, 0, 0, W.bc_z, W.rho1, W.rho2, fl.binding.PLAN_CALLER_WORKSPACE)
+    d = [to_dev(a) for a in W.fields()]
+    assert fl.lib.flutas_projection_step(h, *[t.data_ptr() for t in d], W.dt, None) == 1
+    assert b"workspace" in fl.lib.flutas_last_error()
+    fl.lib.flutas_plan_destroy(h)
 
 
 def test_step_is_deterministic_and_plan_is_reusable(oracle_mod):
@@ -164,6 +220,7 @@ def test_non_default_stream_and_timing(oracle_mod):
     ms, steps = plan.read_timing()
     assert steps == 1 and len(ms) == len(plan.kernel_names) == 7 and all(m > 0 for m in ms)
     assert plan.kernel_names[0] == "splitting_rhs" and plan.kernel_names[-1] == "correction"
+    assert plan.kernel_symbols[0] == "splitting_rhs_kernel2" and plan.kernel_symbols[3] == "fft_tma1_kernel"
     plan.destroy()
 
 

@@ -6,7 +6,7 @@ import pytest
 import torch
 
 import paper_2204_08834_b200 as fl
-from paper_2204_08834_b200 import workloads as wl
+import workloads as wl
 from tests.gpu_util import gpu_step, plan_for, rel_l2, to_dev
 
 pytestmark = pytest.mark.gpu

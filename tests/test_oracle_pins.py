@@ -20,7 +20,7 @@ pressure or a divergence), so the pins are structural:
 import numpy as np
 import pytest
 
-from paper_2204_08834_b200 import workloads as wl
+import workloads as wl
 from tests import np_ops as ops
 
 PER, WALL = 0, 1
@@ -170,6 +170,37 @@ def test_p3b_fixed_point(oracle_mod, bc, ratio):
     assert ops.rel_l2(pn, p) < 1e-10
     for a, b in ((u, ut), (v, vt), (w, wt)):
         assert ops.rel_l2(a, b) < 1e-12
+
+
+# ------------------------------------------- P3c: the correction entry point on its own
+@pytest.mark.parametrize("bc,ratio", [(PER, 50.0), (WALL, 1000.0)])
+def test_p3c_correction_entry_point(oracle_mod, bc, ratio):
+    """oracle.correction (the call that certifies u, v, w at full size) against an independent numpy statement of
+    eq. 18 in the north_star grouping, against the step it is a part of (bit for bit), and with its pressure
+    arguments swapped (must differ: a transposed p / p_old / p_new in the entry point or its wrapper fails here)."""
+    W = wl.random_case(12, 10, 8, bc, ratio, 61)
+    wall = bc == WALL
+    rhs = oracle_mod.rhs(*W.fields(), W.box, bc, W.rho1, W.rho2, W.dt)
+    pn = oracle_mod.poisson(rhs, W.box, bc)
+    got = oracle_mod.correction(*W.fields(), pn, W.box, bc, W.rho1, W.rho2, W.dt)
+    # (a) independent numpy restatement: u = u* - dt [ grad p_new / rho0 + (1/rho_f - 1/rho0) grad p_hat ]
+    rho0 = min(W.rho1, W.rho2)
+    rf = ops.face_density(W.phi, W.rho1, W.rho2, wall)
+    gn, gh = ops.grad(pn, W.box, wall), ops.grad(2.0 * W.p - W.p_old, W.box, wall)
+    for a, us, r, g1, g2 in zip(got, (W.u, W.v, W.w), rf, gn, gh):
+        assert ops.rel_l2(a, us - W.dt * (g1 / rho0 + (1.0 / r - 1.0 / rho0) * g2)) < 1e-13
+    # (b) the same arithmetic as the whole step: bit for bit
+    step = _step(oracle_mod, W)
+    for a, b in zip(got, step[:3]):
+        assert np.array_equal(a, b)
+    assert np.array_equal(pn, step[3])
+    # (c) every transposition of the three pressure arguments changes the result
+    f = W.fields()
+    for perm in ((pn, f[5], f[4]), (f[4], pn, f[5]), (f[5], f[4], pn), (f[4], f[5], f[4])):
+        bad = oracle_mod.correction(f[0], f[1], f[2], f[3], perm[0], perm[1], perm[2], W.box, bc, W.rho1, W.rho2, W.dt)
+        assert ops.rel_l2(bad[0], got[0]) > 1e-6
+    if wall:
+        assert np.array_equal(got[2][-1], W.w[-1])
 
 
 # --------------------------------------------------------------------- P6: special cases

@@ -1,7 +1,7 @@
 """Host-side checks of the seeded input generators (no method arithmetic here)."""
 import numpy as np
 
-from paper_2204_08834_b200 import workloads as wl
+import workloads as wl
 
 
 def test_mode_sum_matches_direct_evaluation():
