@@ -20,6 +20,7 @@
 
 typedef struct {
     int nx, ny, nz, wall;
+    int bcx, bcy, bcz;   /* ORACLE_BC_PERIODIC / _NEUMANN / _DIRICHLET per direction; wall = (bcz == NEUMANN) */
     double dx, dy, dz;
     double rho1, rho2, rho0, dt;
     double r;   /* dt^(n+1) / dt^n, the time-step ratio of the pressure extrapolation; 1 = constant dt */
@@ -32,11 +33,23 @@ static int grid_init(grid_t *g, int nx, int ny, int nz, double lx, double ly, do
     if (bc_z != ORACLE_BC_Z_PERIODIC && bc_z != ORACLE_BC_Z_WALL) return 1;
     if (bc_z == ORACLE_BC_Z_WALL && nz < 2) return 1;
     g->nx = nx; g->ny = ny; g->nz = nz; g->wall = (bc_z == ORACLE_BC_Z_WALL);
+    g->bcx = ORACLE_BC_PERIODIC; g->bcy = ORACLE_BC_PERIODIC; g->bcz = bc_z;
     g->dx = lx / nx; g->dy = ly / ny; g->dz = lz / nz;         /* uniform spacing */
     g->rho1 = rho1; g->rho2 = rho2;
     g->rho0 = rho1 < rho2 ? rho1 : rho2;                        /* rho0 = min density, PAPER.md:161 (R3) */
     g->dt = dt;
     g->r = 1.0;
+    return 0;
+}
+
+/* the same with boundary conditions along x and y as well; Dirichlet along z is allowed here (Poisson problem only) */
+static int grid_init_bc(grid_t *g, int nx, int ny, int nz, double lx, double ly, double lz,
+                        int bc_x, int bc_y, int bc_z, double rho1, double rho2, double dt) {
+    if (bc_x < 0 || bc_x > 2 || bc_y < 0 || bc_y > 2 || bc_z < 0 || bc_z > 2) return 1;
+    if (grid_init(g, nx, ny, nz, lx, ly, lz, bc_z == ORACLE_BC_DIRICHLET ? ORACLE_BC_NEUMANN : bc_z, rho1, rho2, dt)) return 1;
+    if ((bc_x != ORACLE_BC_PERIODIC && nx < 2) || (bc_y != ORACLE_BC_PERIODIC && ny < 2)) return 1;
+    g->bcx = bc_x; g->bcy = bc_y; g->bcz = bc_z;
+    g->wall = (bc_z == ORACLE_BC_NEUMANN);
     return 0;
 }
 
@@ -64,22 +77,37 @@ static inline double p_hat(const grid_t *g, const double *p, const double *p_old
 }
 
 /* gradient of a centred field f on the east / north / top face of cell (i,j,k) */
+/* On the LAST face of a non-periodic direction (the boundary face): Neumann -> the normal gradient is 0 (a wall,
+ * PAPER.md:161, R8); Dirichlet -> f = 0 ON the face, i.e. ghost value -f_last (cell-centred reflection), so the
+ * gradient is (-f_last - f_last)/d. */
 static inline double grad_x(const grid_t *g, const double *f, int i, int j, int k) {
+    if (g->bcx != ORACLE_BC_PERIODIC && i == g->nx - 1)
+        return g->bcx == ORACLE_BC_NEUMANN ? 0.0 : (-f[at(g, i, j, k)] - f[at(g, i, j, k)]) / g->dx;
     return (f[at(g, wrap(i + 1, g->nx), j, k)] - f[at(g, i, j, k)]) / g->dx;
 }
 static inline double grad_y(const grid_t *g, const double *f, int i, int j, int k) {
+    if (g->bcy != ORACLE_BC_PERIODIC && j == g->ny - 1)
+        return g->bcy == ORACLE_BC_NEUMANN ? 0.0 : (-f[at(g, i, j, k)] - f[at(g, i, j, k)]) / g->dy;
     return (f[at(g, i, wrap(j + 1, g->ny), k)] - f[at(g, i, j, k)]) / g->dy;
 }
 static inline double grad_z(const grid_t *g, const double *f, int i, int j, int k) {
     if (g->wall && k == g->nz - 1) return 0.0;    /* top wall face: normal gradient is 0 (R8) */
+    if (g->bcz == ORACLE_BC_DIRICHLET && k == g->nz - 1) return (-f[at(g, i, j, k)] - f[at(g, i, j, k)]) / g->dz;
     return (f[at(g, i, j, wrap(k + 1, g->nz))] - f[at(g, i, j, k)]) / g->dz;
+}
+/* gradient on the FIRST boundary face of a non-periodic direction (west / south / bottom of cell 0; not a stored
+ * face): Neumann 0, Dirichlet (f_0 - (-f_0))/d */
+static inline double grad_first_face(int bc, double f0, double d) {
+    return bc == ORACLE_BC_NEUMANN ? 0.0 : (f0 + f0) / d;
 }
 
 /* the same three gradients for p_hat */
 static inline double gph_x(const grid_t *g, const double *p, const double *po, int i, int j, int k) {
+    if (g->bcx == ORACLE_BC_NEUMANN && i == g->nx - 1) return 0.0;      /* east wall face */
     return (p_hat(g, p, po, wrap(i + 1, g->nx), j, k) - p_hat(g, p, po, i, j, k)) / g->dx;
 }
 static inline double gph_y(const grid_t *g, const double *p, const double *po, int i, int j, int k) {
+    if (g->bcy == ORACLE_BC_NEUMANN && j == g->ny - 1) return 0.0;      /* north wall face */
     return (p_hat(g, p, po, i, wrap(j + 1, g->ny), k) - p_hat(g, p, po, i, j, k)) / g->dy;
 }
 static inline double gph_z(const grid_t *g, const double *p, const double *po, int i, int j, int k) {
@@ -89,9 +117,11 @@ static inline double gph_z(const grid_t *g, const double *p, const double *po, i
 
 /* face densities: arithmetic mean of the two adjacent cells (R2) */
 static inline double rho_fx(const grid_t *g, const double *phi, int i, int j, int k) {
+    if (g->bcx == ORACLE_BC_NEUMANN && i == g->nx - 1) return rho_c(g, phi, i, j, k);   /* wall face: as rho_fz below */
     return 0.5 * (rho_c(g, phi, i, j, k) + rho_c(g, phi, wrap(i + 1, g->nx), j, k));
 }
 static inline double rho_fy(const grid_t *g, const double *phi, int i, int j, int k) {
+    if (g->bcy == ORACLE_BC_NEUMANN && j == g->ny - 1) return rho_c(g, phi, i, j, k);
     return 0.5 * (rho_c(g, phi, i, j, k) + rho_c(g, phi, i, wrap(j + 1, g->ny), k));
 }
 static inline double rho_fz(const grid_t *g, const double *phi, int i, int j, int k) {
@@ -113,8 +143,9 @@ static inline double flux_z(const grid_t *g, const double *phi, const double *p,
 
 /* divergence of a face field at cell (i,j,k); the bottom wall face (k = -1) is 0 and not stored */
 static inline double div_at(const grid_t *g, const double *a, const double *b, const double *c, int i, int j, int k) {
-    double am = a[at(g, wrap(i - 1, g->nx), j, k)];
-    double bm = b[at(g, i, wrap(j - 1, g->ny), k)];
+    /* the first wall face of a walled direction (west / south / bottom) carries 0 and is not stored */
+    double am = (g->bcx == ORACLE_BC_NEUMANN && i == 0) ? 0.0 : a[at(g, wrap(i - 1, g->nx), j, k)];
+    double bm = (g->bcy == ORACLE_BC_NEUMANN && j == 0) ? 0.0 : b[at(g, i, wrap(j - 1, g->ny), k)];
     double cm = (g->wall && k == 0) ? 0.0 : c[at(g, i, j, wrap(k - 1, g->nz))];
     size_t q = at(g, i, j, k);
     return (a[q] - am) / g->dx + (b[q] - bm) / g->dy + (c[q] - cm) / g->dz;
@@ -124,8 +155,15 @@ static inline double div_at(const grid_t *g, const double *a, const double *b, c
 
 int oracle_divergence(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
                       const double *u, const double *v, const double *w, double *div_out, int nthreads) {
+    return oracle_divergence_bc(nx, ny, nz, lx, ly, lz, ORACLE_BC_PERIODIC, ORACLE_BC_PERIODIC, bc_z, u, v, w, div_out, nthreads);
+}
+
+/* walls (Neumann) along x / y as along z: the first wall face carries 0 and is not stored */
+int oracle_divergence_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                         const double *u, const double *v, const double *w, double *div_out, int nthreads) {
     grid_t g;
-    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, 1.0, 1.0, 1.0)) return 1;
+    if (bc_x == ORACLE_BC_DIRICHLET || bc_y == ORACLE_BC_DIRICHLET || bc_z == ORACLE_BC_DIRICHLET) return 1;
+    if (grid_init_bc(&g, nx, ny, nz, lx, ly, lz, bc_x, bc_y, bc_z, 1.0, 1.0, 1.0)) return 1;
     set_threads(nthreads);
 #pragma omp parallel for collapse(2) schedule(static)
     for (int k = 0; k < nz; ++k)
@@ -137,17 +175,25 @@ int oracle_divergence(int nx, int ny, int nz, double lx, double ly, double lz, i
 /* L p = div(grad p): (Gx p[i] - Gx p[i-1])/dx + ... with the wall faces carrying 0 */
 int oracle_laplacian(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
                      const double *p, double *lap_out, int nthreads) {
+    return oracle_laplacian_bc(nx, ny, nz, lx, ly, lz, ORACLE_BC_PERIODIC, ORACLE_BC_PERIODIC, bc_z, p, lap_out, nthreads);
+}
+
+int oracle_laplacian_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                        const double *p, double *lap_out, int nthreads) {
     grid_t g;
-    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, 1.0, 1.0, 1.0)) return 1;
+    if (grid_init_bc(&g, nx, ny, nz, lx, ly, lz, bc_x, bc_y, bc_z, 1.0, 1.0, 1.0)) return 1;
     set_threads(nthreads);
 #pragma omp parallel for collapse(2) schedule(static)
     for (int k = 0; k < nz; ++k)
         for (int j = 0; j < ny; ++j)
             for (int i = 0; i < nx; ++i) {
-                double gxp = grad_x(&g, p, i, j, k), gxm = grad_x(&g, p, wrap(i - 1, nx), j, k);
-                double gyp = grad_y(&g, p, i, j, k), gym = grad_y(&g, p, i, wrap(j - 1, ny), k);
-                double gzp = grad_z(&g, p, i, j, k);
-                double gzm = (g.wall && k == 0) ? 0.0 : grad_z(&g, p, i, j, wrap(k - 1, nz));
+                double gxp = grad_x(&g, p, i, j, k), gyp = grad_y(&g, p, i, j, k), gzp = grad_z(&g, p, i, j, k);
+                double gxm = (g.bcx != ORACLE_BC_PERIODIC && i == 0) ? grad_first_face(g.bcx, p[at(&g, i, j, k)], g.dx)
+                                                                      : grad_x(&g, p, wrap(i - 1, nx), j, k);
+                double gym = (g.bcy != ORACLE_BC_PERIODIC && j == 0) ? grad_first_face(g.bcy, p[at(&g, i, j, k)], g.dy)
+                                                                      : grad_y(&g, p, i, wrap(j - 1, ny), k);
+                double gzm = (g.bcz != ORACLE_BC_PERIODIC && k == 0) ? grad_first_face(g.bcz, p[at(&g, i, j, k)], g.dz)
+                                                                      : grad_z(&g, p, i, j, wrap(k - 1, nz));
                 lap_out[at(&g, i, j, k)] = (gxp - gxm) / g.dx + (gyp - gym) / g.dy + (gzp - gzm) / g.dz;
             }
     return 0;
@@ -159,8 +205,17 @@ int oracle_rhs_vdt(int nx, int ny, int nz, double lx, double ly, double lz, int 
                    double rho1, double rho2, double dt, double dt_ratio,
                    const double *u, const double *v, const double *w, const double *phi,
                    const double *p, const double *p_old, double *rhs_out, int nthreads) {
+    return oracle_rhs_bc(nx, ny, nz, lx, ly, lz, ORACLE_BC_PERIODIC, ORACLE_BC_PERIODIC, bc_z, rho1, rho2, dt, dt_ratio,
+                         u, v, w, phi, p, p_old, rhs_out, nthreads);
+}
+
+int oracle_rhs_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                  double rho1, double rho2, double dt, double dt_ratio,
+                  const double *u, const double *v, const double *w, const double *phi,
+                  const double *p, const double *p_old, double *rhs_out, int nthreads) {
     grid_t g;
-    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt)) return 1;
+    if (bc_x == ORACLE_BC_DIRICHLET || bc_y == ORACLE_BC_DIRICHLET || bc_z == ORACLE_BC_DIRICHLET) return 1;
+    if (grid_init_bc(&g, nx, ny, nz, lx, ly, lz, bc_x, bc_y, bc_z, rho1, rho2, dt)) return 1;
     if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0) || !(dt_ratio > 0.0)) return 1;
     g.r = dt_ratio;
     set_threads(nthreads);
@@ -172,9 +227,9 @@ int oracle_rhs_vdt(int nx, int ny, int nz, double lx, double ly, double lz, int 
                 double d_u = div_at(&g, u, v, w, i, j, k);
                 /* div[(1 - rho0/rho) grad p_hat]  -- splitting term of eq. (16) moved to the RHS (R1) */
                 double fxp = flux_x(&g, phi, p, p_old, i, j, k);
-                double fxm = flux_x(&g, phi, p, p_old, wrap(i - 1, nx), j, k);
+                double fxm = (g.bcx == ORACLE_BC_NEUMANN && i == 0) ? 0.0 : flux_x(&g, phi, p, p_old, wrap(i - 1, nx), j, k);
                 double fyp = flux_y(&g, phi, p, p_old, i, j, k);
-                double fym = flux_y(&g, phi, p, p_old, i, wrap(j - 1, ny), k);
+                double fym = (g.bcy == ORACLE_BC_NEUMANN && j == 0) ? 0.0 : flux_y(&g, phi, p, p_old, i, wrap(j - 1, ny), k);
                 double fzp = flux_z(&g, phi, p, p_old, i, j, k);
                 double fzm = (g.wall && k == 0) ? 0.0 : flux_z(&g, phi, p, p_old, i, j, wrap(k - 1, nz));
                 double d_f = (fxp - fxm) / g.dx + (fyp - fym) / g.dy + (fzp - fzm) / g.dz;
@@ -244,6 +299,57 @@ int oracle_dft_axis(long n_outer, int n, long n_inner, int sign,
     return 0;
 }
 
+/* ------------------------------------------- naive cosine / sine expansions (non-periodic directions)
+ *
+ * "Fourier-based expansions [that] depend on the boundary conditions": the eigenvectors of the
+ * second-difference operator on n cell centres (i + 1/2) d with homogeneous conditions at both boundary FACES are
+ *   Neumann   (ghost f_{-1} = f_0, f_n = f_{n-1}):    e_m[i] = cos(pi m (2i+1) / (2n)),      m = 0..n-1
+ *   Dirichlet (ghost f_{-1} = -f_0, f_n = -f_{n-1}):  e_m[i] = sin(pi (m+1) (2i+1) / (2n)),  m = 0..n-1
+ * with eigenvalues -2 (1 - cos(pi m / n)) / d^2 and -2 (1 - cos(pi (m+1) / n)) / d^2 (oracle_eigenvalues).
+ * They are orthogonal: sum_i e_m[i]^2 = n for the constant / alternating vector (Neumann m = 0, Dirichlet m = n-1),
+ * n/2 otherwise.  sign = -1 (analysis):  c_m = sum_i f[i] e_m[i] / |e_m|^2;   sign = +1 (synthesis):  f[i] = sum_m c_m e_m[i].
+ * Both are plain O(n^2) sums; the argument of cos / sin is reduced exactly in integers (q mod 4n) and looked up in a
+ * table evaluated in long double.  Real data, (n_outer, n, n_inner) C order like oracle_dft_axis. */
+int oracle_r2r_axis(long n_outer, int n, long n_inner, int bc, int sign,
+                    const double *in, double *out, int nthreads) {
+    if (n_outer < 1 || n < 1 || n_inner < 1 || (sign != 1 && sign != -1)) return 1;
+    if (bc != ORACLE_BC_NEUMANN && bc != ORACLE_BC_DIRICHLET) return 1;
+    const int n4 = 4 * n;
+    double *tab = (double *)malloc(sizeof(double) * (size_t)n4);   /* cos (Neumann) or sin (Dirichlet) of pi q / (2n) */
+    if (!tab) return 2;
+    const long double pi = 3.141592653589793238462643383279502884L;
+    for (int q = 0; q < n4; ++q) {
+        long double a = pi * (long double)q / (long double)(2 * n);
+        tab[q] = (double)(bc == ORACLE_BC_NEUMANN ? cosl(a) : sinl(a));
+    }
+    const int mode_shift = bc == ORACLE_BC_NEUMANN ? 0 : 1;        /* mode m has "frequency" m (Neumann) or m + 1 (Dirichlet) */
+    const int long_mode = bc == ORACLE_BC_NEUMANN ? 0 : n - 1;     /* the one mode of squared norm n */
+    set_threads(nthreads);
+    long n_batch = (n_inner + LINE_BATCH - 1) / LINE_BATCH;
+#pragma omp parallel for collapse(2) schedule(dynamic, 1)
+    for (long o = 0; o < n_outer; ++o)
+        for (long b = 0; b < n_batch; ++b) {
+            long q0 = b * LINE_BATCH;
+            int len = (int)((n_inner - q0) < LINE_BATCH ? (n_inner - q0) : LINE_BATCH);
+            double acc[LINE_BATCH];
+            for (int r = 0; r < n; ++r) {            /* output index: mode m (analysis) or cell i (synthesis) */
+                for (int q = 0; q < len; ++q) acc[q] = 0.0;
+                for (int t = 0; t < n; ++t) {        /* the O(n) sum, in increasing index */
+                    int m = sign < 0 ? r : t, i = sign < 0 ? t : r;
+                    int arg = (int)(((long)(m + mode_shift) * (long)(2 * i + 1)) % n4);
+                    double e = tab[arg];
+                    const double *x = in + ((size_t)o * n + t) * (size_t)n_inner + q0;
+                    for (int q = 0; q < len; ++q) acc[q] += e * x[q];
+                }
+                double norm2 = (sign < 0) ? ((r == long_mode) ? (double)n : 0.5 * (double)n) : 1.0;
+                double *y = out + ((size_t)o * n + r) * (size_t)n_inner + q0;
+                for (int q = 0; q < len; ++q) y[q] = acc[q] / norm2;
+            }
+        }
+    free(tab);
+    return 0;
+}
+
 /* eigenvalues of the periodic second-difference operator (R6):
  * lambda[m] = -2 (1 - cos(2 pi m / n)) / d^2 */
 static double *eigenvalues(int n, double d) {
@@ -254,6 +360,26 @@ static double *eigenvalues(int n, double d) {
         lam[m] = (double)(-2.0L * (1.0L - cosl(two_pi * (long double)m / (long double)n))) / (d * d);
     return lam;
 }
+/* ... and of the Neumann / Dirichlet second difference: -2 (1 - cos(pi m / n)) / d^2, -2 (1 - cos(pi (m+1) / n)) / d^2 */
+static double *eigenvalues_bc(int n, double d, int bc) {
+    if (bc == ORACLE_BC_PERIODIC) return eigenvalues(n, d);
+    double *lam = (double *)malloc(sizeof(double) * (size_t)n);
+    if (!lam) return NULL;
+    const long double pi = 3.141592653589793238462643383279502884L;
+    for (int m = 0; m < n; ++m) {
+        int f = bc == ORACLE_BC_NEUMANN ? m : m + 1;
+        lam[m] = (double)(-2.0L * (1.0L - cosl(pi * (long double)f / (long double)n))) / (d * d);
+    }
+    return lam;
+}
+int oracle_eigenvalues(int n, double d, int bc, double *lam_out) {
+    if (n < 1 || !(d > 0.0) || bc < 0 || bc > 2) return 1;
+    double *lam = eigenvalues_bc(n, d, bc);
+    if (!lam) return 2;
+    memcpy(lam_out, lam, sizeof(double) * (size_t)n);
+    free(lam);
+    return 0;
+}
 
 /* ------------------------------------------------------ tridiagonal in z */
 
@@ -261,12 +387,14 @@ static double *eigenvalues(int n, double d) {
  * b_k = -2/dz^2 + lam_xy inside, -1/dz^2 + lam_xy in the first/last row (Neumann, R7).
  * d is complex (dr, di), the coefficients are real.  stride = distance between k and k+1.
  * singular != 0 (the (0,0) column, lam_xy = 0): eliminate rows 0..nz-2, pin x_{nz-1} = 0,
- * back-substitute, then remove the mean over k (R5). cp, dpr, dpi: scratch of length nz. */
-static void thomas_column(int nz, double dz, double lam_xy, int singular,
+ * back-substitute, then remove the mean over k (R5). cp, dpr, dpi: scratch of length nz.
+ * end_coef: the diagonal of the first / last row is -end_coef/dz^2 + lam_xy: 1 for Neumann (ghost = interior, R7),
+ * 3 for Dirichlet (ghost = -interior: p = 0 on the boundary face). */
+static void thomas_column(int nz, double dz, double lam_xy, int singular, double end_coef,
                           double *dr, double *di, size_t stride,
                           double *cp, double *dpr, double *dpi) {
     const double a = 1.0 / (dz * dz), c = a;
-    const double b_end = -1.0 / (dz * dz) + lam_xy, b_in = -2.0 / (dz * dz) + lam_xy;
+    const double b_end = -end_coef / (dz * dz) + lam_xy, b_in = -2.0 / (dz * dz) + lam_xy;
     cp[0] = c / b_end;
     dpr[0] = dr[0] / b_end;
     dpi[0] = di[0] / b_end;
@@ -296,31 +424,48 @@ static void thomas_column(int nz, double dz, double lam_xy, int singular,
 
 int oracle_poisson(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
                    const double *rhs, double *p_out, double *imag_residue_out, int nthreads) {
+    return oracle_poisson_bc(nx, ny, nz, lx, ly, lz, ORACLE_BC_PERIODIC, ORACLE_BC_PERIODIC, bc_z, rhs, p_out,
+                             imag_residue_out, nthreads);
+}
+
+/* one expansion step along an axis of the (re, im) pair a -> b: complex DFT when periodic, the real cosine / sine
+ * expansion applied to the real and imaginary parts when not */
+static int expand_axis(long n_outer, int n, long n_inner, int bc, int sign,
+                       const double *ar, const double *ai, double *br, double *bi, int nthreads) {
+    if (bc == ORACLE_BC_PERIODIC) return oracle_dft_axis(n_outer, n, n_inner, sign, ar, ai, br, bi, nthreads);
+    if (oracle_r2r_axis(n_outer, n, n_inner, bc, sign, ar, br, nthreads)) return 2;
+    return oracle_r2r_axis(n_outer, n, n_inner, bc, sign, ai, bi, nthreads);
+}
+
+int oracle_poisson_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                      const double *rhs, double *p_out, double *imag_residue_out, int nthreads) {
     grid_t g;
-    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, 1.0, 1.0, 1.0)) return 1;
+    if (grid_init_bc(&g, nx, ny, nz, lx, ly, lz, bc_x, bc_y, bc_z, 1.0, 1.0, 1.0)) return 1;
     set_threads(nthreads);
     const size_t n = (size_t)nx * ny * nz;
+    /* the operator has a null space (constants) unless some direction is Dirichlet */
+    const int has_null = bc_x != ORACLE_BC_DIRICHLET && bc_y != ORACLE_BC_DIRICHLET && bc_z != ORACLE_BC_DIRICHLET;
     double *ar = (double *)malloc(sizeof(double) * n), *ai = (double *)calloc(n, sizeof(double));
     double *br = (double *)malloc(sizeof(double) * n), *bi = (double *)malloc(sizeof(double) * n);
-    double *lamx = eigenvalues(nx, g.dx), *lamy = eigenvalues(ny, g.dy), *lamz = eigenvalues(nz, g.dz);
+    double *lamx = eigenvalues_bc(nx, g.dx, bc_x), *lamy = eigenvalues_bc(ny, g.dy, bc_y), *lamz = eigenvalues(nz, g.dz);
     int rc = 0;
     if (!ar || !ai || !br || !bi || !lamx || !lamy || !lamz) { rc = 2; goto done; }
     memcpy(ar, rhs, sizeof(double) * n);
 
-    /* step 1: forward transform along x;  a -> b */
-    if (oracle_dft_axis((long)ny * nz, nx, 1, -1, ar, ai, br, bi, nthreads)) { rc = 2; goto done; }
-    /* step 3: forward transform along y;  b -> a   (steps 2,4,6,8 are transposes: no-ops here) */
-    if (oracle_dft_axis(nz, ny, nx, -1, br, bi, ar, ai, nthreads)) { rc = 2; goto done; }
+    /* step 1: forward expansion along x;  a -> b */
+    if (expand_axis((long)ny * nz, nx, 1, bc_x, -1, ar, ai, br, bi, nthreads)) { rc = 2; goto done; }
+    /* step 3: forward expansion along y;  b -> a   (steps 2,4,6,8 are transposes: no-ops here) */
+    if (expand_axis(nz, ny, nx, bc_y, -1, br, bi, ar, ai, nthreads)) { rc = 2; goto done; }
 
-    if (!g.wall) {
-        /* triply periodic: expand along z as well, divide by the eigenvalue sum, (0,0,0) mode -> 0 */
+    if (bc_z == ORACLE_BC_PERIODIC) {
+        /* periodic z: expand along z as well, divide by the eigenvalue sum, the null mode -> 0 */
         if (oracle_dft_axis(1, nz, (long)nx * ny, -1, ar, ai, br, bi, nthreads)) { rc = 2; goto done; }
 #pragma omp parallel for collapse(2) schedule(static)
         for (int kz = 0; kz < nz; ++kz)
             for (int ky = 0; ky < ny; ++ky)
                 for (int kx = 0; kx < nx; ++kx) {
                     size_t q = at(&g, kx, ky, kz);
-                    if (kx == 0 && ky == 0 && kz == 0) { br[q] = 0.0; bi[q] = 0.0; }
+                    if (has_null && kx == 0 && ky == 0 && kz == 0) { br[q] = 0.0; bi[q] = 0.0; }
                     else {
                         double lam = lamx[kx] + lamy[ky] + lamz[kz];
                         br[q] = br[q] / lam;
@@ -331,6 +476,7 @@ int oracle_poisson(int nx, int ny, int nz, double lx, double ly, double lz, int 
     } else {
         /* step 5: Gauss elimination along z for every (kx,ky) */
         int fail = 0;
+        const double end_coef = bc_z == ORACLE_BC_NEUMANN ? 1.0 : 3.0;
 #pragma omp parallel
         {
             double *cp = (double *)malloc(sizeof(double) * (size_t)nz);
@@ -344,7 +490,7 @@ int oracle_poisson(int nx, int ny, int nz, double lx, double ly, double lz, int 
                 for (int ky = 0; ky < ny; ++ky)
                     for (int kx = 0; kx < nx; ++kx) {
                         size_t q = at(&g, kx, ky, 0);
-                        thomas_column(nz, g.dz, lamx[kx] + lamy[ky], (kx == 0 && ky == 0),
+                        thomas_column(nz, g.dz, lamx[kx] + lamy[ky], (has_null && kx == 0 && ky == 0), end_coef,
                                       ar + q, ai + q, (size_t)nx * ny, cp, dpr, dpi);
                     }
             }
@@ -353,14 +499,18 @@ int oracle_poisson(int nx, int ny, int nz, double lx, double ly, double lz, int 
         if (fail) { rc = 2; goto done; }
     }
 
-    /* step 7: backward transform along y;  a -> b */
-    if (oracle_dft_axis(nz, ny, nx, +1, ar, ai, br, bi, nthreads)) { rc = 2; goto done; }
-    /* step 9: backward transform along x;  b -> a */
-    if (oracle_dft_axis((long)ny * nz, nx, 1, +1, br, bi, ar, ai, nthreads)) { rc = 2; goto done; }
+    /* step 7: backward expansion along y;  a -> b */
+    if (expand_axis(nz, ny, nx, bc_y, +1, ar, ai, br, bi, nthreads)) { rc = 2; goto done; }
+    /* step 9: backward expansion along x;  b -> a */
+    if (expand_axis((long)ny * nz, nx, 1, bc_x, +1, br, bi, ar, ai, nthreads)) { rc = 2; goto done; }
 
     {
-        /* normalisation of the unnormalised forward/backward pair (R9); real part */
-        const double norm = g.wall ? (double)nx * (double)ny : (double)nx * (double)ny * (double)nz;
+        /* normalisation of the unnormalised forward/backward DFT pairs (R9; the cosine / sine expansions carry
+         * their own 1/|e_m|^2); real part */
+        double norm = 1.0;
+        if (bc_x == ORACLE_BC_PERIODIC) norm *= (double)nx;
+        if (bc_y == ORACLE_BC_PERIODIC) norm *= (double)ny;
+        if (bc_z == ORACLE_BC_PERIODIC) norm *= (double)nz;
         double max_re = 0.0, max_im = 0.0;
 #pragma omp parallel for reduction(max : max_re, max_im) schedule(static)
         for (size_t q = 0; q < n; ++q) {
@@ -401,8 +551,17 @@ int oracle_correction(int nx, int ny, int nz, double lx, double ly, double lz, i
                       double rho1, double rho2, double dt,
                       double *u, double *v, double *w, const double *phi,
                       const double *p, const double *p_old, const double *p_new, int nthreads) {
+    return oracle_correction_bc(nx, ny, nz, lx, ly, lz, ORACLE_BC_PERIODIC, ORACLE_BC_PERIODIC, bc_z, rho1, rho2, dt,
+                                u, v, w, phi, p, p_old, p_new, nthreads);
+}
+
+int oracle_correction_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                         double rho1, double rho2, double dt,
+                         double *u, double *v, double *w, const double *phi,
+                         const double *p, const double *p_old, const double *p_new, int nthreads) {
     grid_t g;
-    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt)) return 1;
+    if (bc_x == ORACLE_BC_DIRICHLET || bc_y == ORACLE_BC_DIRICHLET || bc_z == ORACLE_BC_DIRICHLET) return 1;
+    if (grid_init_bc(&g, nx, ny, nz, lx, ly, lz, bc_x, bc_y, bc_z, rho1, rho2, dt)) return 1;
     if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0)) return 1;
     set_threads(nthreads);
     correct_velocity(&g, u, v, w, phi, p_new, p, p_old);
@@ -413,17 +572,29 @@ int oracle_projection_step_vdt(int nx, int ny, int nz, double lx, double ly, dou
                                double rho1, double rho2, double dt, double dt_ratio,
                                double *u, double *v, double *w, const double *phi,
                                double *p, const double *p_old, double *rhs_out, int nthreads) {
+    return oracle_projection_step_bc(nx, ny, nz, lx, ly, lz, ORACLE_BC_PERIODIC, ORACLE_BC_PERIODIC, bc_z, rho1, rho2, dt,
+                                     dt_ratio, u, v, w, phi, p, p_old, rhs_out, nthreads);
+}
+
+/* the step with walls (Neumann p, u_n = 0) along x and / or y as well: the closed cavity of PAPER.md:287 is
+ * (NEUMANN, NEUMANN, NEUMANN).  Wall faces: the last stored face of a walled direction is the wall (0 on entry, passed
+ * through), the first wall face is not stored. */
+int oracle_projection_step_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                              double rho1, double rho2, double dt, double dt_ratio,
+                              double *u, double *v, double *w, const double *phi,
+                              double *p, const double *p_old, double *rhs_out, int nthreads) {
     grid_t g;
-    if (grid_init(&g, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt)) return 1;
+    if (bc_x == ORACLE_BC_DIRICHLET || bc_y == ORACLE_BC_DIRICHLET || bc_z == ORACLE_BC_DIRICHLET) return 1;
+    if (grid_init_bc(&g, nx, ny, nz, lx, ly, lz, bc_x, bc_y, bc_z, rho1, rho2, dt)) return 1;
     if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0) || !(dt_ratio > 0.0)) return 1;
     g.r = dt_ratio;
     const size_t n = (size_t)nx * ny * nz;
     double *rhs = (double *)malloc(sizeof(double) * n), *p_new = (double *)malloc(sizeof(double) * n);
     int rc = 0;
     if (!rhs || !p_new) { rc = 2; goto done; }
-    if ((rc = oracle_rhs_vdt(nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, dt, dt_ratio, u, v, w, phi, p, p_old, rhs, nthreads))) goto done;
+    if ((rc = oracle_rhs_bc(nx, ny, nz, lx, ly, lz, bc_x, bc_y, bc_z, rho1, rho2, dt, dt_ratio, u, v, w, phi, p, p_old, rhs, nthreads))) goto done;
     if (rhs_out) memcpy(rhs_out, rhs, sizeof(double) * n);
-    if ((rc = oracle_poisson(nx, ny, nz, lx, ly, lz, bc_z, rhs, p_new, NULL, nthreads))) goto done;
+    if ((rc = oracle_poisson_bc(nx, ny, nz, lx, ly, lz, bc_x, bc_y, bc_z, rhs, p_new, NULL, nthreads))) goto done;
     set_threads(nthreads);
     correct_velocity(&g, u, v, w, phi, p_new, p, p_old);
     memcpy(p, p_new, sizeof(double) * n);                       /* p <- p^(n+1), zero mean */

@@ -36,6 +36,11 @@ extern "C" {
 #endif
 
 enum { ORACLE_BC_Z_PERIODIC = 0, ORACLE_BC_Z_WALL = 1 };
+/* per-direction boundary conditions of the *_bc functions below (homogeneous pressure conditions, PAPER.md:61, 163,
+ * 167): PERIODIC; NEUMANN = a wall (u_n = 0, dp/dn = 0 on the boundary faces); DIRICHLET = p = 0 ON the boundary
+ * faces (Poisson problem and operators only: the step needs the boundary-normal velocity on both boundary faces, which
+ * the nx-faces-per-line layout does not store). */
+enum { ORACLE_BC_PERIODIC = 0, ORACLE_BC_NEUMANN = 1, ORACLE_BC_DIRICHLET = 2 };
 
 /* rhs = rho0/dt * div(u*) + div[(1 - rho0/rho_f) grad p_hat],  p_hat = 2 p - p_old
  * (north_star grouping of eqs. 16-17; reading R1 of DESIGN.md). */
@@ -105,6 +110,42 @@ int oracle_divergence(int nx, int ny, int nz, double lx, double ly, double lz, i
                       int nthreads);
 int oracle_laplacian(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
                      const double *p, double *lap_out, int nthreads);
+
+/* ---- the same path with non-periodic x / y ("all the possible homogeneous pressure boundary conditions",
+ * PAPER.md:163, 167 "Fourier-based expansions [that] depend on the boundary conditions"; closed cavity PAPER.md:287).
+ * bc_x, bc_y, bc_z in {ORACLE_BC_PERIODIC, _NEUMANN, _DIRICHLET}; with all-periodic x, y these are the functions above,
+ * bit for bit (those call these). */
+
+/* naive cosine (Neumann) / sine (Dirichlet) eigen-expansion of REAL data along one axis of an (n_outer, n, n_inner)
+ * array: sign = -1 analysis c_m = <f, e_m> / |e_m|^2, sign = +1 synthesis f = sum_m c_m e_m, with
+ * e_m[i] = cos(pi m (2i+1)/(2n)) or sin(pi (m+1)(2i+1)/(2n)): the eigenvectors of the cell-centred second difference. */
+int oracle_r2r_axis(long n_outer, int n, long n_inner, int bc, int sign,
+                    const double *in, double *out, int nthreads);
+/* the eigenvalue of mode m = 0..n-1 of the second difference with spacing d under bc (R6) */
+int oracle_eigenvalues(int n, double d, int bc, double *lam_out);
+
+int oracle_divergence_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                         const double *u, const double *v, const double *w, double *div_out, int nthreads);
+int oracle_laplacian_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                        const double *p, double *lap_out, int nthreads);
+/* L p = rhs with the given conditions; the zero-mean gauge (R5) applies when no direction is Dirichlet, otherwise L is
+ * non-singular and nothing is removed.  Non-periodic z: Thomas with first / last diagonal -1/dz^2 + lam (Neumann) or
+ * -3/dz^2 + lam (Dirichlet). */
+int oracle_poisson_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                      const double *rhs, double *p_out, double *imag_residue_out, int nthreads);
+/* rhs / correction / whole step with walls along any direction (no Dirichlet); dt_ratio as in the _vdt calls */
+int oracle_rhs_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                  double rho1, double rho2, double dt, double dt_ratio,
+                  const double *u, const double *v, const double *w, const double *phi,
+                  const double *p, const double *p_old, double *rhs_out, int nthreads);
+int oracle_correction_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                         double rho1, double rho2, double dt,
+                         double *u, double *v, double *w, const double *phi,
+                         const double *p, const double *p_old, const double *p_new, int nthreads);
+int oracle_projection_step_bc(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y, int bc_z,
+                              double rho1, double rho2, double dt, double dt_ratio,
+                              double *u, double *v, double *w, const double *phi,
+                              double *p, const double *p_old, double *rhs_out, int nthreads);
 
 /* number of OpenMP threads a call with this nthreads argument would use */
 int oracle_threads(int nthreads);

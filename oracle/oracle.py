@@ -11,6 +11,7 @@ from .build import build as _build
 
 BC_Z_PERIODIC = 0
 BC_Z_WALL = 1
+BC_PERIODIC, BC_NEUMANN, BC_DIRICHLET = 0, 1, 2
 
 _lib = ctypes.CDLL(_build())
 _dp = ctypes.POINTER(ctypes.c_double)
@@ -28,6 +29,18 @@ _lib.oracle_correction.restype = _ci
 _lib.oracle_dft_axis.argtypes = [_cl, _ci, _cl, _ci, _dp, _dp, _dp, _dp, _ci]
 _lib.oracle_divergence.argtypes = _GRID + [_dp] * 4 + [_ci]
 _lib.oracle_laplacian.argtypes = _GRID + [_dp] * 2 + [_ci]
+_GRID3 = [_ci, _ci, _ci, _cd, _cd, _cd, _ci, _ci, _ci]
+_lib.oracle_r2r_axis.argtypes = [_cl, _ci, _cl, _ci, _ci, _dp, _dp, _ci]
+_lib.oracle_eigenvalues.argtypes = [_ci, _cd, _ci, _dp]
+_lib.oracle_divergence_bc.argtypes = _GRID3 + [_dp] * 4 + [_ci]
+_lib.oracle_laplacian_bc.argtypes = _GRID3 + [_dp] * 2 + [_ci]
+_lib.oracle_poisson_bc.argtypes = _GRID3 + [_dp, _dp, _dp, _ci]
+_lib.oracle_rhs_bc.argtypes = _GRID3 + [_cd, _cd, _cd, _cd] + [_dp] * 7 + [_ci]
+_lib.oracle_correction_bc.argtypes = _GRID3 + [_cd, _cd, _cd] + [_dp] * 7 + [_ci]
+_lib.oracle_projection_step_bc.argtypes = _GRID3 + [_cd, _cd, _cd, _cd] + [_dp] * 7 + [_ci]
+for _f in ("oracle_r2r_axis", "oracle_eigenvalues", "oracle_divergence_bc", "oracle_laplacian_bc", "oracle_poisson_bc",
+           "oracle_rhs_bc", "oracle_correction_bc", "oracle_projection_step_bc"):
+    getattr(_lib, _f).restype = _ci
 _lib.oracle_threads.argtypes = [_ci]
 for _f in ("oracle_rhs_vdt", "oracle_projection_step_vdt", "oracle_rhs", "oracle_poisson", "oracle_projection_step", "oracle_projection_step_paper",
            "oracle_dft_axis", "oracle_divergence", "oracle_laplacian", "oracle_threads"):
@@ -49,6 +62,13 @@ def _grid(shape, box, bc_z):
     nz, ny, nx = shape
     lx, ly, lz = box
     return [nx, ny, nz, float(lx), float(ly), float(lz), int(bc_z)]
+
+
+def _grid3(shape, box, bc):
+    """bc = (bc_x, bc_y, bc_z)"""
+    nz, ny, nx = shape
+    lx, ly, lz = box
+    return [nx, ny, nz, float(lx), float(ly), float(lz), int(bc[0]), int(bc[1]), int(bc[2])]
 
 
 def _check(rc, name):
@@ -150,3 +170,76 @@ def laplacian(p, box, bc_z, nthreads=0):
     out = np.empty_like(p)
     _check(_lib.oracle_laplacian(*_grid(p.shape, box, bc_z), _p(p), _p(out), nthreads), "oracle_laplacian")
     return out
+
+
+# ---------------------------------------------------------------- non-periodic x / y (bc = (bc_x, bc_y, bc_z))
+
+def r2r_axis(x, axis, bc, sign, nthreads=0):
+    """naive cosine (bc = 1) / sine (bc = 2) eigen-expansion of a real array along one axis; sign = -1 analysis
+    (normalised coefficients), +1 synthesis"""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    n = x.shape[axis]
+    n_outer = int(np.prod(x.shape[:axis], dtype=np.int64))
+    n_inner = int(np.prod(x.shape[axis + 1:], dtype=np.int64))
+    out = np.empty_like(x)
+    _check(_lib.oracle_r2r_axis(n_outer, n, n_inner, int(bc), int(sign), _p(x), _p(out), nthreads), "oracle_r2r_axis")
+    return out
+
+
+def eigenvalues(n, d, bc):
+    out = np.empty(n)
+    _check(_lib.oracle_eigenvalues(int(n), float(d), int(bc), _p(out)), "oracle_eigenvalues")
+    return out
+
+
+def divergence_bc(u, v, w, box, bc, nthreads=0):
+    u = _field(u)
+    v, w = _field(v, u.shape), _field(w, u.shape)
+    out = np.empty_like(u)
+    _check(_lib.oracle_divergence_bc(*_grid3(u.shape, box, bc), _p(u), _p(v), _p(w), _p(out), nthreads), "oracle_divergence_bc")
+    return out
+
+
+def laplacian_bc(p, box, bc, nthreads=0):
+    p = _field(p)
+    out = np.empty_like(p)
+    _check(_lib.oracle_laplacian_bc(*_grid3(p.shape, box, bc), _p(p), _p(out), nthreads), "oracle_laplacian_bc")
+    return out
+
+
+def poisson_bc(rhs_field, box, bc, nthreads=0, return_imag_residue=False):
+    r = _field(rhs_field)
+    out = np.empty_like(r)
+    res = ctypes.c_double(0.0)
+    _check(_lib.oracle_poisson_bc(*_grid3(r.shape, box, bc), _p(r), _p(out), ctypes.byref(res), nthreads), "oracle_poisson_bc")
+    return (out, res.value) if return_imag_residue else out
+
+
+def rhs_bc(u, v, w, phi, p, p_old, box, bc, rho1, rho2, dt, nthreads=0, dt_ratio=1.0):
+    u = _field(u)
+    f = [_field(a, u.shape) for a in (v, w, phi, p, p_old)]
+    out = np.empty_like(u)
+    _check(_lib.oracle_rhs_bc(*_grid3(u.shape, box, bc), rho1, rho2, dt, float(dt_ratio), _p(u), *[_p(a) for a in f],
+                              _p(out), nthreads), "oracle_rhs_bc")
+    return out
+
+
+def correction_bc(u, v, w, phi, p, p_old, p_new, box, bc, rho1, rho2, dt, nthreads=0):
+    u = _field(u).copy()
+    v, w = (_field(a, u.shape).copy() for a in (v, w))
+    phi, p, p_old, p_new = (_field(a, u.shape) for a in (phi, p, p_old, p_new))
+    _check(_lib.oracle_correction_bc(*_grid3(u.shape, box, bc), rho1, rho2, dt, _p(u), _p(v), _p(w), _p(phi),
+                                     _p(p), _p(p_old), _p(p_new), nthreads), "oracle_correction_bc")
+    return u, v, w
+
+
+def projection_step_bc(u, v, w, phi, p, p_old, box, bc, rho1, rho2, dt, nthreads=0, return_rhs=False, dt_ratio=1.0):
+    """the step with walls along any direction: bc = (bc_x, bc_y, bc_z), each PERIODIC or NEUMANN"""
+    u = _field(u).copy()
+    v, w, p = (_field(a, u.shape).copy() for a in (v, w, p))
+    phi, p_old = _field(phi, u.shape), _field(p_old, u.shape)
+    r = np.empty_like(u) if return_rhs else None
+    _check(_lib.oracle_projection_step_bc(*_grid3(u.shape, box, bc), rho1, rho2, dt, float(dt_ratio), _p(u), _p(v), _p(w),
+                                          _p(phi), _p(p), _p(p_old), _p(r) if return_rhs else None, nthreads),
+           "oracle_projection_step_bc")
+    return (u, v, w, p, r) if return_rhs else (u, v, w, p)
