@@ -7,6 +7,7 @@ A "step" is one pass of the whole hot path (splitting RHS -> Poisson solve -> co
 batch of synthetic input.  Workloads (BASELINE.json `metric` names both):
   cfg4  512^3 triply periodic, box (2 pi)^3, drops at 5 % volume fraction, rho2/rho1 = 50   [primary line]
   cfg5  1024 x 1024 x 512 wall-bounded, box 4 x 4 x 1, two-layer, rho2/rho1 = 1000          [under "also"]
+  cavity 512 x 512 x 256 closed box, walls in x, y, z (cosine expansions; NEXT-2)           [under "also"]
 N > 1 (torchrun): N independent replicas, one per GPU, no data-path collective ("replicas only").
 Prints ONE JSON line on rank 0.  --impl reference times the CPU oracle (tests' ground truth) on the same workload
 (one or two steps of the full 512^3 box); it is a deliberately slow baseline, not a target.
@@ -28,6 +29,8 @@ UNIT = "Mpts/s"
 WORKLOAD_DESC = {
     "cfg4": "cfg4: 512^3 triply periodic, box (2pi)^3, drops R=16 cells at 5% volume, rho2/rho1=50, dt=1e-3",
     "cfg5": "cfg5: 1024x1024x512 wall-bounded (Neumann p, Thomas in z), box 4x4x1, two-layer, rho2/rho1=1000, dt=1e-3",
+    "cavity": "cavity: 512x512x256 closed box, walls (Neumann p, no-slip) in x, y and z: cosine expansions in x, y + Thomas in z "
+              "(PAPER.md:287 shape, extruded; SURVEY sec. 8(f) NEXT-2), two-layer, rho2/rho1=5, dt=1e-3",
     "cfg2": "cfg2: 128^3 triply periodic emulsion-shaped (small case)",
     "cfg3": "cfg3: 256x256x128 wall-bounded two-layer (small case)",
 }
@@ -39,6 +42,8 @@ def make_workload(name, ratio=None):
         return wl.config4(512, 50.0 if ratio is None else ratio)
     if name == "cfg5":
         return wl.config5()
+    if name == "cavity":
+        return wl.cavity(512, 512, 256, 5.0)
     if name == "cfg2":
         return wl.config2()
     if name == "cfg3":
@@ -127,7 +132,7 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     t0 = time.time()
     W = make_workload(name, ratio)
     gen_s = time.time() - t0
-    plan = fl.Plan(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2)
+    plan = fl.Plan(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2, bc_x=W.bc_x, bc_y=W.bc_y)
     for kv in (args.opt or []):                       # experiments only: plan tuning knobs
         k_, v_ = kv.split("=")
         plan.set_option(k_, int(v_))
@@ -198,6 +203,7 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms / args.steps, 4),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOAD_DESC[name], "grid": [W.nx, W.ny, W.nz], "bc_z": "wall" if W.bc_z else "periodic",
+                   "bc_xyz": ["periodic" if b == 0 else "wall" for b in W.bc],
                    "rho2_over_rho1": W.rho2 / W.rho1, "parallelism": f"replicas x{world} (no data-path collective)",
                    "l2": "inputs larger than L2 (6 fields of %.1f GiB each); steps run back to back in place; per-kernel event "
                          "recording off in the timed region" % (W.npts * 8 / 2**30),
@@ -370,6 +376,7 @@ def run_reference(args):
            "warmup": n_warm, "ms_per_step": round(secs / len(samples) * 1e3, 1), "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": WORKLOAD_DESC[name], "grid": [W.nx, W.ny, W.nz], "bc_z": "wall" if W.bc_z else "periodic",
+                   "bc_xyz": ["periodic" if b == 0 else "wall" for b in W.bc],
                       "rho2_over_rho1": W.rho2 / W.rho1, "sample": samples[0]["sample"],
                       "steps_note": "bounded to %d step(s) of the full box (requested %d)" % (len(samples), args.steps)},
            "cpu_baseline": dict(samples[0], value=val),
@@ -384,7 +391,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workloads", default="cfg4,cfg5")
+    ap.add_argument("--workloads", default="cfg4,cfg5,cavity")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-all", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -46,8 +46,19 @@ extern "C" {
 typedef struct flutas_plan flutas_plan;
 
 enum { FLUTAS_BC_Z_PERIODIC = 0, FLUTAS_BC_Z_WALL = 1 };
-/* boundary conditions (the same values, for any direction) */
-enum { FLUTAS_BC_PERIODIC = 0, FLUTAS_BC_NEUMANN = 1 };
+/* boundary conditions per direction (flutas_plan_create_ex): the homogeneous pressure conditions the FFT-based solver
+ * covers.
+ *   PERIODIC
+ *   NEUMANN    a wall at both ends: u_n = 0, dp/dn = 0 on the boundary faces (what FLUTAS_BC_Z_WALL is along z).  The last
+ *              stored face of the direction (u[nx-1,.,.], v[.,ny-1,.], w[.,.,nz-1]) is the wall face: it MUST be 0 on entry
+ *              (not checked) and is left unchanged; the first wall face is not stored.  Closed cavity:
+ *              NEUMANN in all three directions.
+ *   DIRICHLET  p = 0 ON both boundary faces (ghost value = -interior value).  flutas_poisson_solve only: the step would
+ *              need the boundary-normal velocity on both boundary faces and a line of n cells stores n faces.
+ * Expansions: cosine (NEUMANN) / sine (DIRICHLET) series computed with the real-to-complex FFT machinery and pre- / post-
+ * processing fused into the transform kernels; eigenvalues -2 (1 - cos(pi m / n)) / d^2 and
+ * -2 (1 - cos(pi (m+1) / n)) / d^2.  With any DIRICHLET direction the operator is non-singular and no mean is removed. */
+enum { FLUTAS_BC_PERIODIC = 0, FLUTAS_BC_NEUMANN = 1, FLUTAS_BC_DIRICHLET = 2 };
 
 /* flags of flutas_plan_create_ex */
 enum { FLUTAS_PLAN_CALLER_WORKSPACE = 1 };   /* do not allocate the workspace: flutas_plan_set_workspace supplies it */
@@ -75,8 +86,11 @@ enum {
 flutas_plan *flutas_plan_create(int nx, int ny, int nz, double lx, double ly, double lz,
                                 int bc_z, double rho1, double rho2);
 
-/* flutas_plan_create with boundary conditions along x and y and flags (same problem).
- *   bc_x, bc_y: FLUTAS_BC_PERIODIC (what flutas_plan_create passes); see "boundary conditions" above.
+/* flutas_plan_create with boundary conditions per direction and flags (same problem;
+ * "all the possible homogeneous pressure boundary conditions").
+ *   bc_x, bc_y, bc_z: FLUTAS_BC_PERIODIC / _NEUMANN / _DIRICHLET (flutas_plan_create passes PERIODIC, PERIODIC, bc_z).
+ *   sizes, beyond those of flutas_plan_create: non-periodic y: ny <= 1024; non-periodic x: 16 <= nx <= 1024, ny <= 1024,
+ *          z not periodic and nz <= 444 (put a periodic direction first); otherwise FLUTAS_ERR_UNSUPPORTED_SIZE.
  *   FLUTAS_PLAN_CALLER_WORKSPACE: the plan allocates its small tables only; before the first step the caller hands it
  *   a device buffer with flutas_plan_set_workspace (e.g. one torch tensor, so that the framework's allocator
  *   accounts for every large byte).  A step on a plan without a workspace fails with FLUTAS_ERR_INVALID_ARG. */

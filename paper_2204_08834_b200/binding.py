@@ -12,6 +12,7 @@ BC_Z_PERIODIC = 0
 BC_Z_WALL = 1
 BC_PERIODIC = 0
 BC_NEUMANN = 1
+BC_DIRICHLET = 2
 PLAN_CALLER_WORKSPACE = 1
 
 _vp, _ci, _cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double

@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "kernels_r2r.cuh"
 #include "kernels_rhs.cuh"
 #include "kernels_thomas.cuh"
 #include "kernels_tma.cuh"
@@ -51,7 +52,14 @@ enum KernelId { K_RHS = 0, K_FFTX, K_FFTY, K_Z, K_ZS, K_IFFTY, K_IFFTX, K_CORR, 
 static const int kMaxPendingSteps = 256;
 
 struct flutas_plan {
-    int nx, ny, nz, bc_z;
+    int nx, ny, nz, bc_z;        // bc_z: FLUTAS_BC_Z_PERIODIC (transform along z) or FLUTAS_BC_Z_WALL (elimination along z)
+    int bc[3];                   // the conditions as given, per direction: FLUTAS_BC_PERIODIC / _NEUMANN / _DIRICHLET
+    int xsplit;                  // x is not periodic: columns of the spectrum hold two real modes (kernels_r2r.cuh)
+    int y_r2r;                   // y expansion: 0 complex FFT, 1 half-complex (periodic y under xsplit), 2 cosine, 3 sine
+    int has_null;                // no Dirichlet direction: the (0,0,0) mode is singular, zero-mean gauge (R5)
+    double end_coef_z;           // first / last diagonal of the elimination along z: -end_coef/dz^2 + lam (1 Neumann, 3 Dirichlet)
+    double2 *wq_x, *wq_y;        // e^{-i pi k / (2n)}, k = 0 .. n/2, of the cosine / sine expansions
+    double *lam_x2;              // eigenvalue along x per (column, component): 2 * pitch entries
     double lx, ly, lz, rho1, rho2;
     GridParams grid;
     int n2, nxh, pitch;          // nx/2, nx/2+1, padded row length of the half-spectrum (multiple of 8)
@@ -128,23 +136,43 @@ static double host_lambda(int m, int n, double d) {
     return (double)(-2.0L * (1.0L - cosl(two_pi * (long double)m / (long double)n))) / (d * d);
 }
 
+// eigenvalue of mode index k of the cosine (Neumann) / sine (Dirichlet) expansion AS THE KERNELS INDEX IT: the cosine
+// transform index k is mode k; the sine expansion is computed as a cosine transform of the sign-flipped line read
+// backwards, so transform index k is sine mode n-1-k, frequency n-k:  lambda = -2 (1 - cos(pi f / n)) / d^2
+static double host_lambda_r2r(int k, int n, double d, int bc) {
+    const long double pi = 3.141592653589793238462643383279502884L;
+    const int f = bc == FLUTAS_BC_NEUMANN ? k : n - k;
+    return (double)(-2.0L * (1.0L - cosl(pi * (long double)f / (long double)n))) / (d * d);
+}
+static void host_wq(int n, std::vector<double2> &t) {
+    t.resize(n / 2 + 1);
+    const long double pi = 3.141592653589793238462643383279502884L;
+    for (int k = 0; k <= n / 2; ++k) {
+        const long double a = -pi * (long double)k / (long double)(2 * n);
+        t[k] = make_double2((double)cosl(a), (double)sinl(a));
+    }
+}
+
 // eigenvalues along y in the storage order of the transform in use (the 16 x 8 x 8 kernel has its own digit order)
 static int upload_lam_y(flutas_plan *pl) {
     std::vector<double> lam(pl->ny);
     const double dy = pl->ly / pl->ny;
-    for (int pos = 0; pos < pl->ny; ++pos)
-        lam[pos] = host_lambda(pl->y16 ? y1024_freq_of_pos(pos) : host_freq_of_pos(pl->ny, pos), pl->ny, dy);
+    for (int pos = 0; pos < pl->ny; ++pos) {
+        const int k = pl->y16 ? y1024_freq_of_pos(pos) : host_freq_of_pos(pl->ny, pos);
+        lam[pos] = pl->bc[1] == FLUTAS_BC_PERIODIC ? host_lambda(k, pl->ny, dy) : host_lambda_r2r(k, pl->ny, dy, pl->bc[1]);
+    }
     CUDA_TRY(cudaMemcpy(pl->lam_y, lam.data(), sizeof(double) * pl->ny, cudaMemcpyHostToDevice));
     return FLUTAS_OK;
 }
 
 // elimination coefficients of the one-pass wall solve (they depend on lam_x + lam_y in storage order)
+static int thomas_cw(const flutas_plan *pl) { return pl->xsplit ? 16 : ThomasGeom::C; }
 static int build_thomas_table(flutas_plan *pl) {
-    const int n_tiles_x = (pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C;
-    const long long ncol = (long long)n_tiles_x * pl->ny * ThomasGeom::C;
+    const int n_tiles_x = (pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C, cw = thomas_cw(pl);
+    const long long ncol = (long long)n_tiles_x * pl->ny * cw;
     const double inv_dz = 1.0 / (pl->lz / pl->nz);
-    thomas_table_kernel<<<(unsigned)((ncol + 127) / 128), 128>>>(pl->ttab, n_tiles_x, pl->ny, pl->nz, pl->nxh, pl->lam_x,
-                                                               pl->lam_y, inv_dz * inv_dz);
+    thomas_table_kernel<<<(unsigned)((ncol + 127) / 128), 128>>>(pl->ttab, n_tiles_x, pl->ny, pl->nz, pl->nxh, cw, pl->lam_x2,
+                                                               pl->lam_y, inv_dz * inv_dz, pl->end_coef_z, pl->has_null);
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaDeviceSynchronize());
     return FLUTAS_OK;
@@ -162,7 +190,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-static int make_spectrum_map(flutas_plan *pl, CUtensorMap *map, int cols, int line_dim, int n) {
+static int make_spectrum_map(flutas_plan *pl, CUtensorMap *map, int cols, int line_dim, int n, int box_rows = 0) {
     static EncodeTiledFn encode = nullptr;
     if (!encode) {
         void *fn = nullptr;
@@ -171,7 +199,7 @@ static int make_spectrum_map(flutas_plan *pl, CUtensorMap *map, int cols, int li
         if (!fn || q != cudaDriverEntryPointSuccess) return fail(FLUTAS_ERR_CUDA, "cuTensorMapEncodeTiled is not available");
         encode = (EncodeTiledFn)fn;
     }
-    const cuuint32_t rows = (cuuint32_t)(n < 256 ? n : 256);
+    const cuuint32_t rows = (cuuint32_t)(box_rows ? box_rows : (n < 256 ? n : 256));
     const cuuint64_t gdim[3] = {(cuuint64_t)2 * pl->nxh, (cuuint64_t)pl->ny, (cuuint64_t)pl->nz};
     const cuuint64_t gstride[2] = {(cuuint64_t)pl->pitch * 16, (cuuint64_t)pl->plane * 16};
     const cuuint32_t box[3] = {(cuuint32_t)(2 * cols), line_dim == 1 ? rows : 1u, line_dim == 2 ? rows : 1u};
@@ -189,17 +217,26 @@ static int plan_make_maps(flutas_plan *pl) {
     if (pl->bc_z == FLUTAS_BC_Z_PERIODIC) {
         if (int rc = make_spectrum_map(pl, &pl->map_z, pl->z_cols, 2, pl->nz)) return rc;
     } else if (pl->thomas_variant == 1) {
-        if (int rc = make_spectrum_map(pl, &pl->map_z, ThomasGeom::C, 2, pl->nz)) return rc;
+        if (int rc = make_spectrum_map(pl, &pl->map_z, ThomasGeom::C, 2, pl->nz, ThomasGeom::box_rows(pl->nz))) return rc;
     }
     return FLUTAS_OK;
 }
 
 // ---- sizes: everything that follows from (nx, ny, nz, bc_z) alone, no device needed
 static bool sizes_supported(int nx, int ny, int nz, int bc_x, int bc_y, int bc_z) {
-    if (bc_x != FLUTAS_BC_PERIODIC || bc_y != FLUTAS_BC_PERIODIC) return false;
-    if (bc_z != FLUTAS_BC_Z_PERIODIC && bc_z != FLUTAS_BC_Z_WALL) return false;
+    const auto bc_ok = [](int b) { return b == FLUTAS_BC_PERIODIC || b == FLUTAS_BC_NEUMANN || b == FLUTAS_BC_DIRICHLET; };
+    if (!bc_ok(bc_x) || !bc_ok(bc_y) || !bc_ok(bc_z)) return false;
     if (!is_pow2(nx) || nx < 8 || nx > 2048 || !is_pow2(ny) || ny < 8 || ny > 2048) return false;
-    if (bc_z == FLUTAS_BC_Z_WALL) return nz >= 2 && nz <= 4096;
+    const bool xsplit = bc_x != FLUTAS_BC_PERIODIC;
+    if (xsplit) {
+        // cosine / sine expansion along x: staged kernels for nx = 16 .. 1024; the z stage must then be the one-pass
+        // elimination with per-component coefficients (no transform along z; the column tile and its coefficient
+        // table must fit in shared memory: nz <= 444)
+        if (nx < 16 || nx > 1024) return false;
+        if (bc_z == FLUTAS_BC_PERIODIC || nz < 2 || ThomasGeom::smem_bytes(nz, 16) > 227 * 1024) return false;   // nz <= 444
+    }
+    if ((xsplit || bc_y != FLUTAS_BC_PERIODIC) && ny > 1024) return false;   // the one-butterfly-per-thread y kernel
+    if (bc_z != FLUTAS_BC_PERIODIC) return nz >= 2 && nz <= 4096;
     return is_pow2(nz) && nz >= 8 && nz <= 2048;
 }
 
@@ -220,9 +257,9 @@ static WsLayout plan_layout(const flutas_plan *pl) {
     w.wp = o; o += align_up(fb);
     w.zaux = o;
     if (pl->bc_z == FLUTAS_BC_Z_WALL) {
-        if (ThomasGeom::smem_bytes(pl->nz) <= 227 * 1024) {   // coefficient table of the one-pass solve
+        if (ThomasGeom::smem_bytes(pl->nz, thomas_cw(pl)) <= 227 * 1024) {   // coefficient table of the one-pass solve
             const int n_tiles_x = (pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C;
-            o += align_up(sizeof(double) * ThomasGeom::tab_doubles(pl->nz) * (size_t)n_tiles_x * pl->ny);
+            o += align_up(sizeof(double) * ThomasGeom::tab_doubles(pl->nz, thomas_cw(pl)) * (size_t)n_tiles_x * pl->ny);
         } else {                                              // c' of the two sweeps
             o += align_up(sb / 2);
         }
@@ -234,7 +271,8 @@ static WsLayout plan_layout(const flutas_plan *pl) {
 static void plan_geometry(flutas_plan *pl) {
     const int nx = pl->nx, ny = pl->ny, nz = pl->nz;
     pl->n2 = nx / 2;
-    pl->nxh = nx / 2 + 1;
+    pl->xsplit = pl->bc[0] != FLUTAS_BC_PERIODIC;
+    pl->nxh = pl->xsplit ? nx / 2 : nx / 2 + 1;      // valid columns: nx/2 split columns, or kx = 0 .. nx/2
     pl->pitch = nx / 2 + 8;
     pl->npts = (long long)nx * ny * nz;
     // One unused row per plane, so that the stride of a line along z is an odd multiple of the row size instead of
@@ -261,7 +299,7 @@ static int plan_attach_workspace(flutas_plan *pl, void *base, bool owned) {
     // padding columns / the pad row of the spectrum are read (never used) by the strided kernels: keep them finite
     CUDA_TRY(cudaMemset(pl->spec, 0, sizeof(double2) * (size_t)pl->nspec));
     if (pl->bc_z == FLUTAS_BC_Z_WALL) {
-        if (ThomasGeom::smem_bytes(pl->nz) <= 227 * 1024) {
+        if (ThomasGeom::smem_bytes(pl->nz, thomas_cw(pl)) <= 227 * 1024) {
             pl->ttab = (double *)(b + w.zaux);
             if (int rc = build_thomas_table(pl)) return rc;
         } else if (!pl->cp_owned) {
@@ -285,9 +323,13 @@ static int plan_build(flutas_plan *pl, unsigned flags) {
     const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
     const double dx = pl->lx / nx, dy = pl->ly / ny, dz = pl->lz / nz;
     const bool same_rho = pl->rho1 == pl->rho2;    // (1 - rho0/rho_f) is then exactly 0 (flux_coef)
-    pl->grid = GridParams{nx, ny, nz, wall ? 1 : 0, 1.0 / dx, 1.0 / dy, 1.0 / dz, pl->rho1, pl->rho2,
-                          pl->rho1 < pl->rho2 ? pl->rho1 : pl->rho2, 2.0, 1.0, same_rho ? 0.0 : 1.0};
+    pl->grid = GridParams{nx, ny, nz, pl->bc[2] == FLUTAS_BC_NEUMANN ? 1 : 0, 1.0 / dx, 1.0 / dy, 1.0 / dz, pl->rho1, pl->rho2,
+                          pl->rho1 < pl->rho2 ? pl->rho1 : pl->rho2, 2.0, 1.0, same_rho ? 0.0 : 1.0,
+                          pl->bc[0] == FLUTAS_BC_NEUMANN ? 1 : 0, pl->bc[1] == FLUTAS_BC_NEUMANN ? 1 : 0};
     plan_geometry(pl);
+    pl->has_null = pl->bc[0] != FLUTAS_BC_DIRICHLET && pl->bc[1] != FLUTAS_BC_DIRICHLET && pl->bc[2] != FLUTAS_BC_DIRICHLET;
+    pl->end_coef_z = pl->bc[2] == FLUTAS_BC_DIRICHLET ? 3.0 : 1.0;
+    pl->y_r2r = pl->bc[1] == FLUTAS_BC_NEUMANN ? 2 : (pl->bc[1] == FLUTAS_BC_DIRICHLET ? 3 : (pl->xsplit ? 1 : 0));
 
     size_t tb = 0;   // table bytes (not part of the workspace)
     std::vector<double2> t;
@@ -302,7 +344,26 @@ static int plan_build(flutas_plan *pl, unsigned flags) {
     std::vector<double> lam(pl->pitch, 1.0);
     for (int k = 0; k <= pl->n2; ++k) lam[k] = host_lambda(k, nx, dx);   // x columns are stored in natural order
     if (int rc = upload(&pl->lam_x, lam, &tb)) return rc;
-    pl->y16 = ny == Y16Geom::N ? 1 : 0;
+    {   // the same per (column, component).  Split columns (kernels_r2r.cuh): column k = (mode k, mode nx - k), column 0 = (0, nx/2)
+        std::vector<double> lam2(2 * (size_t)pl->pitch, 1.0);
+        for (int k = 0; k < pl->nxh; ++k) {
+            if (!pl->xsplit) lam2[2 * k] = lam2[2 * k + 1] = lam[k];
+            else {
+                lam2[2 * k] = host_lambda_r2r(k, nx, dx, pl->bc[0]);
+                lam2[2 * k + 1] = host_lambda_r2r(k == 0 ? nx / 2 : nx - k, nx, dx, pl->bc[0]);
+            }
+        }
+        if (int rc = upload(&pl->lam_x2, lam2, &tb)) return rc;
+    }
+    if (pl->xsplit) {
+        host_wq(nx, t);
+        if (int rc = upload(&pl->wq_x, t, &tb)) return rc;
+    }
+    if (pl->y_r2r >= 2) {
+        host_wq(ny, t);
+        if (int rc = upload(&pl->wq_y, t, &tb)) return rc;
+    }
+    pl->y16 = (ny == Y16Geom::N && pl->y_r2r == 0) ? 1 : 0;
     CUDA_TRY(cudaMalloc((void **)&pl->lam_y, sizeof(double) * ny));
     if (int rc = upload_lam_y(pl)) return rc;
     if (!wall) {
@@ -314,7 +375,7 @@ static int plan_build(flutas_plan *pl, unsigned flags) {
         // the (0,0) column: lam = 0; the elimination coefficients do not depend on the data (same recurrence, same
         // IEEE divisions as a per-step evaluation would do)
         std::vector<double> sc(2 * (size_t)nz, 0.0);
-        const double a = (1.0 / dz) * (1.0 / dz), b_end = -a, b_in = -2.0 * a;   // as GridParams::inv_dz squared
+        const double a = (1.0 / dz) * (1.0 / dz), b_end = -a, b_in = -2.0 * a;   // as GridParams::inv_dz squared (Neumann: singular)
         double inv = 1.0 / b_end, cpv = a * inv;
         sc[0] = inv; sc[1] = cpv;
         for (int k = 1; k <= nz - 2; ++k) {
@@ -324,7 +385,7 @@ static int plan_build(flutas_plan *pl, unsigned flags) {
         }
         sc[2 * (size_t)nz - 1] = a;
         if (int rc = upload(&pl->sing_coef, sc, &tb)) return rc;
-        pl->thomas_variant = ThomasGeom::smem_bytes(nz) <= 227 * 1024 ? 1 : 0;
+        pl->thomas_variant = ThomasGeom::smem_bytes(nz, thomas_cw(pl)) <= 227 * 1024 ? 1 : 0;
         pl->thomas_warps = 2;
     }
 
@@ -333,7 +394,7 @@ static int plan_build(flutas_plan *pl, unsigned flags) {
     pl->launch_ids[n++] = K_FFTX;
     pl->launch_ids[n++] = K_FFTY;
     pl->launch_ids[n++] = K_Z;
-    if (wall) pl->launch_ids[n++] = K_ZS;
+    if (wall && pl->has_null) pl->launch_ids[n++] = K_ZS;
     pl->launch_ids[n++] = K_IFFTY;
     pl->launch_ids[n++] = K_IFFTX;
     pl->launch_ids[n++] = K_CORR;
@@ -353,10 +414,11 @@ static int plan_build(flutas_plan *pl, unsigned flags) {
 
 extern "C" flutas_plan *flutas_plan_create_ex(int nx, int ny, int nz, double lx, double ly, double lz, int bc_x, int bc_y,
                                               int bc_z, double rho1, double rho2, unsigned flags) {
-    if (bc_z != FLUTAS_BC_Z_PERIODIC && bc_z != FLUTAS_BC_Z_WALL) {
-        fail(FLUTAS_ERR_INVALID_ARG, "bc_z must be FLUTAS_BC_Z_PERIODIC or FLUTAS_BC_Z_WALL");
-        return nullptr;
-    }
+    for (int b : {bc_x, bc_y, bc_z})
+        if (b != FLUTAS_BC_PERIODIC && b != FLUTAS_BC_NEUMANN && b != FLUTAS_BC_DIRICHLET) {
+            fail(FLUTAS_ERR_INVALID_ARG, "boundary conditions must be FLUTAS_BC_PERIODIC, FLUTAS_BC_NEUMANN (wall) or FLUTAS_BC_DIRICHLET");
+            return nullptr;
+        }
     if (flags & ~(unsigned)FLUTAS_PLAN_CALLER_WORKSPACE) {
         fail(FLUTAS_ERR_INVALID_ARG, "unknown flag bits 0x%x", flags);
         return nullptr;
@@ -371,8 +433,9 @@ extern "C" flutas_plan *flutas_plan_create_ex(int nx, int ny, int nz, double lx,
     }
     if (!sizes_supported(nx, ny, nz, bc_x, bc_y, bc_z)) {
         fail(FLUTAS_ERR_UNSUPPORTED_SIZE,
-             "unsupported grid %d x %d x %d: nx, ny powers of two in [8,2048]; nz a power of two in [8,2048] (periodic) "
-             "or any value in [2,4096] (wall); bc_x, bc_y periodic", nx, ny, nz);
+             "unsupported grid %d x %d x %d with conditions (%d, %d, %d): nx, ny powers of two in [8,2048]; nz a power of two "
+             "in [8,2048] (periodic z) or any value in [2,4096]; non-periodic y: ny <= 1024; non-periodic x: nx in [16,1024], "
+             "ny <= 1024, z not periodic and nz <= 444", nx, ny, nz, bc_x, bc_y, bc_z);
         return nullptr;
     }
     int ndev = 0;
@@ -387,7 +450,9 @@ extern "C" flutas_plan *flutas_plan_create_ex(int nx, int ny, int nz, double lx,
         return nullptr;
     }
     memset(pl, 0, sizeof(*pl));
-    pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->bc_z = bc_z;
+    pl->nx = nx; pl->ny = ny; pl->nz = nz;
+    pl->bc[0] = bc_x; pl->bc[1] = bc_y; pl->bc[2] = bc_z;
+    pl->bc_z = bc_z == FLUTAS_BC_PERIODIC ? FLUTAS_BC_Z_PERIODIC : FLUTAS_BC_Z_WALL;
     pl->lx = lx; pl->ly = ly; pl->lz = lz; pl->rho1 = rho1; pl->rho2 = rho2;
     if (plan_build(pl, flags) != FLUTAS_OK) {
         flutas_plan_destroy(pl);   // keeps g_err of the failure
@@ -405,7 +470,9 @@ extern "C" size_t flutas_workspace_bytes(int nx, int ny, int nz, int bc_x, int b
     if (!sizes_supported(nx, ny, nz, bc_x, bc_y, bc_z)) return 0;
     flutas_plan tmp;
     memset(&tmp, 0, sizeof(tmp));
-    tmp.nx = nx; tmp.ny = ny; tmp.nz = nz; tmp.bc_z = bc_z;
+    tmp.nx = nx; tmp.ny = ny; tmp.nz = nz;
+    tmp.bc[0] = bc_x; tmp.bc[1] = bc_y; tmp.bc[2] = bc_z;
+    tmp.bc_z = bc_z == FLUTAS_BC_PERIODIC ? FLUTAS_BC_Z_PERIODIC : FLUTAS_BC_Z_WALL;
     plan_geometry(&tmp);
     return tmp.bytes;
 }
@@ -431,7 +498,8 @@ extern "C" void flutas_plan_destroy(flutas_plan *pl) {
     if (!pl) return;
     cudaDeviceSynchronize();
     cudaFree(pl->tw_x); cudaFree(pl->tw_y); cudaFree(pl->tw_z);
-    cudaFree(pl->lam_x); cudaFree(pl->lam_y); cudaFree(pl->lam_z);
+    cudaFree(pl->lam_x); cudaFree(pl->lam_y); cudaFree(pl->lam_z); cudaFree(pl->lam_x2);
+    cudaFree(pl->wq_x); cudaFree(pl->wq_y);
     cudaFree(pl->sing_coef);
     if (pl->cp_owned) cudaFree(pl->cp);
     plan_detach_workspace(pl);
@@ -471,7 +539,7 @@ extern "C" double flutas_plan_kernel_bytes(const flutas_plan *pl, int idx) {
         case K_Z:
             if (pl->bc_z != FLUTAS_BC_Z_WALL) return 2 * s;
             if (pl->thomas_variant == 1)   // one pass + the coefficient table (one double per column and half the planes)
-                return 2 * s + 8.0 * ThomasGeom::tab_doubles(pl->nz) * ((pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C) * pl->ny;
+                return 2 * s + 8.0 * ThomasGeom::tab_doubles(pl->nz, thomas_cw(pl)) * ((pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C) * pl->ny;
             return 4 * s + 2 * (s / 2);    // two sweeps + c'
         case K_ZS: return 2.0 * 16.0 * pl->nz;
         case K_IFFTX: return s + f;                // read spectrum, write p
@@ -485,8 +553,8 @@ extern "C" const char *flutas_plan_kernel_symbol(const flutas_plan *pl, int idx)
     const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
     switch (pl->launch_ids[idx]) {
         case K_RHS: return rhs_takes_ranges(pl) ? "splitting_rhs_kernel3" : "splitting_rhs_kernel2";
-        case K_FFTX: return pl->nx == 8 ? "fft_x8_r2c_kernel" : (x_is_persistent(pl) ? "fft_x_r2c_tma_kernel" : "fft_x_r2c_kernel");
-        case K_IFFTX: return pl->nx == 8 ? "fft_x8_c2r_kernel" : (x_is_persistent(pl) ? "fft_x_c2r_tma_kernel" : "fft_x_c2r_kernel");
+        case K_FFTX: return pl->xsplit ? "fft_x_r2r_fwd_kernel" : pl->nx == 8 ? "fft_x8_r2c_kernel" : (x_is_persistent(pl) ? "fft_x_r2c_tma_kernel" : "fft_x_r2c_kernel");
+        case K_IFFTX: return pl->xsplit ? "fft_x_r2r_inv_kernel" : pl->nx == 8 ? "fft_x8_c2r_kernel" : (x_is_persistent(pl) ? "fft_x_c2r_tma_kernel" : "fft_x_c2r_kernel");
         case K_FFTY: case K_IFFTY:
             return pl->y16 ? "fft_y1024_kernel" : (pl->ny * pl->y_cols / 8 <= 512 ? "fft_tma1_kernel" : "fft_tma_kernel");
         case K_Z:
@@ -500,7 +568,8 @@ extern "C" const char *flutas_plan_kernel_symbol(const flutas_plan *pl, int idx)
 
 extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int value) {
     if (!pl || !name) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan or option name");
-    if (!strcmp(name, "thomas") && pl->bc_z == FLUTAS_BC_Z_WALL && (value == 0 || (value == 1 && ThomasGeom::smem_bytes(pl->nz) <= 227 * 1024))) {
+    if (!strcmp(name, "thomas") && pl->bc_z == FLUTAS_BC_Z_WALL && !(value == 0 && pl->xsplit) &&
+        (value == 0 || (value == 1 && ThomasGeom::smem_bytes(pl->nz, thomas_cw(pl)) <= 227 * 1024))) {
         if (value == 0 && !pl->cp) {   // the two-sweep kernel keeps c' in half a spectrum of its own
             CUDA_TRY(cudaMalloc((void **)&pl->cp, sizeof(double) * (size_t)pl->nspec));
             pl->cp_owned = true;
@@ -508,7 +577,7 @@ extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int val
         pl->thomas_variant = value;
         return pl->ws_base ? plan_make_maps(pl) : FLUTAS_OK;
     }
-    if (!strcmp(name, "y16") && (value == 0 || (value == 1 && pl->ny == Y16Geom::N))) {
+    if (!strcmp(name, "y16") && (value == 0 || (value == 1 && pl->ny == Y16Geom::N && pl->y_r2r == 0))) {
         CUDA_TRY(cudaDeviceSynchronize());
         pl->y16 = value;                        // the storage order along y changes with the kernel
         if (int rc = upload_lam_y(pl)) return rc;
@@ -556,7 +625,9 @@ static cudaError_t launch_tma_nc(const CUtensorMap &map, const TmaFftArgs &a, co
             return cudaGetLastError();
         }
     }
-    // lines of 2048 (1024 butterflies per tile): the generic kernel, several butterflies per thread
+    // lines of 2048 (1024 butterflies per tile): the generic kernel, several butterflies per thread (complex transforms only)
+    if constexpr (MODE == MODE_R2R_FWD || MODE == MODE_R2R_INV) return cudaErrorInvalidValue;
+    else {
     constexpr int NT = tma_nt(N, C), NBUF = tma_nbuf(N, C);
     const size_t smem = (size_t)NBUF * N * C * 16 + 128;
     auto kern = fft_tma_kernel<N, C, MODE, NT, NBUF>;
@@ -570,6 +641,7 @@ static cudaError_t launch_tma_nc(const CUtensorMap &map, const TmaFftArgs &a, co
     if (grid > ntiles) grid = ntiles;
     kern<<<(unsigned)grid, NT, smem, st>>>(map, a);
     return cudaGetLastError();
+    }
 }
 template <int N, int MODE>
 static cudaError_t launch_tma_n(int cols, const CUtensorMap &map, TmaFftArgs a, Tma1Args a1, cudaStream_t st,
@@ -589,6 +661,7 @@ static cudaError_t launch_tma(int n, int cols, const CUtensorMap &map, TmaFftArg
     a1.data = data; a1.row_stride = row_stride; a1.outer_stride = outer_stride;
     a1.n_outer = a.n_outer; a1.line_dim = a.line_dim; a1.nxh = a.nxh; a1.tw = a.tw;
     a1.lam_x = a.lam_x; a1.lam_outer = a.lam_outer; a1.lam_pos = a.lam_pos;
+    a1.wq = a.wq; a1.reorder = a.reorder; a1.neg = a.neg;
     switch (n) {
         case 8: return launch_tma_n<8, MODE>(cols, map, a, a1, st, num_sms);
         case 16: return launch_tma_n<16, MODE>(cols, map, a, a1, st, num_sms);
@@ -619,6 +692,27 @@ template <int N2> static cudaError_t launch_c2r_n(const flutas_plan *pl, double 
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
     kern<<<(unsigned)ntiles, NT, smem, st>>>(pl->spec, out + tile0 * 8 * 2 * N2, pl->tw_x, scale, SpecRows{pl->ny, pl->plane, tile0 * 8});
+    return cudaGetLastError();
+}
+// cosine / sine expansion along x (non-periodic x; staged kernels, nx = 16 .. 1024)
+template <int N2> static cudaError_t launch_r2r_fwd_n(const flutas_plan *pl, const double *rhs, cudaStream_t st, long long tile0, long long ntiles) {
+    constexpr int NT = clamp_nt(N2);
+    const size_t smem = sizeof(double2) * (size_t)N2 * 16;
+    auto kern = fft_x_r2r_fwd_kernel<N2, NT>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<(unsigned)ntiles, NT, smem, st>>>(rhs + tile0 * 8 * 2 * N2, pl->spec, pl->tw_x, pl->wq_x, pl->bc[0] == FLUTAS_BC_DIRICHLET ? 1 : 0,
+                                             SpecRows{pl->ny, pl->plane, tile0 * 8});
+    return cudaGetLastError();
+}
+template <int N2> static cudaError_t launch_r2r_inv_n(const flutas_plan *pl, double *out, double scale, cudaStream_t st, long long tile0, long long ntiles) {
+    constexpr int NT = clamp_nt(N2);
+    const size_t smem = sizeof(double2) * (size_t)N2 * 16;
+    auto kern = fft_x_r2r_inv_kernel<N2, NT>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<(unsigned)ntiles, NT, smem, st>>>(pl->spec, out + tile0 * 8 * 2 * N2, pl->tw_x, pl->wq_x, pl->bc[0] == FLUTAS_BC_DIRICHLET ? 1 : 0, scale,
+                                             SpecRows{pl->ny, pl->plane, tile0 * 8});
     return cudaGetLastError();
 }
 // persistent bulk-copy-fed x kernels (nx = 128 .. 1024)
@@ -655,6 +749,12 @@ template <int N2> static cudaError_t launch_c2r_tma_n(const flutas_plan *pl, dou
 // planes k0 .. k1 - 1 (a tile is 8 consecutive x-lines; ny is a multiple of 8)
 static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStream_t st, int k0, int k1) {
     const long long tile0 = (long long)k0 * pl->ny / 8, ntiles = (long long)(k1 - k0) * pl->ny / 8;
+    if (pl->xsplit)
+        switch (pl->n2) {
+#define X(n) case n: return launch_r2r_fwd_n<n>(pl, rhs, st, tile0, ntiles);
+            X(8) X(16) X(32) X(64) X(128) X(256) X(512)
+#undef X
+        }
     if (pl->nx == 8) {   // the degenerate length: one thread per line
         const long long nlines = ntiles * 8;
         fft_x8_r2c_kernel<<<(unsigned)((nlines + 127) / 128), 128, 0, st>>>(rhs + tile0 * 64, pl->spec, nlines, SpecRows{pl->ny, pl->plane, tile0 * 8});
@@ -675,6 +775,12 @@ static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStre
 }
 static cudaError_t launch_c2r(const flutas_plan *pl, double *out, double scale, cudaStream_t st, int k0, int k1) {
     const long long tile0 = (long long)k0 * pl->ny / 8, ntiles = (long long)(k1 - k0) * pl->ny / 8;
+    if (pl->xsplit)
+        switch (pl->n2) {
+#define X(n) case n: return launch_r2r_inv_n<n>(pl, out, scale, st, tile0, ntiles);
+            X(8) X(16) X(32) X(64) X(128) X(256) X(512)
+#undef X
+        }
     if (pl->nx == 8) {
         const long long nlines = ntiles * 8;
         fft_x8_c2r_kernel<<<(unsigned)((nlines + 127) / 128), 128, 0, st>>>(pl->spec, out + tile0 * 64, scale, nlines, SpecRows{pl->ny, pl->plane, tile0 * 8});
@@ -769,6 +875,14 @@ template <int MODE> static int enqueue_y(flutas_plan *pl, cudaStream_t st, int k
     ty.line_dim = 1;
     ty.nxh = pl->nxh;
     ty.tw = pl->tw_y;
+    if (pl->y_r2r) {   // real-linear expansion of both components of every column (kernels_r2r.cuh, kernels_tma.cuh)
+        ty.wq = pl->y_r2r >= 2 ? pl->wq_y : nullptr;
+        ty.reorder = pl->y_r2r >= 2 ? 1 : 0;
+        ty.neg = pl->y_r2r == 3 ? 1 : 0;
+        constexpr int RMODE = MODE == MODE_FWD ? MODE_R2R_FWD : MODE_R2R_INV;
+        return check_launch(launch_tma<RMODE>(pl->ny, pl->y_cols, pl->map_y, ty, row_stride, outer_stride, pl->spec,
+                                              st, pl->num_sms, k0, k1 - k0), what);
+    }
     return check_launch(launch_tma<MODE>(pl->ny, pl->y_cols, pl->map_y, ty, row_stride, outer_stride, pl->spec,
                                          st, pl->num_sms, k0, k1 - k0), what);
 }
@@ -798,22 +912,25 @@ static int enqueue_z(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
             ta.ny = pl->ny;
             ta.nz = pl->nz;
             ta.dz2 = 1.0 / inv_dz2;
-            const size_t smem_t = ThomasGeom::smem_bytes(pl->nz);
-            auto kern = pl->thomas_warps == 2 ? thomas_tma_kernel<2> : thomas_tma_kernel<1>;
+            ta.has_null = pl->has_null;
+            const size_t smem_t = ThomasGeom::smem_bytes(pl->nz, thomas_cw(pl));
+            auto kern = pl->xsplit ? (pl->thomas_warps == 2 ? thomas_tma_kernel<2, 16> : thomas_tma_kernel<1, 16>)
+                                   : (pl->thomas_warps == 2 ? thomas_tma_kernel<2, 8> : thomas_tma_kernel<1, 8>);
             if (set_smem(kern, smem_t) != cudaSuccess) return check_launch(cudaGetLastError(), "z_solve attr");
             long long grid = pl->num_sms;
             if (grid > (long long)ta.n_tiles_x * ta.ny) grid = (long long)ta.n_tiles_x * ta.ny;
             kern<<<(unsigned)grid, 32 * (pl->thomas_warps + 1), smem_t, st>>>(pl->map_z, ta);
         } else {
             thomas_kernel<<<(unsigned)((ncol + 127) / 128), 128, 0, st>>>(pl->spec, pl->cp, pl->pitch, pl->ny, pl->nz, pl->nxh,
-                                                                        pl->lam_x, pl->lam_y, inv_dz2, pl->plane);
+                                                                        pl->lam_x, pl->lam_y, inv_dz2, pl->plane, pl->end_coef_z, pl->has_null);
         }
         if (int rc = check_launch(cudaGetLastError(), "z_solve (thomas)")) return rc;
         if (tm) tm->mark();
+        if (!pl->has_null) return FLUTAS_OK;   // a Dirichlet direction: no singular mode
         const size_t smem = sizeof(double) * (4 * (size_t)pl->nz + 2);
         // nz <= 4096 (checked at plan creation): at most 128 KB
         if (set_smem(thomas_singular_kernel, smem) != cudaSuccess) return check_launch(cudaGetLastError(), "z_singular attr");
-        thomas_singular_kernel<<<1, 256, smem, st>>>(pl->spec, pl->plane, pl->nz, pl->sing_coef);
+        thomas_singular_kernel<<<1, 256, smem, st>>>(pl->spec, pl->plane, pl->nz, pl->sing_coef, pl->xsplit);
         if (int rc = check_launch(cudaGetLastError(), "z_singular")) return rc;
         if (tm) tm->mark();
     }
@@ -871,6 +988,16 @@ static int ensure_lanes(flutas_plan *pl, int nchunk) {
     return FLUTAS_OK;
 }
 
+// Dirichlet pressure conditions are for flutas_poisson_solve only: the step needs the boundary-normal velocity on both
+// boundary faces of such a direction, and a line of n cells stores n faces (include/flutas.h)
+static int check_step_bc(const flutas_plan *pl) {
+    for (int d = 0; d < 3; ++d)
+        if (pl->bc[d] == FLUTAS_BC_DIRICHLET)
+            return fail(FLUTAS_ERR_INVALID_ARG, "the projection step takes periodic or wall (Neumann) directions only; "
+                                                "a Dirichlet plan serves flutas_poisson_solve");
+    return FLUTAS_OK;
+}
+
 // p_out may be p (in place) or p_old (ping-pong) exactly, or a seventh field; anything else must not overlap
 static int check_step_fields(const flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
                              const double *p, const double *p_old, const double *p_out) {
@@ -886,6 +1013,7 @@ extern "C" int flutas_projection_step_ex(flutas_plan *pl, double *u, double *v, 
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail(FLUTAS_ERR_INVALID_ARG, "dt must be positive and finite");
     if (!(dt_ratio > 0.0) || !std::isfinite(dt_ratio)) return fail(FLUTAS_ERR_INVALID_ARG, "dt_ratio must be positive and finite");
     if (int rc = check_step_fields(pl, u, v, w, phi, p, p_old, p_out)) return rc;
+    if (int rc = check_step_bc(pl)) return rc;
     if (!pl->ws_base) return fail(FLUTAS_ERR_INVALID_ARG, "the plan has no workspace (flutas_plan_set_workspace)");
     cudaStream_t st = (cudaStream_t)stream;
     StepTimer tm(pl, st);
@@ -963,6 +1091,7 @@ extern "C" int flutas_splitting_rhs_ex(flutas_plan *pl, const double *u, const d
     if (!(dt_ratio > 0.0) || !std::isfinite(dt_ratio)) return fail(FLUTAS_ERR_INVALID_ARG, "dt_ratio must be positive and finite");
     const void *ptrs[7] = {u, v, w, phi, p, p_old, rhs_out};
     if (int rc = check_fields(pl, ptrs, 7)) return rc;
+    if (int rc = check_step_bc(pl)) return rc;
     if (!pl->ws_base) return fail(FLUTAS_ERR_INVALID_ARG, "the plan has no workspace (flutas_plan_set_workspace)");
     return enqueue_rhs(pl, u, v, w, phi, p, p_old, dt, dt_ratio, rhs_out, (cudaStream_t)stream, 0, pl->nz);
 }

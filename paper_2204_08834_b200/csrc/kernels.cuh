@@ -35,6 +35,8 @@ struct GridParams {
     double rho1, rho2, rho0;
     double c_pn, c_po;   // p_hat = c_pn p^n - c_po p^(n-1); (2, 1) for constant dt, (1 + r, r) in general
     double flux_one;     // 1, or 0 when rho1 == rho2: the splitting coefficient 1 - rho0/rho_f is then exactly 0
+    int wall_x, wall_y;  // walls (u_n = 0, dp/dn = 0) at both ends of x / y: the last stored face is the wall face (passes through),
+                         // the first wall face is not stored and carries 0 (as `wall` along z)
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -151,19 +153,25 @@ splitting_rhs_kernel2(GridParams g, double dt, int kc, const double *__restrict_
         double rc_e = __shfl_down_sync(0xffffffffu, rc_c.x, 1), ph_e = __shfl_down_sync(0xffffffffu, ph_c.x, 1);
         if (edge_r) { rc_e = rho_of(e_phi); ph_e = phat(e_p, e_po); }
         const double fm = flux_coef(rc_c.x, rc_c.y, m2rho0, one) * ((ph_c.y - ph_c.x) * idx);
-        const double fe = flux_coef(rc_c.y, rc_e, m2rho0, one) * ((ph_e - ph_c.y) * idx);
+        double fe = flux_coef(rc_c.y, rc_e, m2rho0, one) * ((ph_e - ph_c.y) * idx);
+        if (g.wall_x && i0 + 2 == nx) fe = 0.0;
         double f_w = __shfl_up_sync(0xffffffffu, fe, 1), u_w = __shfl_up_sync(0xffffffffu, uc.y, 1);
         if (edge_l) {
             f_w = flux_coef(rho_of(w_phi), rc_c.x, m2rho0, one) * ((ph_c.x - phat(w_p, w_po)) * idx);
             u_w = w_u;
         }
+        const bool wall_w = g.wall_x && i0 == 0, wall_e = g.wall_x && i0 + 2 == nx;
+        const bool wall_s = g.wall_y && j == 0, wall_n = g.wall_y && j + 1 == ny;
+        if (wall_w) { f_w = 0.0; u_w = 0.0; }
         // ---- y faces
         const double2 rc_n = rho2_of(r_nphi), ph_n = phat2(r_np, r_npo);
         const double2 rc_s = rho2_of(r_sphi), ph_s = phat2(r_sp, r_spo);
-        const double fn0 = flux_coef(rc_c.x, rc_n.x, m2rho0, one) * ((ph_n.x - ph_c.x) * idy);
-        const double fn1 = flux_coef(rc_c.y, rc_n.y, m2rho0, one) * ((ph_n.y - ph_c.y) * idy);
-        const double fs0 = flux_coef(rc_s.x, rc_c.x, m2rho0, one) * ((ph_c.x - ph_s.x) * idy);
-        const double fs1 = flux_coef(rc_s.y, rc_c.y, m2rho0, one) * ((ph_c.y - ph_s.y) * idy);
+        double fn0 = flux_coef(rc_c.x, rc_n.x, m2rho0, one) * ((ph_n.x - ph_c.x) * idy);
+        double fn1 = flux_coef(rc_c.y, rc_n.y, m2rho0, one) * ((ph_n.y - ph_c.y) * idy);
+        if (wall_n) fn0 = fn1 = 0.0;
+        double fs0 = flux_coef(rc_s.x, rc_c.x, m2rho0, one) * ((ph_c.x - ph_s.x) * idy);
+        double fs1 = flux_coef(rc_s.y, rc_c.y, m2rho0, one) * ((ph_c.y - ph_s.y) * idy);
+        if (wall_s) { fs0 = fs1 = 0.0; vs = make_double2(0.0, 0.0); }
 
         double2 out;
         out.x = c_div * ((uc.x - u_w) * idx + (vc.x - vs.x) * idy + (wc.x - wb.x) * idz) +
@@ -198,13 +206,14 @@ correction_kernel(GridParams g, double dt, long long q0, long long q1, const dou
     const long long qjp = (j + 1 == g.ny) ? q - (g.ny - 1) * sy : q + sy;
     const long long qkp = (k + 1 == g.nz) ? q - (g.nz - 1) * sz : q + sz;
     const bool top = g.wall && (k + 1 == g.nz);
+    const bool east = g.wall_x && (i + 2 == g.nx), north = g.wall_y && (j + 1 == g.ny);   // wall faces pass through
     const double c = dt / g.rho0;
     auto ld2 = [](const double *f, long long a) { return *reinterpret_cast<const double2 *>(f + a); };
     const double2 pc = ld2(pn, q), pj = ld2(pn, qjp), pk = ld2(pn, qkp);
     const double pe = pn[qip];
     const double2 a = ld2(up, q), b = ld2(vp, q), d = ld2(wp, q);
-    stcs2(u, q, make_double2(a.x - c * ((pc.y - pc.x) * g.inv_dx), a.y - c * ((pe - pc.y) * g.inv_dx)));
-    stcs2(v, q, make_double2(b.x - c * ((pj.x - pc.x) * g.inv_dy), b.y - c * ((pj.y - pc.y) * g.inv_dy)));
+    stcs2(u, q, make_double2(a.x - c * ((pc.y - pc.x) * g.inv_dx), east ? a.y : a.y - c * ((pe - pc.y) * g.inv_dx)));
+    stcs2(v, q, north ? b : make_double2(b.x - c * ((pj.x - pc.x) * g.inv_dy), b.y - c * ((pj.y - pc.y) * g.inv_dy)));
     stcs2(w, q, top ? d : make_double2(d.x - c * ((pk.x - pc.x) * g.inv_dz), d.y - c * ((pk.y - pc.y) * g.inv_dz)));
 }
 
@@ -235,7 +244,7 @@ __device__ __forceinline__ void tile_fft(double2 *s, const double2 *__restrict__
 }
 
 // modes of the strided transform kernels (kernels_tma.cuh, kernels_y16.cuh)
-enum { MODE_FWD = 0, MODE_INV = 1, MODE_SOLVE = 2 };
+enum { MODE_FWD = 0, MODE_INV = 1, MODE_SOLVE = 2, MODE_R2R_FWD = 3, MODE_R2R_INV = 4 };
 
 // ------------------------------------------------------------------------------------------------
 // Cooperative copy of TOT contiguous elements with B loads in flight per thread: all loads of a batch are
@@ -363,14 +372,15 @@ fft_x8_c2r_kernel(const double2 *__restrict__ spec, double *__restrict__ out, do
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128)
 thomas_kernel(double2 *__restrict__ spec, double *__restrict__ cp, int pitch, int ny, int nz, int nxh,
-              const double *__restrict__ lam_x, const double *__restrict__ lam_y, double inv_dz2, long long plane) {
+              const double *__restrict__ lam_x, const double *__restrict__ lam_y, double inv_dz2, long long plane,
+              double end_coef /* 1 Neumann, 3 Dirichlet */, int has_null) {
     const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long ncol = (long long)pitch * ny;
-    if (c >= ncol || c == 0) return;
+    if (c >= ncol || (has_null && c == 0)) return;
     const int kx = (int)(c % pitch), jy = (int)(c / pitch);
     if (kx >= nxh) return;
     const double lam = lam_x[kx] + lam_y[jy];
-    const double a = inv_dz2, b_end = -inv_dz2 + lam, b_in = -2.0 * inv_dz2 + lam;
+    const double a = inv_dz2, b_end = -end_coef * inv_dz2 + lam, b_in = -2.0 * inv_dz2 + lam;
     double inv = 1.0 / b_end;
     double cpv = a * inv;
     double2 d = spec[c];
@@ -401,8 +411,9 @@ thomas_kernel(double2 *__restrict__ spec, double *__restrict__ cp, int pitch, in
 
 // The (kx,ky) = (0,0) column: lam_xy = 0, the system is singular (pure Neumann).  Eliminate rows
 // 0..nz-2, pin x_{nz-1} = 0, back-substitute, then remove the mean over k (zero-mean gauge, R5).
+// re_only: with non-periodic x the imaginary part of column 0 is another (regular) mode and is left alone.
 __global__ void thomas_singular_kernel(double2 *__restrict__ spec, long long col_stride, int nz,
-                                       const double *__restrict__ coef /* inv_k, c'_k interleaved: 2 nz doubles */) {
+                                       const double *__restrict__ coef /* inv_k, c'_k interleaved: 2 nz doubles */, int re_only) {
     extern __shared__ double sm[];
     double *dr = sm, *di = sm + nz, *cf = sm + 2 * nz, *mean = sm + 4 * nz;
     for (int k = threadIdx.x; k < nz; k += blockDim.x) {
@@ -413,7 +424,8 @@ __global__ void thomas_singular_kernel(double2 *__restrict__ spec, long long col
         cf[2 * k + 1] = coef[2 * k + 1];
     }
     __syncthreads();
-    if (threadIdx.x < 2) {                      // thread 0: real parts, thread 1: imaginary parts
+    if (threadIdx.x == 1 && re_only) mean[1] = 0.0;
+    if (threadIdx.x < (re_only ? 1 : 2)) {      // thread 0: real parts, thread 1: imaginary parts
         double *x = threadIdx.x == 0 ? dr : di;
         const double a = cf[2 * nz - 1];        // slot of c'_{nz-1} (never used as such) carries a = 1/dz^2
         double prev = x[0] * cf[0];

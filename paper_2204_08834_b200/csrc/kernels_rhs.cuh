@@ -133,6 +133,8 @@ splitting_rhs_kernel3(GridParams g, double dt, int kc, int k_base, int k_end, co
     const int col = 2 + 2 * tx;                         // column of cell i0 inside a haloed row
     const int c_row = (ty + 1) * G::RP + col;           // centre row of phi / p / p_old
     const long long out0 = (long long)(j0 + ty) * nx + x0 + 2 * tx;
+    const bool wall_w = g.wall_x && x0 + 2 * tx == 0, wall_e = g.wall_x && x0 + 2 * tx + 2 == nx;
+    const bool wall_s = g.wall_y && j0 + ty == 0, wall_n = g.wall_y && j0 + ty + 1 == ny;
 
     // carried from plane to plane
     double2 rc_b = make_double2(1.0, 1.0), ph_b = make_double2(0.0, 0.0);   // rho_c, p_hat of the plane below
@@ -169,19 +171,26 @@ splitting_rhs_kernel3(GridParams g, double dt, int kc, int k_base, int k_end, co
             const double e_phi = S[G::O_PHI + c_row + 2], e_p = S[G::O_P + c_row + 2], e_po = S[G::O_PO + c_row + 2];
             const double w_phi = S[G::O_PHI + c_row - 1], w_p = S[G::O_P + c_row - 1], w_po = S[G::O_PO + c_row - 1];
             const double2 uc = ld2s(S + G::O_U + ty * G::RP + col);
-            const double u_w = S[G::O_U + ty * G::RP + col - 1];
-            const double2 vc = ld2s(S + G::O_V + (ty + 1) * G::X + 2 * tx), vs = ld2s(S + G::O_V + ty * G::X + 2 * tx);
+            double u_w = S[G::O_U + ty * G::RP + col - 1];
+            const double2 vc = ld2s(S + G::O_V + (ty + 1) * G::X + 2 * tx);
+            double2 vs = ld2s(S + G::O_V + ty * G::X + 2 * tx);
             const double2 wc = ld2s(S + G::O_W + ty * G::X + 2 * tx);
 
             const double fm = flux_coef(rc.x, rc.y, m2rho0, one) * ((ph.y - ph.x) * idx);
-            const double fe = flux_coef(rc.y, rho_of(e_phi), m2rho0, one) * ((phat(e_p, e_po) - ph.y) * idx);
-            const double fw = flux_coef(rho_of(w_phi), rc.x, m2rho0, one) * ((ph.x - phat(w_p, w_po)) * idx);
+            double fe = flux_coef(rc.y, rho_of(e_phi), m2rho0, one) * ((phat(e_p, e_po) - ph.y) * idx);
+            double fw = flux_coef(rho_of(w_phi), rc.x, m2rho0, one) * ((ph.x - phat(w_p, w_po)) * idx);
             const double2 rc_n = make_double2(rho_of(n_phi.x), rho_of(n_phi.y)), ph_n = make_double2(phat(n_p.x, n_po.x), phat(n_p.y, n_po.y));
             const double2 rc_s = make_double2(rho_of(s_phi.x), rho_of(s_phi.y)), ph_s = make_double2(phat(s_p.x, s_po.x), phat(s_p.y, s_po.y));
-            const double fn0 = flux_coef(rc.x, rc_n.x, m2rho0, one) * ((ph_n.x - ph.x) * idy);
-            const double fn1 = flux_coef(rc.y, rc_n.y, m2rho0, one) * ((ph_n.y - ph.y) * idy);
-            const double fs0 = flux_coef(rc_s.x, rc.x, m2rho0, one) * ((ph.x - ph_s.x) * idy);
-            const double fs1 = flux_coef(rc_s.y, rc.y, m2rho0, one) * ((ph.y - ph_s.y) * idy);
+            double fn0 = flux_coef(rc.x, rc_n.x, m2rho0, one) * ((ph_n.x - ph.x) * idy);
+            double fn1 = flux_coef(rc.y, rc_n.y, m2rho0, one) * ((ph_n.y - ph.y) * idy);
+            double fs0 = flux_coef(rc_s.x, rc.x, m2rho0, one) * ((ph.x - ph_s.x) * idy);
+            double fs1 = flux_coef(rc_s.y, rc.y, m2rho0, one) * ((ph.y - ph_s.y) * idy);
+            // walls along x / y: wall faces carry no flux and the unstored first wall face no velocity;
+            // the halo the copies wrapped around periodically is then simply not used
+            if (wall_e) fe = 0.0;
+            if (wall_w) { fw = 0.0; u_w = 0.0; }
+            if (wall_n) fn0 = fn1 = 0.0;
+            if (wall_s) { fs0 = fs1 = 0.0; vs = make_double2(0.0, 0.0); }
 
             part.x = c_div * ((uc.x - u_w) * idx + (vc.x - vs.x) * idy + (wc.x - wb.x) * idz) +
                      ((fm - fw) * idx + (fn0 - fs0) * idy);

@@ -42,75 +42,86 @@ struct ThomasGeom {
     static constexpr int NBUF = 3, NTAB = 2, B = 8;   // data buffers, table buffers, chain steps per register batch
     __host__ __device__ static int nzh(int nz) { return nz - nz / 2; }            // steps of the longer chain
     // per tile: entries j = 0 .. nzh (c_0 .. c_{nzh-1}, then f), two consecutive j packed per column so that a lane
-    // fetches c_j, c_{j+1} with one 16-byte load: [j / 2][column][j % 2]
-    __host__ __device__ static size_t tab_doubles(int nz) { return (size_t)((nzh(nz) + 2) / 2) * 2 * C; }
-    __host__ __device__ static int box_rows(int nz) { return nz < 256 ? nz : 256; }
+    // fetches c_j, c_{j+1} with one 16-byte load: [j / 2][column][j % 2].  cw = coefficient columns per tile: 8 when the
+    // real and imaginary part of a column share their eigenvalue (periodic x), 16 = (column, component) when they are
+    // two different modes along x (non-periodic x, kernels_r2r.cuh)
+    __host__ __device__ static size_t tab_doubles(int nz, int cw = C) { return (size_t)((nzh(nz) + 2) / 2) * 2 * cw; }
+    // rows per TMA box (<= 256): the column is cut into equal boxes, so a buffer is at most one row per box longer than nz
+    __host__ __device__ static int box_rows(int nz) { const int nb = (nz + 255) / 256; return (nz + nb - 1) / nb; }
     // a buffer holds whole boxes: the last one may hang over the end of the column (zero-filled, never stored)
     __host__ __device__ static size_t data_bytes(int nz) {
         return (size_t)((nz + box_rows(nz) - 1) / box_rows(nz)) * box_rows(nz) * C * 16;
     }
     // a warp's table buffer, with room for the 2B rows the forward loop requests past the end
-    __host__ __device__ static size_t tab_stride(int nz) { return ((tab_doubles(nz) + 2 * B * C) * 8 + 127) / 128 * 128; }
-    __host__ __device__ static int tab_index(int j, int col) { return (j >> 1) * 2 * C + col * 2 + (j & 1); }
-    __host__ static size_t smem_bytes(int nz) {
-        return NBUF * data_bytes(nz) + NTAB * tab_stride(nz) + 128;
+    __host__ __device__ static size_t tab_stride(int nz, int cw = C) { return ((tab_doubles(nz, cw) + 2 * B * cw) * 8 + 127) / 128 * 128; }
+    __host__ __device__ static int tab_index(int j, int col, int cw = C) { return (j >> 1) * 2 * cw + col * 2 + (j & 1); }
+    __host__ static size_t smem_bytes(int nz, int cw = C) {
+        return NBUF * data_bytes(nz) + NTAB * tab_stride(nz, cw) + 128;
     }
 };
 
-// one thread per column of the tiled table; true divisions (this runs once per plan)
-__global__ void thomas_table_kernel(double *__restrict__ tab, int n_tiles_x, int ny, int nz, int nxh,
-                                    const double *__restrict__ lam_x, const double *__restrict__ lam_y, double inv_dz2) {
+// one thread per coefficient column of the tiled table; true divisions (this runs once per plan).
+// lam_x2[2 kx + component]: eigenvalue along x of the real (0) / imaginary (1) part of column kx; cw = 8 uses component 0.
+// end_coef: first / last diagonal = -end_coef a + lam: 1 Neumann (R7), 3 Dirichlet (p = 0 on the boundary face).
+// has_null: the (0, 0) mode is singular (no Dirichlet direction) and gets benign coefficients (thomas_singular_kernel).
+__global__ void thomas_table_kernel(double *__restrict__ tab, int n_tiles_x, int ny, int nz, int nxh, int cw,
+                                    const double *__restrict__ lam_x2, const double *__restrict__ lam_y, double inv_dz2,
+                                    double end_coef, int has_null) {
     using G = ThomasGeom;
     const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long ncol = (long long)n_tiles_x * ny * G::C;
+    const long long ncol = (long long)n_tiles_x * ny * cw;
     if (c >= ncol) return;
-    const int col = (int)(c % G::C);
-    const long long tile = c / G::C;
+    const int cc = (int)(c % cw);
+    const int col = cw == G::C ? cc : cc >> 1, comp = cw == G::C ? 0 : cc & 1;
+    const long long tile = c / cw;
     const int tx = (int)(tile % n_tiles_x), jy = (int)(tile / n_tiles_x);
     const int kx = tx * G::C + col;
     const int nzh = G::nzh(nz), m = nz / 2;
-    double *t = tab + tile * G::tab_doubles(nz);
-    if (kx >= nxh || (kx == 0 && jy == 0)) {          // padding columns and the singular column: benign values
-        for (int j = 0; j < nzh; ++j) t[G::tab_index(j, col)] = 0.0;
-        t[G::tab_index(nzh, col)] = 1.0;
+    double *t = tab + tile * G::tab_doubles(nz, cw);
+    if (kx >= nxh || (has_null && kx == 0 && comp == 0 && jy == 0)) {   // padding columns and the singular mode: benign values
+        for (int j = 0; j < nzh; ++j) t[G::tab_index(j, cc, cw)] = 0.0;
+        t[G::tab_index(nzh, cc, cw)] = 1.0;
         return;
     }
-    const double lam = lam_x[kx] + lam_y[jy];
-    const double a = inv_dz2, b_end = -inv_dz2 + lam, b_in = -2.0 * inv_dz2 + lam;
+    const double lam = lam_x2[2 * kx + comp] + lam_y[jy];
+    const double a = inv_dz2, b_end = -end_coef * inv_dz2 + lam, b_in = -2.0 * inv_dz2 + lam;
     double cj = a / b_end, c_m1 = 0.0;                // c_m1 = c_{m-1}
-    t[G::tab_index(0, col)] = cj;
+    t[G::tab_index(0, cc, cw)] = cj;
     if (m == 1) c_m1 = cj;
     for (int j = 1; j < nzh; ++j) {
         cj = a / (b_in - a * cj);
-        t[G::tab_index(j, col)] = cj;
+        t[G::tab_index(j, cc, cw)] = cj;
         if (j == m - 1) c_m1 = cj;
     }
-    t[G::tab_index(nzh, col)] = 1.0 / (1.0 - cj * c_m1);   // cj = c_{nzh-1} = c~_m
+    t[G::tab_index(nzh, cc, cw)] = 1.0 / (1.0 - cj * c_m1);   // cj = c_{nzh-1} = c~_m
 }
 
 struct ThomasArgs {
     const double *tab;
     int n_tiles_x, ny, nz;
     double dz2;               // 1 / a
+    int has_null;             // the (0, 0) mode is left to thomas_singular_kernel
 };
 
-template <int NWARP>
+template <int NWARP, int CW>
 __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const __grid_constant__ CUtensorMap tmap, ThomasArgs a) {
     using G = ThomasGeom;
+    static_assert(CW == 8 || CW == 16, "coefficient columns per tile");
     extern __shared__ unsigned char smem_raw[];
     __shared__ uint64_t full_d[G::NBUF], full_c[G::NTAB], done[G::NBUF];
 
     const int nz = a.nz, nzh = G::nzh(nz), m = nz / 2;
     const int rows = G::box_rows(nz), nbox = (nz + rows - 1) / rows;
     const uint32_t box_bytes = (uint32_t)rows * G::C * 16u;
-    const uint32_t tab_bytes = (uint32_t)G::tab_doubles(nz) * 8u;
+    const uint32_t tab_bytes = (uint32_t)G::tab_doubles(nz, CW) * 8u;
     unsigned char *base = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
     const uint32_t buf_stride = (uint32_t)nbox * box_bytes;   // = G::data_bytes(nz)
     unsigned char *tab_base = base + G::NBUF * buf_stride;
-    const uint32_t tab_stride = (uint32_t)G::tab_stride(nz);
+    const uint32_t tab_stride = (uint32_t)G::tab_stride(nz, CW);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int col = lane & 7, comp = (lane >> 3) & 1, top = lane >> 4;   // top = 1: the chain that starts at k = nz-1
+    const int cc = CW == 8 ? col : col * 2 + comp;                       // this lane's coefficient column
     const long long ntiles = (long long)a.n_tiles_x * a.ny;
     const long long my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
     auto tile_of = [&](long long n) { return (long long)blockIdx.x + n * gridDim.x; };
@@ -135,7 +146,7 @@ __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const _
     auto issue_table = [&](long long n) {
         const int w = (int)(n % G::NTAB);
         mbar_arrive_expect_tx(&full_c[w], tab_bytes);
-        bulk_load(tab_base + w * tab_stride, a.tab + tile_of(n) * G::tab_doubles(nz), tab_bytes, &full_c[w]);
+        bulk_load(tab_base + w * tab_stride, a.tab + tile_of(n) * G::tab_doubles(nz, CW), tab_bytes, &full_c[w]);
     };
     auto issue_store = [&](long long n) {
         const long long tile = tile_of(n);
@@ -178,11 +189,12 @@ __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const _
         const uint32_t it_c = (uint32_t)(n / G::NTAB), it_d = (uint32_t)(n / G::NBUF);
         double *s = reinterpret_cast<double *>(base + b * buf_stride) + col * 2 + comp;   // element (row, col): s[row * 16]
         const double *ctab = reinterpret_cast<const double *>(tab_base + tb * tab_stride);
-        const double2 *ct2 = reinterpret_cast<const double2 *>(ctab) + col;      // (c_2q, c_2q+1): ct2[q * 8]
-        auto c_at = [&](int j) { return ctab[G::tab_index(j, col)]; };
-        const bool nostore = tile_of(n) == 0 && col == 0;   // the (0,0) column is left as it is (thomas_singular_kernel)
+        const double2 *ct2 = reinterpret_cast<const double2 *>(ctab) + cc;      // (c_2q, c_2q+1): ct2[q * CW]
+        auto c_at = [&](int j) { return ctab[G::tab_index(j, cc, CW)]; };
+        // the singular (0,0) mode is left as it is (thomas_singular_kernel): the whole column, or its real part only
+        const bool nostore = a.has_null && tile_of(n) == 0 && col == 0 && (CW == 8 || comp == 0);
         if (lane == 0 && n + G::NTAB < my_tiles)       // the table that takes this buffer next: on its way to L2 meanwhile
-            bulk_prefetch_l2(a.tab + tile_of(n + G::NTAB) * G::tab_doubles(nz), tab_bytes);
+            bulk_prefetch_l2(a.tab + tile_of(n + G::NTAB) * G::tab_doubles(nz, CW), tab_bytes);
         mbar_wait(&full_c[tb], it_c & 1);
         mbar_wait(&full_d[b], it_d & 1);
         auto row_of = [&](int j) { return top ? nz - 1 - j : j; };
@@ -202,7 +214,7 @@ __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const _
             double2 cn[G::B / 2];
 #pragma unroll
             for (int q = 0; q < G::B / 2; ++q) {
-                const double2 c2 = cp[q * 8];
+                const double2 c2 = cp[q * CW];
                 cc[2 * q] = c2.x; cc[2 * q + 1] = c2.y;
                 ec[2 * q] = sp[(2 * q) * ds] * (c2.x * dz2);
                 ec[2 * q + 1] = sp[(2 * q + 1) * ds] * (c2.y * dz2);
@@ -210,7 +222,7 @@ __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const _
 #pragma unroll
             for (int e = 0; e < G::B; ++e) dn[e] = sp[(G::B + e) * ds];
 #pragma unroll
-            for (int q = 0; q < G::B / 2; ++q) cn[q] = cp[(G::B / 2 + q) * 8];
+            for (int q = 0; q < G::B / 2; ++q) cn[q] = cp[(G::B / 2 + q) * CW];
 #pragma unroll 2
             for (int bt = 0; bt < nfull; ++bt) {
                 double d2[G::B], gv[G::B];
@@ -218,7 +230,7 @@ __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const _
 #pragma unroll
                 for (int e = 0; e < G::B; ++e) d2[e] = sp[(2 * G::B + e) * ds];
 #pragma unroll
-                for (int q = 0; q < G::B / 2; ++q) c2[q] = cp[(G::B + q) * 8];
+                for (int q = 0; q < G::B / 2; ++q) c2[q] = cp[(G::B + q) * CW];
 #pragma unroll
                 for (int e = 0; e < G::B; ++e) {
                     g = fma(-cc[e], g, ec[e]);             // the only dependent operation of a step
@@ -236,7 +248,7 @@ __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const _
 #pragma unroll
                 for (int q = 0; q < G::B / 2; ++q) cn[q] = c2[q];
                 sp += G::B * ds;
-                cp += (G::B / 2) * 8;
+                cp += (G::B / 2) * CW;
             }
         }
         for (int j0 = nfull * G::B; j0 < nzh; j0 += G::B) {
@@ -277,13 +289,13 @@ __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const _
         const int nfull_b = m >= 4 * G::B ? (m - 2) / G::B : 0;   // every lane has at least m - 2 steps left
         if (nfull_b > 0) {
             double *sp = s + row_of(jb) * 16;
-            const double2 *cp = ct2 + (jb >> 1) * 8;   // jb is odd: the pair (c_{jb-1}, c_jb)
+            const double2 *cp = ct2 + (jb >> 1) * CW;   // jb is odd: the pair (c_{jb-1}, c_jb)
             double dn[G::B];
             double2 cn[G::B / 2];
 #pragma unroll
             for (int e = 0; e < G::B; ++e) dn[e] = sp[-e * ds];
 #pragma unroll
-            for (int q = 0; q < G::B / 2; ++q) cn[q] = cp[-q * 8];
+            for (int q = 0; q < G::B / 2; ++q) cn[q] = cp[-q * CW];
             auto batch = [&](auto request_next) {
                 double d[G::B];
                 double2 c[G::B / 2];
@@ -295,7 +307,7 @@ __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const _
 #pragma unroll
                     for (int e = 0; e < G::B; ++e) dn[e] = sp[-(G::B + e) * ds];
 #pragma unroll
-                    for (int q = 0; q < G::B / 2; ++q) cn[q] = cp[-(G::B / 2 + q) * 8];
+                    for (int q = 0; q < G::B / 2; ++q) cn[q] = cp[-(G::B / 2 + q) * CW];
                 }
 #pragma unroll
                 for (int e = 0; e < G::B; ++e) {           // step e: j = jb - e, odd j first
@@ -307,7 +319,7 @@ __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const _
                     for (int e = 0; e < G::B; ++e) sp[-e * ds] = d[e];
                 }
                 sp -= G::B * ds;
-                cp -= (G::B / 2) * 8;
+                cp -= (G::B / 2) * CW;
             };
 #pragma unroll 2
             for (int bt = 0; bt + 1 < nfull_b; ++bt) batch(std::true_type{});

@@ -38,6 +38,8 @@ struct TmaFftArgs {
     int nxh;         // valid kx columns
     const double2 *tw;                            // e^{-2 pi i m / N}
     const double *lam_x, *lam_outer, *lam_pos;    // SOLVE: eigenvalues in storage (permuted) order
+    const double2 *wq;                            // MODE_R2R_*: see Tma1Args
+    int reorder, neg;
 };
 
 // reciprocal of a normal, non-zero double (either sign): hardware seed + two Newton steps, <= ~1 ulp
@@ -206,6 +208,11 @@ struct Tma1Args {
     int n_tiles_x, n_outer, outer0, line_dim, nxh;   // outer indices outer0 .. outer0 + n_outer - 1
     const double2 *tw;
     const double *lam_x, *lam_outer, *lam_pos;
+    // MODE_R2R_FWD / MODE_R2R_INV (non-periodic directions, kernels_r2r.cuh): the real-linear expansion applied to the
+    // real and the imaginary part of every column separately
+    const double2 *wq;       // e^{-i pi k / (2N)}, k = 0 .. N/2 (cosine / sine expansion); nullptr = half-complex (w = 1)
+    int reorder;             // 1: rows enter as v[n] = z[2n], v[N-1-n] = z[2n+1] (cosine / sine), 0: as they are
+    int neg;                 // 1: the odd rows change sign (sine expansion)
 };
 
 template <int N, int P_IDX> struct PassGeom {     // geometry of pass P_IDX (1-based) for one thread
@@ -238,6 +245,15 @@ __device__ __forceinline__ void butterfly_pass(double2 *v, const double2 *twr) {
     }
 }
 
+// MODE_R2R_FWD / MODE_R2R_INV: a complex FFT of the (re-ordered) rows gives F; the expansion of the real part and of
+// the imaginary part, still packed as one complex number per column, is a butterfly between k and N-k:
+//     P = w_k F[k],  Q = conj(w_k) F[N-k]:   out[k] = P + Q,   out[N-k] = i (P - Q)        (k = 1 .. N/2 - 1)
+//     out[0] = 2 F[0],  out[N/2] = 2 Re(w_{N/2}) F[N/2]
+// (w_k = e^{-i pi k / (2N)}: componentwise unnormalised DCT-II, out[k] = X_re[k] + i X_im[k]; sign flip of the odd rows on
+// entry: DST-II read backwards; w = 1 and no re-ordering: twice the cosine and minus twice the sine coefficient of the
+// periodic expansion, both with eigenvalue lam[k]).  out[k] is stored at the position the FFT leaves frequency k at,
+// so the eigenvalue tables are permuted exactly as in the periodic case.  One more trip through shared memory than the
+// plain transform (the last pass cannot store straight to global), no extra trip through HBM.
 template <int N, int C, int MODE, int NT, int NCACHE>
 __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__ CUtensorMap tmap, Tma1Args a) {
     static_assert(NT == N * C / 8 || (N * C / 8 < 32 && NT == 32), "one butterfly per thread");
@@ -364,6 +380,99 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
                     global_store(std::integral_constant<int, PI>{}, gp, valid, v);
                 }
             });
+        } else if (MODE == MODE_R2R_FWD) {
+            auto row_of = [&](int n) { return a.reorder ? (n < N / 2 ? 2 * n : 2 * N - 1 - 2 * n) : n; };
+            {   // pass 1 reads the rows in the order of the expansion; it is not in place, so all reads come first
+                using G = PassGeom<N, 1>;
+                const int base = G::base(t);
+                if (active) {
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int n = base + e * G::M;
+                        v[e] = s[row_of(n) * C + l];
+                        if (a.neg && n >= N / 2) v[e] = make_double2(-v[e].x, -v[e].y);
+                    }
+                }
+                __syncthreads();
+                if (NCACHE >= 1) butterfly_pass<N, 1, -1>(v, twr);
+                else {
+                    double2 tl[7];
+                    if (G::HAS_TW) {
+#pragma unroll
+                        for (int k1 = 1; k1 < 8; ++k1) tl[k1 - 1] = a.tw[(active ? G::n2(t) : 0) * k1];
+                    }
+                    butterfly_pass<N, 1, -1>(v, tl);
+                }
+                if (active) smem_store(std::integral_constant<int, 1>{}, s, v);
+                __syncthreads();
+            }
+            static_for<2, P>([&](auto pi) {
+                if (active) {
+                    smem_pass(pi, std::integral_constant<int, -1>{}, s, v);
+                    smem_store(pi, s, v);
+                }
+                __syncthreads();
+            });
+            if (valid) {   // the butterfly between k and N - k, straight to global memory
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int k = t + r * (N / 8);
+                    if (k == 0) {
+                        const double2 f0 = s[l], fh = s[pos_of_freq<N>(N / 2) * C + l];
+                        const double wh = a.wq ? 2.0 * a.wq[N / 2].x : 2.0;
+                        gp[0] = make_double2(2.0 * f0.x, 2.0 * f0.y);
+                        gp[(long long)pos_of_freq<N>(N / 2) * a.row_stride] = make_double2(wh * fh.x, wh * fh.y);
+                    } else {
+                        const int pa = pos_of_freq<N>(k), pb = pos_of_freq<N>(N - k);
+                        const double2 w = a.wq ? a.wq[k] : make_double2(1.0, 0.0);
+                        const double2 pp = cmul(w, s[pa * C + l]), qq = cmulc(s[pb * C + l], w);
+                        gp[(long long)pa * a.row_stride] = cadd(pp, qq);
+                        const double2 d = csub(pp, qq);
+                        gp[(long long)pb * a.row_stride] = make_double2(-d.y, d.x);
+                    }
+                }
+            }
+        } else if (MODE == MODE_R2R_INV) {
+            if (active) {   // undo the butterfly in place (every pair belongs to one thread)
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int k = t + r * (N / 8);
+                    if (k == 0) {
+                        const int ph = pos_of_freq<N>(N / 2) * C + l;
+                        const double wh = a.wq ? 0.5 / a.wq[N / 2].x : 0.5;
+                        s[l] = make_double2(0.5 * s[l].x, 0.5 * s[l].y);
+                        s[ph] = make_double2(wh * s[ph].x, wh * s[ph].y);
+                    } else {
+                        const int pa = pos_of_freq<N>(k) * C + l, pb = pos_of_freq<N>(N - k) * C + l;
+                        const double2 w = a.wq ? a.wq[k] : make_double2(1.0, 0.0);
+                        const double2 c = s[pa], sn = s[pb];
+                        const double2 pp = make_double2(0.5 * (c.x + sn.y), 0.5 * (c.y - sn.x));   // (c - i s) / 2
+                        const double2 qq = make_double2(0.5 * (c.x - sn.y), 0.5 * (c.y + sn.x));   // (c + i s) / 2
+                        s[pa] = cmulc(pp, w);
+                        s[pb] = cmul(w, qq);
+                    }
+                }
+            }
+            __syncthreads();
+            static_for<1, P>([&](auto pr) {
+                constexpr int PI = P + 1 - decltype(pr)::value;
+                if (active) smem_pass(std::integral_constant<int, PI>{}, std::integral_constant<int, +1>{}, s, v);
+                if (PI > 1) {
+                    if (active) smem_store(std::integral_constant<int, PI>{}, s, v);
+                    __syncthreads();
+                }
+            });
+            if (valid) {   // the last pass leaves natural order: element n goes back to the row it came from
+                using G = PassGeom<N, 1>;
+                const int base = G::base(t);
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int n = base + e * G::M;
+                    const int row = a.reorder ? (n < N / 2 ? 2 * n : 2 * N - 1 - 2 * n) : n;
+                    const bool flip = a.neg && n >= N / 2;
+                    gp[(long long)row * a.row_stride] = flip ? make_double2(-v[e].x, -v[e].y) : v[e];
+                }
+            }
         } else {
             const double lam_xy = a.lam_x[kx < a.nxh ? kx : 0] + a.lam_outer[outer];
             static_for<1, P>([&](auto pi) {

@@ -10,7 +10,7 @@ def to_dev(a):
 
 
 def plan_for(W):
-    return fl.Plan(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2)
+    return fl.Plan(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2, bc_x=getattr(W, "bc_x", 0), bc_y=getattr(W, "bc_y", 0))
 
 
 def gpu_step(W, plan=None):

@@ -21,6 +21,7 @@ import numpy as np
 
 BC_Z_PERIODIC = 0
 BC_Z_WALL = 1
+BC_PERIODIC, BC_NEUMANN, BC_DIRICHLET = 0, 1, 2      # per-direction conditions (NEUMANN = wall)
 TWO_PI = 2.0 * np.pi
 
 
@@ -42,6 +43,12 @@ class Workload:
     phi: np.ndarray = field(repr=False, default=None)
     p: np.ndarray = field(repr=False, default=None)
     p_old: np.ndarray = field(repr=False, default=None)
+    bc_x: int = BC_PERIODIC
+    bc_y: int = BC_PERIODIC
+
+    @property
+    def bc(self):
+        return (self.bc_x, self.bc_y, self.bc_z)
 
     @property
     def shape(self):
@@ -278,6 +285,45 @@ def random_case(nx, ny, nz, bc_z, ratio, seed, box=None):
     phi = 0.5 * (1.0 + np.tanh(-s / 0.1))
     return Workload(f"rand_{nx}x{ny}x{nz}_bc{bc_z}_r{ratio:g}_s{seed}", nx, ny, nz, tuple(box), bc_z, 1.0,
                     float(ratio), 1e-3, seed, u, v, w, phi, p, p_old)
+
+
+def _zero_wall_faces(W):
+    """a walled (NEUMANN) direction stores its far wall face as the last face of every line: no-slip, 0 on entry"""
+    if W.bc_x == BC_NEUMANN:
+        W.u[:, :, -1] = 0.0
+    if W.bc_y == BC_NEUMANN:
+        W.v[:, -1, :] = 0.0
+    if W.bc_z == BC_NEUMANN:
+        W.w[-1] = 0.0
+    return W
+
+
+def random_case_bc(nx, ny, nz, bc, ratio, seed, box=(2.0, 1.5, 1.0)):
+    """random_case with a boundary condition per direction, bc = (bc_x, bc_y, bc_z) in {PERIODIC, NEUMANN}"""
+    W = random_case(nx, ny, nz, BC_Z_WALL if bc[2] == BC_NEUMANN else BC_Z_PERIODIC, ratio, seed, box=box)
+    W.bc_x, W.bc_y = int(bc[0]), int(bc[1])
+    W.name = f"rand_{nx}x{ny}x{nz}_bc{bc[0]}{bc[1]}{bc[2]}_r{ratio:g}_s{seed}"
+    return _zero_wall_faces(W)
+
+
+def cavity(nx=256, ny=256, nz=64, ratio=1.0, seed=6):
+    """Closed-cavity-shaped case (a box whose boundaries are all solid no-slip walls; the paper's run is a
+    256 x 256 plane, this is that plane extruded to nz cells): walls in x, y and z, box 1 x 1 x nz/nx.
+    u*, v*, w* ~ U[-1,1] + one smooth circulation cell (the thermally driven roll of the paper's case), wall faces 0;
+    a stratified two-layer phi; p, p_old ~ U[-0.1,0.1]."""
+    rng = np.random.default_rng(seed)
+    shape, box = (nz, ny, nx), (1.0, 1.0, nz / nx)
+    u, v, w = (_uniform(rng, shape, -1.0, 1.0) for _ in range(3))
+    p, p_old = (_uniform(rng, shape, -0.1, 0.1) for _ in range(2))
+    xc, yc, zc = _centres(nx, box[0]), _centres(ny, box[1]), _centres(nz, box[2])
+    xf, yf = _faces(nx, box[0]), _faces(ny, box[1])
+    # one roll in the (x, y) plane: stream function sin(pi x) sin(pi y) sampled at the faces
+    u += 2.0 * (np.sin(np.pi * xf)[None, None, :] * np.cos(np.pi * yc)[None, :, None]) * np.ones((nz, 1, 1))
+    v -= 2.0 * (np.cos(np.pi * xc)[None, None, :] * np.sin(np.pi * yf)[None, :, None]) * np.ones((nz, 1, 1))
+    phi = np.broadcast_to((0.5 * (1.0 + np.tanh((0.5 - yc) / (2.0 * box[1] / ny))))[None, :, None], shape).copy()
+    W = Workload(f"cavity_{nx}x{ny}x{nz}_walls", nx, ny, nz, box, BC_Z_WALL, 1.0, float(ratio), 1e-3, seed,
+                 u, v, w, phi, p, p_old, BC_NEUMANN, BC_NEUMANN)
+    return _zero_wall_faces(W)
 
 
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
