@@ -133,9 +133,12 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     W = make_workload(name, ratio)
     gen_s = time.time() - t0
     plan = fl.Plan(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2, bc_x=W.bc_x, bc_y=W.bc_y)
-    for kv in (args.opt or []):                       # experiments only: plan tuning knobs
+    for kv in (args.opt or []):                       # experiments only: plan tuning knobs (skipped where they do not apply)
         k_, v_ = kv.split("=")
-        plan.set_option(k_, int(v_))
+        try:
+            plan.set_option(k_, int(v_))
+        except fl.FlutasError:
+            pass
     host = list(W.fields())
     dev = [torch.from_numpy(a).cuda() for a in host]
     torch.cuda.synchronize()

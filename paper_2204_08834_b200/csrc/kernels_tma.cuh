@@ -254,6 +254,18 @@ __device__ __forceinline__ void butterfly_pass(double2 *v, const double2 *twr) {
 // periodic expansion, both with eigenvalue lam[k]).  out[k] is stored at the position the FFT leaves frequency k at,
 // so the eigenvalue tables are permuted exactly as in the periodic case.  One more trip through shared memory than the
 // plain transform (the last pass cannot store straight to global), no extra trip through HBM.
+// Barrier between pass P_IDX and pass P_IDX + 1 (either direction).  The butterflies of pass p + 1 that touch one block
+// of 8 M_p positions are run by exactly the threads that ran pass p on that block (M_p butterflies x C columns,
+// consecutive thread ids), so only the first exchange is CTA-wide; the later ones synchronise M_p C threads: a named
+// barrier for 64 and more, __syncwarp below.  Besides being cheaper, this lets the groups drift apart, so that some are
+// in the FP64 part of a pass while others are in its shared-memory part.
+template <int N, int C, int P_IDX> __device__ __forceinline__ void exchange_sync(int tid) {
+    constexpr int GS = (P_IDX < Fact<N>::P ? N / ipow8(P_IDX) : 1) * C;      // threads per group
+    if constexpr (P_IDX == 1 || GS * 8 >= N * C) __syncthreads();
+    else if constexpr (GS <= 32) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(1 + tid / GS), "n"(GS) : "memory");
+}
+
 template <int N, int C, int MODE, int NT, int NCACHE>
 __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__ CUtensorMap tmap, Tma1Args a) {
     static_assert(NT == N * C / 8 || (N * C / 8 < 32 && NT == 32), "one butterfly per thread");
@@ -364,7 +376,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
                 if (active) smem_pass(pi, std::integral_constant<int, -1>{}, s, v);
                 if (PI < P) {
                     if (active) smem_store(pi, s, v);
-                    __syncthreads();
+                    exchange_sync<N, C, PI>(tid);
                 } else {
                     global_store(pi, gp, valid, v);
                 }
@@ -375,7 +387,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
                 if (active) smem_pass(std::integral_constant<int, PI>{}, std::integral_constant<int, +1>{}, s, v);
                 if (PI > 1) {
                     if (active) smem_store(std::integral_constant<int, PI>{}, s, v);
-                    __syncthreads();
+                    exchange_sync<N, C, (PI > 1 ? PI - 1 : 1)>(tid);
                 } else {
                     global_store(std::integral_constant<int, PI>{}, gp, valid, v);
                 }
@@ -480,7 +492,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
                 if (active) smem_pass(pi, std::integral_constant<int, -1>{}, s, v);
                 if (PI < P) {
                     if (active) smem_store(pi, s, v);
-                    __syncthreads();
+                    exchange_sync<N, C, PI>(tid);
                 }
             });
             // v holds the last forward pass: divide by the eigenvalue sum, run the first inverse pass in registers
@@ -504,7 +516,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
                 }
                 if (P > 1) {
                     if (active) smem_store(std::integral_constant<int, P>{}, s, v);
-                    __syncthreads();
+                    exchange_sync<N, C, (P > 1 ? P - 1 : 1)>(tid);
                 } else {
                     global_store(std::integral_constant<int, P>{}, gp, valid, v);
                 }
@@ -514,7 +526,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
                 if (active) smem_pass(std::integral_constant<int, PI>{}, std::integral_constant<int, +1>{}, s, v);
                 if (PI > 1) {
                     if (active) smem_store(std::integral_constant<int, PI>{}, s, v);
-                    __syncthreads();
+                    exchange_sync<N, C, (PI > 1 ? PI - 1 : 1)>(tid);
                 } else {
                     global_store(std::integral_constant<int, PI>{}, gp, valid, v);
                 }
