@@ -553,8 +553,8 @@ extern "C" const char *flutas_plan_kernel_symbol(const flutas_plan *pl, int idx)
     const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
     switch (pl->launch_ids[idx]) {
         case K_RHS: return rhs_takes_ranges(pl) ? "splitting_rhs_kernel3" : "splitting_rhs_kernel2";
-        case K_FFTX: return pl->xsplit ? "fft_x_r2r_fwd_kernel" : pl->nx == 8 ? "fft_x8_r2c_kernel" : (x_is_persistent(pl) ? "fft_x_r2c_tma_kernel" : "fft_x_r2c_kernel");
-        case K_IFFTX: return pl->xsplit ? "fft_x_r2r_inv_kernel" : pl->nx == 8 ? "fft_x8_c2r_kernel" : (x_is_persistent(pl) ? "fft_x_c2r_tma_kernel" : "fft_x_c2r_kernel");
+        case K_FFTX: return pl->xsplit ? (x_is_persistent(pl) ? "fft_x_r2c_tma_kernel" : "fft_x_r2r_fwd_kernel") : pl->nx == 8 ? "fft_x8_r2c_kernel" : (x_is_persistent(pl) ? "fft_x_r2c_tma_kernel" : "fft_x_r2c_kernel");
+        case K_IFFTX: return pl->xsplit ? (x_is_persistent(pl) ? "fft_x_c2r_tma_kernel" : "fft_x_r2r_inv_kernel") : pl->nx == 8 ? "fft_x8_c2r_kernel" : (x_is_persistent(pl) ? "fft_x_c2r_tma_kernel" : "fft_x_c2r_kernel");
         case K_FFTY: case K_IFFTY:
             return pl->y16 ? "fft_y1024_kernel" : (pl->ny * pl->y_cols / 8 <= 512 ? "fft_tma1_kernel" : "fft_tma_kernel");
         case K_Z:
@@ -716,9 +716,9 @@ template <int N2> static cudaError_t launch_r2r_inv_n(const flutas_plan *pl, dou
     return cudaGetLastError();
 }
 // persistent bulk-copy-fed x kernels (nx = 128 .. 1024)
-template <int N2> static cudaError_t launch_r2c_tma_n(const flutas_plan *pl, const double *rhs, cudaStream_t st, long long tile0, long long ntiles) {
+template <int N2, int KIND> static cudaError_t launch_r2c_tma_n(const flutas_plan *pl, const double *rhs, cudaStream_t st, long long tile0, long long ntiles) {
     const size_t smem = (size_t)2 * 8 * N2 * 16 + 128;
-    auto kern = fft_x_r2c_tma_kernel<N2>;
+    auto kern = fft_x_r2c_tma_kernel<N2, KIND>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
@@ -727,12 +727,13 @@ template <int N2> static cudaError_t launch_r2c_tma_n(const flutas_plan *pl, con
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     long long grid = (long long)pl->num_sms * per_sm;
     if (grid > ntiles) grid = ntiles;
-    kern<<<(unsigned)grid, N2, smem, st>>>(rhs + tile0 * 8 * 2 * N2, pl->spec, pl->tw_x, (int)ntiles, SpecRows{pl->ny, pl->plane, tile0 * 8});
+    kern<<<(unsigned)grid, N2, smem, st>>>(rhs + tile0 * 8 * 2 * N2, pl->spec, pl->tw_x, (int)ntiles, SpecRows{pl->ny, pl->plane, tile0 * 8},
+                                           pl->wq_x, pl->bc[0] == FLUTAS_BC_DIRICHLET ? 1 : 0);
     return cudaGetLastError();
 }
-template <int N2> static cudaError_t launch_c2r_tma_n(const flutas_plan *pl, double *out, double scale, cudaStream_t st, long long tile0, long long ntiles) {
+template <int N2, int KIND> static cudaError_t launch_c2r_tma_n(const flutas_plan *pl, double *out, double scale, cudaStream_t st, long long tile0, long long ntiles) {
     const size_t smem = (size_t)8 * (N2 + 8) * 16 + (size_t)8 * N2 * 16 + 128;
-    auto kern = fft_x_c2r_tma_kernel<N2>;
+    auto kern = fft_x_c2r_tma_kernel<N2, KIND>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
@@ -741,7 +742,8 @@ template <int N2> static cudaError_t launch_c2r_tma_n(const flutas_plan *pl, dou
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     long long grid = (long long)pl->num_sms * per_sm;
     if (grid > ntiles) grid = ntiles;
-    kern<<<(unsigned)grid, N2, smem, st>>>(pl->spec, out + tile0 * 8 * 2 * N2, pl->tw_x, scale, (int)ntiles, SpecRows{pl->ny, pl->plane, tile0 * 8});
+    kern<<<(unsigned)grid, N2, smem, st>>>(pl->spec, out + tile0 * 8 * 2 * N2, pl->tw_x, scale, (int)ntiles, SpecRows{pl->ny, pl->plane, tile0 * 8},
+                                           pl->wq_x, pl->bc[0] == FLUTAS_BC_DIRICHLET ? 1 : 0);
     return cudaGetLastError();
 }
 #define FOR_EACH_N2_TMA(X) X(64) X(128) X(256) X(512)
@@ -749,10 +751,16 @@ template <int N2> static cudaError_t launch_c2r_tma_n(const flutas_plan *pl, dou
 // planes k0 .. k1 - 1 (a tile is 8 consecutive x-lines; ny is a multiple of 8)
 static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStream_t st, int k0, int k1) {
     const long long tile0 = (long long)k0 * pl->ny / 8, ntiles = (long long)(k1 - k0) * pl->ny / 8;
+    if (pl->xsplit && x_is_persistent(pl))
+        switch (pl->n2) {
+#define X(n) case n: return launch_r2c_tma_n<n, X_SPLIT>(pl, rhs, st, tile0, ntiles);
+            FOR_EACH_N2_TMA(X)
+#undef X
+        }
     if (pl->xsplit)
         switch (pl->n2) {
 #define X(n) case n: return launch_r2r_fwd_n<n>(pl, rhs, st, tile0, ntiles);
-            X(8) X(16) X(32) X(64) X(128) X(256) X(512)
+            X(8) X(16) X(32)
 #undef X
         }
     if (pl->nx == 8) {   // the degenerate length: one thread per line
@@ -762,7 +770,7 @@ static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStre
     }
     if (x_is_persistent(pl))
         switch (pl->n2) {
-#define X(n) case n: return launch_r2c_tma_n<n>(pl, rhs, st, tile0, ntiles);
+#define X(n) case n: return launch_r2c_tma_n<n, X_PERIODIC>(pl, rhs, st, tile0, ntiles);
             FOR_EACH_N2_TMA(X)
 #undef X
         }
@@ -775,10 +783,16 @@ static cudaError_t launch_r2c(const flutas_plan *pl, const double *rhs, cudaStre
 }
 static cudaError_t launch_c2r(const flutas_plan *pl, double *out, double scale, cudaStream_t st, int k0, int k1) {
     const long long tile0 = (long long)k0 * pl->ny / 8, ntiles = (long long)(k1 - k0) * pl->ny / 8;
+    if (pl->xsplit && x_is_persistent(pl))
+        switch (pl->n2) {
+#define X(n) case n: return launch_c2r_tma_n<n, X_SPLIT>(pl, out, scale, st, tile0, ntiles);
+            FOR_EACH_N2_TMA(X)
+#undef X
+        }
     if (pl->xsplit)
         switch (pl->n2) {
 #define X(n) case n: return launch_r2r_inv_n<n>(pl, out, scale, st, tile0, ntiles);
-            X(8) X(16) X(32) X(64) X(128) X(256) X(512)
+            X(8) X(16) X(32)
 #undef X
         }
     if (pl->nx == 8) {
@@ -788,7 +802,7 @@ static cudaError_t launch_c2r(const flutas_plan *pl, double *out, double scale, 
     }
     if (x_is_persistent(pl))
         switch (pl->n2) {
-#define X(n) case n: return launch_c2r_tma_n<n>(pl, out, scale, st, tile0, ntiles);
+#define X(n) case n: return launch_c2r_tma_n<n, X_PERIODIC>(pl, out, scale, st, tile0, ntiles);
             FOR_EACH_N2_TMA(X)
 #undef X
         }
