@@ -664,3 +664,126 @@ done:
     free(us); free(vs); free(ws); free(rhs); free(psi);
     return rc;
 }
+
+/* ------------------------------------------------- momentum prediction (eq. 15) */
+
+/* SURVEY.md sec. 8(f) NEXT-5.  PAPER.md:148-151, eq. (15), and PAPER.md:161:
+ *     (u** - u^n) / dt = f1 M(u^n) - f2 M(u^(n-1)) + (sigma kappa delta_Gamma + rho_hat g) / rho,
+ *     f1 = 1 + dt_ratio / 2,  f2 = dt_ratio / 2  (the Adams-Bashforth coefficients of eq. (13)),
+ *     M(u) = - div(u u) + (1/rho) div[ mu (grad u + grad u^T) ]   (eq. (5); "central schemes")
+ * on the staggered grid, triply periodic, written out face by face:
+ *   convection in divergence form with arithmetic two-point means of the transported and the transporting velocity;
+ *   the stress tensor with mu = mu1 phi + mu2 (1 - phi) at cell centres (eq. 2) for the normal stresses and the mean of
+ *   the four surrounding cells at cell edges for the shear stresses; 1/rho on the face with the face density of the
+ *   projection (R2);
+ *   surface tension as the continuum surface force sigma kappa grad(phi) with kappa a given cell-centred field
+ *   (it comes from the VoF module) averaged to the face, and gravity with rho_hat = rho (no thermal
+ *   expansion): readings R18-R20 of DESIGN.md.
+ * In: u, v, w = u^n; mold_* = M(u^(n-1)).  Out: us, vs, ws = u**; mnew_* = M(u^n).  kappa may be NULL (sigma = 0). */
+static inline double mu_c(double mu1, double mu2, const double *phi, size_t q) {
+    return mu1 * phi[q] + mu2 * (1.0 - phi[q]);
+}
+
+int oracle_momentum_prediction(int nx, int ny, int nz, double lx, double ly, double lz,
+                               double rho1, double rho2, double mu1, double mu2, double sigma,
+                               double gx, double gy, double gz, double dt, double dt_ratio,
+                               const double *u, const double *v, const double *w, const double *phi, const double *kappa,
+                               const double *mold_u, const double *mold_v, const double *mold_w,
+                               double *us, double *vs, double *ws,
+                               double *mnew_u, double *mnew_v, double *mnew_w, int nthreads) {
+    grid_t g;
+    if (grid_init(&g, nx, ny, nz, lx, ly, lz, ORACLE_BC_Z_PERIODIC, rho1, rho2, dt)) return 1;
+    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(mu1 >= 0.0) || !(mu2 >= 0.0) || !(dt > 0.0) || !(dt_ratio > 0.0)) return 1;
+    const double f1 = 1.0 + 0.5 * dt_ratio, f2 = 0.5 * dt_ratio;
+    const double dx = g.dx, dy = g.dy, dz = g.dz;
+    set_threads(nthreads);
+#define AT(i, j, k) at(&g, wrap((i), nx), wrap((j), ny), wrap((k), nz))
+#define MU(i, j, k) mu_c(mu1, mu2, phi, AT(i, j, k))
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const size_t q = at(&g, i, j, k);
+                /* ------------------------------------------------ x component, east face (i+1/2, j, k) */
+                {
+                    double ue = 0.5 * (u[AT(i, j, k)] + u[AT(i + 1, j, k)]), uw = 0.5 * (u[AT(i - 1, j, k)] + u[AT(i, j, k)]);
+                    double un = 0.5 * (u[AT(i, j, k)] + u[AT(i, j + 1, k)]), us_ = 0.5 * (u[AT(i, j - 1, k)] + u[AT(i, j, k)]);
+                    double ut = 0.5 * (u[AT(i, j, k)] + u[AT(i, j, k + 1)]), ub = 0.5 * (u[AT(i, j, k - 1)] + u[AT(i, j, k)]);
+                    double vn = 0.5 * (v[AT(i, j, k)] + v[AT(i + 1, j, k)]), vs_ = 0.5 * (v[AT(i, j - 1, k)] + v[AT(i + 1, j - 1, k)]);
+                    double wt = 0.5 * (w[AT(i, j, k)] + w[AT(i + 1, j, k)]), wb = 0.5 * (w[AT(i, j, k - 1)] + w[AT(i + 1, j, k - 1)]);
+                    double conv = -((ue * ue - uw * uw) / dx + (un * vn - us_ * vs_) / dy + (ut * wt - ub * wb) / dz);
+                    double txx_e = 2.0 * MU(i + 1, j, k) * (u[AT(i + 1, j, k)] - u[AT(i, j, k)]) / dx;
+                    double txx_w = 2.0 * MU(i, j, k) * (u[AT(i, j, k)] - u[AT(i - 1, j, k)]) / dx;
+                    double mu_n = 0.25 * (MU(i, j, k) + MU(i + 1, j, k) + MU(i, j + 1, k) + MU(i + 1, j + 1, k));
+                    double mu_s = 0.25 * (MU(i, j - 1, k) + MU(i + 1, j - 1, k) + MU(i, j, k) + MU(i + 1, j, k));
+                    double mu_t = 0.25 * (MU(i, j, k) + MU(i + 1, j, k) + MU(i, j, k + 1) + MU(i + 1, j, k + 1));
+                    double mu_b = 0.25 * (MU(i, j, k - 1) + MU(i + 1, j, k - 1) + MU(i, j, k) + MU(i + 1, j, k));
+                    double txy_n = mu_n * ((u[AT(i, j + 1, k)] - u[AT(i, j, k)]) / dy + (v[AT(i + 1, j, k)] - v[AT(i, j, k)]) / dx);
+                    double txy_s = mu_s * ((u[AT(i, j, k)] - u[AT(i, j - 1, k)]) / dy + (v[AT(i + 1, j - 1, k)] - v[AT(i, j - 1, k)]) / dx);
+                    double txz_t = mu_t * ((u[AT(i, j, k + 1)] - u[AT(i, j, k)]) / dz + (w[AT(i + 1, j, k)] - w[AT(i, j, k)]) / dx);
+                    double txz_b = mu_b * ((u[AT(i, j, k)] - u[AT(i, j, k - 1)]) / dz + (w[AT(i + 1, j, k - 1)] - w[AT(i, j, k - 1)]) / dx);
+                    double rf = rho_fx(&g, phi, i, j, k);
+                    double diff = ((txx_e - txx_w) / dx + (txy_n - txy_s) / dy + (txz_t - txz_b) / dz) / rf;
+                    double src = gx;
+                    if (kappa) src += sigma * 0.5 * (kappa[AT(i, j, k)] + kappa[AT(i + 1, j, k)]) * (phi[AT(i + 1, j, k)] - phi[AT(i, j, k)]) / dx / rf;
+                    double m = conv + diff;
+                    mnew_u[q] = m;
+                    us[q] = u[q] + dt * (f1 * m - f2 * mold_u[q] + src);
+                }
+                /* ------------------------------------------------ y component, north face (i, j+1/2, k) */
+                {
+                    double vn = 0.5 * (v[AT(i, j, k)] + v[AT(i, j + 1, k)]), vs_ = 0.5 * (v[AT(i, j - 1, k)] + v[AT(i, j, k)]);
+                    double ve = 0.5 * (v[AT(i, j, k)] + v[AT(i + 1, j, k)]), vw = 0.5 * (v[AT(i - 1, j, k)] + v[AT(i, j, k)]);
+                    double vt = 0.5 * (v[AT(i, j, k)] + v[AT(i, j, k + 1)]), vb = 0.5 * (v[AT(i, j, k - 1)] + v[AT(i, j, k)]);
+                    double ue = 0.5 * (u[AT(i, j, k)] + u[AT(i, j + 1, k)]), uw = 0.5 * (u[AT(i - 1, j, k)] + u[AT(i - 1, j + 1, k)]);
+                    double wt = 0.5 * (w[AT(i, j, k)] + w[AT(i, j + 1, k)]), wb = 0.5 * (w[AT(i, j, k - 1)] + w[AT(i, j + 1, k - 1)]);
+                    double conv = -((ve * ue - vw * uw) / dx + (vn * vn - vs_ * vs_) / dy + (vt * wt - vb * wb) / dz);
+                    double tyy_n = 2.0 * MU(i, j + 1, k) * (v[AT(i, j + 1, k)] - v[AT(i, j, k)]) / dy;
+                    double tyy_s = 2.0 * MU(i, j, k) * (v[AT(i, j, k)] - v[AT(i, j - 1, k)]) / dy;
+                    double mu_e = 0.25 * (MU(i, j, k) + MU(i + 1, j, k) + MU(i, j + 1, k) + MU(i + 1, j + 1, k));
+                    double mu_w = 0.25 * (MU(i - 1, j, k) + MU(i, j, k) + MU(i - 1, j + 1, k) + MU(i, j + 1, k));
+                    double mu_t = 0.25 * (MU(i, j, k) + MU(i, j + 1, k) + MU(i, j, k + 1) + MU(i, j + 1, k + 1));
+                    double mu_b = 0.25 * (MU(i, j, k - 1) + MU(i, j + 1, k - 1) + MU(i, j, k) + MU(i, j + 1, k));
+                    double tyx_e = mu_e * ((v[AT(i + 1, j, k)] - v[AT(i, j, k)]) / dx + (u[AT(i, j + 1, k)] - u[AT(i, j, k)]) / dy);
+                    double tyx_w = mu_w * ((v[AT(i, j, k)] - v[AT(i - 1, j, k)]) / dx + (u[AT(i - 1, j + 1, k)] - u[AT(i - 1, j, k)]) / dy);
+                    double tyz_t = mu_t * ((v[AT(i, j, k + 1)] - v[AT(i, j, k)]) / dz + (w[AT(i, j + 1, k)] - w[AT(i, j, k)]) / dy);
+                    double tyz_b = mu_b * ((v[AT(i, j, k)] - v[AT(i, j, k - 1)]) / dz + (w[AT(i, j + 1, k - 1)] - w[AT(i, j, k - 1)]) / dy);
+                    double rf = rho_fy(&g, phi, i, j, k);
+                    double diff = ((tyx_e - tyx_w) / dx + (tyy_n - tyy_s) / dy + (tyz_t - tyz_b) / dz) / rf;
+                    double src = gy;
+                    if (kappa) src += sigma * 0.5 * (kappa[AT(i, j, k)] + kappa[AT(i, j + 1, k)]) * (phi[AT(i, j + 1, k)] - phi[AT(i, j, k)]) / dy / rf;
+                    double m = conv + diff;
+                    mnew_v[q] = m;
+                    vs[q] = v[q] + dt * (f1 * m - f2 * mold_v[q] + src);
+                }
+                /* ------------------------------------------------ z component, top face (i, j, k+1/2) */
+                {
+                    double wt = 0.5 * (w[AT(i, j, k)] + w[AT(i, j, k + 1)]), wb = 0.5 * (w[AT(i, j, k - 1)] + w[AT(i, j, k)]);
+                    double we = 0.5 * (w[AT(i, j, k)] + w[AT(i + 1, j, k)]), ww = 0.5 * (w[AT(i - 1, j, k)] + w[AT(i, j, k)]);
+                    double wn = 0.5 * (w[AT(i, j, k)] + w[AT(i, j + 1, k)]), ws_ = 0.5 * (w[AT(i, j - 1, k)] + w[AT(i, j, k)]);
+                    double ue = 0.5 * (u[AT(i, j, k)] + u[AT(i, j, k + 1)]), uw = 0.5 * (u[AT(i - 1, j, k)] + u[AT(i - 1, j, k + 1)]);
+                    double vn = 0.5 * (v[AT(i, j, k)] + v[AT(i, j, k + 1)]), vs_ = 0.5 * (v[AT(i, j - 1, k)] + v[AT(i, j - 1, k + 1)]);
+                    double conv = -((we * ue - ww * uw) / dx + (wn * vn - ws_ * vs_) / dy + (wt * wt - wb * wb) / dz);
+                    double tzz_t = 2.0 * MU(i, j, k + 1) * (w[AT(i, j, k + 1)] - w[AT(i, j, k)]) / dz;
+                    double tzz_b = 2.0 * MU(i, j, k) * (w[AT(i, j, k)] - w[AT(i, j, k - 1)]) / dz;
+                    double mu_e = 0.25 * (MU(i, j, k) + MU(i + 1, j, k) + MU(i, j, k + 1) + MU(i + 1, j, k + 1));
+                    double mu_w = 0.25 * (MU(i - 1, j, k) + MU(i, j, k) + MU(i - 1, j, k + 1) + MU(i, j, k + 1));
+                    double mu_n = 0.25 * (MU(i, j, k) + MU(i, j + 1, k) + MU(i, j, k + 1) + MU(i, j + 1, k + 1));
+                    double mu_s = 0.25 * (MU(i, j - 1, k) + MU(i, j, k) + MU(i, j - 1, k + 1) + MU(i, j, k + 1));
+                    double tzx_e = mu_e * ((w[AT(i + 1, j, k)] - w[AT(i, j, k)]) / dx + (u[AT(i, j, k + 1)] - u[AT(i, j, k)]) / dz);
+                    double tzx_w = mu_w * ((w[AT(i, j, k)] - w[AT(i - 1, j, k)]) / dx + (u[AT(i - 1, j, k + 1)] - u[AT(i - 1, j, k)]) / dz);
+                    double tzy_n = mu_n * ((w[AT(i, j + 1, k)] - w[AT(i, j, k)]) / dy + (v[AT(i, j, k + 1)] - v[AT(i, j, k)]) / dz);
+                    double tzy_s = mu_s * ((w[AT(i, j, k)] - w[AT(i, j - 1, k)]) / dy + (v[AT(i, j - 1, k + 1)] - v[AT(i, j - 1, k)]) / dz);
+                    double rf = rho_fz(&g, phi, i, j, k);
+                    double diff = ((tzx_e - tzx_w) / dx + (tzy_n - tzy_s) / dy + (tzz_t - tzz_b) / dz) / rf;
+                    double src = gz;
+                    if (kappa) src += sigma * 0.5 * (kappa[AT(i, j, k)] + kappa[AT(i, j, k + 1)]) * (phi[AT(i, j, k + 1)] - phi[AT(i, j, k)]) / dz / rf;
+                    double m = conv + diff;
+                    mnew_w[q] = m;
+                    ws[q] = w[q] + dt * (f1 * m - f2 * mold_w[q] + src);
+                }
+            }
+#undef AT
+#undef MU
+    return 0;
+}

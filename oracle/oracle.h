@@ -147,6 +147,19 @@ int oracle_projection_step_bc(int nx, int ny, int nz, double lx, double ly, doub
                               double *u, double *v, double *w, const double *phi,
                               double *p, const double *p_old, double *rhs_out, int nthreads);
 
+/* ---- momentum prediction, eq. (15) (eq. (5)), triply
+ * periodic:  u** = u^n + dt [ (1 + r/2) M(u^n) - (r/2) M(u^(n-1)) + g + sigma kappa grad(phi) / rho_f ],  r = dt_ratio,
+ * M(u) = -div(u u) + (1/rho_f) div[ mu (grad u + grad u^T) ], central differences on the staggered grid, mu = mu1 phi +
+ * mu2 (1 - phi) (see oracle.c for every face formula).  In: u, v, w = u^n, mold_* = M(u^(n-1)), kappa (nullable) the
+ * cell-centred curvature.  Out: us, vs, ws = u**, mnew_* = M(u^n).  No array may alias another. */
+int oracle_momentum_prediction(int nx, int ny, int nz, double lx, double ly, double lz,
+                               double rho1, double rho2, double mu1, double mu2, double sigma,
+                               double gx, double gy, double gz, double dt, double dt_ratio,
+                               const double *u, const double *v, const double *w, const double *phi, const double *kappa,
+                               const double *mold_u, const double *mold_v, const double *mold_w,
+                               double *us, double *vs, double *ws,
+                               double *mnew_u, double *mnew_v, double *mnew_w, int nthreads);
+
 /* number of OpenMP threads a call with this nthreads argument would use */
 int oracle_threads(int nthreads);
 

@@ -41,6 +41,8 @@ _lib.oracle_projection_step_bc.argtypes = _GRID3 + [_cd, _cd, _cd, _cd] + [_dp] 
 for _f in ("oracle_r2r_axis", "oracle_eigenvalues", "oracle_divergence_bc", "oracle_laplacian_bc", "oracle_poisson_bc",
            "oracle_rhs_bc", "oracle_correction_bc", "oracle_projection_step_bc"):
     getattr(_lib, _f).restype = _ci
+_lib.oracle_momentum_prediction.argtypes = [_ci, _ci, _ci, _cd, _cd, _cd] + [_cd] * 10 + [_dp] * 14 + [_ci]
+_lib.oracle_momentum_prediction.restype = _ci
 _lib.oracle_threads.argtypes = [_ci]
 for _f in ("oracle_rhs_vdt", "oracle_projection_step_vdt", "oracle_rhs", "oracle_poisson", "oracle_projection_step", "oracle_projection_step_paper",
            "oracle_dft_axis", "oracle_divergence", "oracle_laplacian", "oracle_threads"):
@@ -243,3 +245,20 @@ def projection_step_bc(u, v, w, phi, p, p_old, box, bc, rho1, rho2, dt, nthreads
                                           _p(phi), _p(p), _p(p_old), _p(r) if return_rhs else None, nthreads),
            "oracle_projection_step_bc")
     return (u, v, w, p, r) if return_rhs else (u, v, w, p)
+
+
+def momentum_prediction(u, v, w, phi, kappa, m_old, box, rho1, rho2, mu1, mu2, sigma, grav, dt, dt_ratio=1.0, nthreads=0):
+    """eq. (15), triply periodic.  m_old = (Mu, Mv, Mw) of the previous step; kappa may be None.
+    Returns (u**, v**, w**), (Mu, Mv, Mw) of this step."""
+    u = _field(u)
+    v, w, phi = (_field(a, u.shape) for a in (v, w, phi))
+    mo = [_field(a, u.shape) for a in m_old]
+    kap = None if kappa is None else _field(kappa, u.shape)
+    out = [np.empty_like(u) for _ in range(6)]
+    nz, ny, nx = u.shape
+    _check(_lib.oracle_momentum_prediction(nx, ny, nz, float(box[0]), float(box[1]), float(box[2]), rho1, rho2, mu1, mu2,
+                                           sigma, float(grav[0]), float(grav[1]), float(grav[2]), dt, float(dt_ratio),
+                                           _p(u), _p(v), _p(w), _p(phi), None if kap is None else _p(kap),
+                                           *[_p(a) for a in mo], *[_p(a) for a in out], nthreads),
+           "oracle_momentum_prediction")
+    return tuple(out[:3]), tuple(out[3:])
