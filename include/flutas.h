@@ -147,6 +147,39 @@ int flutas_projection_step_host(flutas_plan *plan, double *u_host, double *v_hos
                                 const double *phi_host, double *p_host, const double *p_old_host,
                                 double dt, void *stream);
 
+/* One whole velocity / pressure update: the momentum prediction of eq. (15) fused with the projection step
+ * (Algorithm 1 lines 10-13):
+ *     u** = u^n + dt [ (1 + r/2) M(u^n) - (r/2) M(u^(n-1)) + g + sigma kappa grad(phi) / rho_f ],   r = dt_ratio
+ *     M(u) = - div(u u) + (1/rho_f) div[ mu (grad u + grad u^T) ],  mu = mu1 phi + mu2 (1 - phi)     (eqs. 5, 15, 2)
+ * (central differences on the staggered grid: divergence-form convection with two-point means, normal stresses with
+ * the cell viscosity, shear stresses with the mean viscosity of the four cells around an edge, 1/rho on the face with
+ * the face density of the projection; surface tension as the continuum surface force with a given cell-centred
+ * curvature field; gravity with rho_hat = rho: DESIGN.md R18-R20), then exactly flutas_projection_step_ex on u**.
+ * ONE kernel forms u**, the splitting terms and the right-hand side, so u** never travels through HBM.
+ *   in : u, v, w = u^n;  phi = phi^(n+1);  kappa = curvature at cell centres, or NULL (no surface tension);
+ *        p = p^n, p_old = p^(n-1);  m_old_* = M(u^(n-1)) (zeros and dt_ratio = ... for an Euler start: pass M(u^n) itself,
+ *        i.e. call once with any m_old and feed m_new back: f1 - f2 = 1);  mu1, mu2 >= 0, sigma, g: plain numbers.
+ *   out: u, v, w = u^(n+1) in place;  p_out = p^(n+1) (may be p or p_old, as in flutas_projection_step_ex);
+ *        m_new_* = M(u^n) (the caller swaps the two sets for the next step).
+ * Triply periodic plans with nx a multiple of 32 only (FLUTAS_ERR_UNSUPPORTED_SIZE otherwise).  All arrays are N doubles on
+ * the device, 16-byte aligned, pairwise distinct except p_out.  Enqueues on `stream`, no synchronisation. */
+int flutas_time_step(flutas_plan *plan, double *u, double *v, double *w, const double *phi, const double *kappa,
+                     const double *p, const double *p_old, double *p_out,
+                     const double *m_old_u, const double *m_old_v, const double *m_old_w,
+                     double *m_new_u, double *m_new_v, double *m_new_w,
+                     double mu1, double mu2, double sigma, double gx, double gy, double gz,
+                     double dt, double dt_ratio, void *stream);
+
+/* The first kernel of flutas_time_step alone (kernel-level parity tests): us/vs/ws_out = u' = u** + the splitting term
+ * (u** itself when p == NULL: no splitting terms), rhs_out = rho0/dt div(u'), m_new_* = M(u^n).  Inputs are not modified. */
+int flutas_momentum_rhs(flutas_plan *plan, const double *u, const double *v, const double *w, const double *phi,
+                        const double *kappa, const double *p, const double *p_old,
+                        const double *m_old_u, const double *m_old_v, const double *m_old_w,
+                        double *m_new_u, double *m_new_v, double *m_new_w,
+                        double mu1, double mu2, double sigma, double gx, double gy, double gz,
+                        double dt, double dt_ratio, double *us_out, double *vs_out, double *ws_out, double *rhs_out,
+                        void *stream);
+
 /* NULL is a no-op.  Frees every device and host resource of the plan (synchronises the device). */
 void flutas_plan_destroy(flutas_plan *plan);
 

@@ -28,6 +28,10 @@ lib.flutas_plan_set_workspace.argtypes = [_vp, _vp, ctypes.c_size_t]
 lib.flutas_plan_set_workspace.restype = _ci
 lib.flutas_plan_kernel_symbol.argtypes = [_vp, _ci]
 lib.flutas_plan_kernel_symbol.restype = ctypes.c_char_p
+lib.flutas_time_step.argtypes = [_vp] * 15 + [_cd] * 8 + [_vp]
+lib.flutas_time_step.restype = _ci
+lib.flutas_momentum_rhs.argtypes = [_vp] * 14 + [_cd] * 8 + [_vp] * 5
+lib.flutas_momentum_rhs.restype = _ci
 lib.flutas_plan_destroy.argtypes = [_vp]
 lib.flutas_plan_destroy.restype = None
 lib.flutas_projection_step.argtypes = [_vp] * 7 + [_cd, _vp]
@@ -68,6 +72,7 @@ EXPORTS = [
     "flutas_plan_set_timing", "flutas_plan_read_timing", "flutas_plan_kernel_bytes", "flutas_plan_set_option",
     "flutas_projection_step_ex", "flutas_splitting_rhs_ex",
     "flutas_plan_create_ex", "flutas_workspace_bytes", "flutas_plan_set_workspace", "flutas_plan_kernel_symbol",
+    "flutas_time_step", "flutas_momentum_rhs",
 ]
 
 
@@ -169,6 +174,24 @@ class Plan:
         ptrs = [_dev_ptr(t, self.npts) for t in (u, v, w, phi, p, p_old)]
         _check(lib.flutas_splitting_rhs_ex(self._h, *ptrs, float(dt), float(dt_ratio),
                                            _dev_ptr(rhs_out, self.npts), _stream() if stream is None else stream))
+
+    # --- momentum prediction (eq. 15) fused with the projection: one velocity / pressure update
+    def time_step(self, u, v, w, phi, kappa, p, p_old, p_out, m_old, m_new, mu1, mu2, sigma, grav, dt, dt_ratio=1.0, stream=None):
+        """u, v, w in place; m_old / m_new: 3-tuples of tensors (M of the previous / this step); kappa may be None"""
+        ptrs = [_dev_ptr(t, self.npts) for t in (u, v, w, phi)] + [None if kappa is None else _dev_ptr(kappa, self.npts)]
+        ptrs += [_dev_ptr(t, self.npts) for t in (p, p_old, p_out, *m_old, *m_new)]
+        _check(lib.flutas_time_step(self._h, *ptrs, float(mu1), float(mu2), float(sigma), float(grav[0]), float(grav[1]),
+                                    float(grav[2]), float(dt), float(dt_ratio), _stream() if stream is None else stream))
+
+    def momentum_rhs(self, u, v, w, phi, kappa, p, p_old, m_old, m_new, mu1, mu2, sigma, grav, dt, dt_ratio, us, vs, ws, rhs,
+                     stream=None):
+        """the first kernel of time_step alone; p = p_old = None gives u** without the splitting terms"""
+        opt = lambda t: None if t is None else _dev_ptr(t, self.npts)
+        ptrs = [_dev_ptr(t, self.npts) for t in (u, v, w, phi)] + [opt(kappa), opt(p), opt(p_old)]
+        ptrs += [_dev_ptr(t, self.npts) for t in (*m_old, *m_new)]
+        outs = [_dev_ptr(t, self.npts) for t in (us, vs, ws, rhs)]
+        _check(lib.flutas_momentum_rhs(self._h, *ptrs, float(mu1), float(mu2), float(sigma), float(grav[0]), float(grav[1]),
+                                       float(grav[2]), float(dt), float(dt_ratio), *outs, _stream() if stream is None else stream))
 
     # --- the step for host arrays (numpy float64 or pinned torch CPU tensors), in place, synchronous
     def projection_step_host(self, u, v, w, phi, p, p_old, dt, stream=None):

@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "kernels_momentum.cuh"
 #include "kernels_r2r.cuh"
 #include "kernels_rhs.cuh"
 #include "kernels_thomas.cuh"
@@ -1087,6 +1088,91 @@ extern "C" int flutas_projection_step_ex(flutas_plan *pl, double *u, double *v, 
         CUDA_TRY(cudaStreamWaitEvent(st, pl->ev_fork, 0));
     }
     if (chunk != nz) { tm.mark(); tm.mark(); }
+    tm.mark();
+    tm.done();
+    return FLUTAS_OK;
+}
+
+// ---- momentum prediction fused with the splitting right-hand side (kernels_momentum.cuh), and the whole update
+static int enqueue_momentum(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
+                            const double *kappa, const double *p, const double *po, const double *const *m_old,
+                            double *const *m_new, const double *prm /* mu1 mu2 sigma gx gy gz */, double dt, double dt_ratio,
+                            double *us, double *vs, double *ws, double *rhs, cudaStream_t st) {
+    GridParams g = pl->grid;
+    g.c_pn = 1.0 + dt_ratio;
+    g.c_po = dt_ratio;
+    MomentumParams mp{prm[0], prm[1], prm[2], prm[3], prm[4], prm[5], 1.0 + 0.5 * dt_ratio, 0.5 * dt_ratio, kappa ? 1 : 0, p ? 1 : 0};
+    const int kc = pl->nz < 32 ? pl->nz : 32;
+    const dim3 block(MomTile::TX, MomTile::TY), grid(pl->nx / MomTile::TX, pl->ny / MomTile::TY, (pl->nz + kc - 1) / kc);
+    momentum_rhs_kernel<<<grid, block, 0, st>>>(g, mp, dt, kc, u, v, w, phi, kappa, p, po, m_old[0], m_old[1], m_old[2],
+                                                m_new[0], m_new[1], m_new[2], rhs, us, vs, ws);
+    return check_launch(cudaGetLastError(), "momentum_rhs");
+}
+
+static int check_momentum_args(const flutas_plan *pl, double mu1, double mu2, double sigma, double gx, double gy, double gz,
+                               double dt, double dt_ratio) {
+    if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
+    if (pl->bc[0] != FLUTAS_BC_PERIODIC || pl->bc[1] != FLUTAS_BC_PERIODIC || pl->bc[2] != FLUTAS_BC_PERIODIC ||
+        pl->nx % MomTile::TX != 0 || pl->ny % MomTile::TY != 0)
+        return fail(FLUTAS_ERR_UNSUPPORTED_SIZE, "the momentum prediction takes triply periodic plans with nx a multiple of 32");
+    if (!(dt > 0.0) || !std::isfinite(dt) || !(dt_ratio > 0.0) || !std::isfinite(dt_ratio))
+        return fail(FLUTAS_ERR_INVALID_ARG, "dt and dt_ratio must be positive and finite");
+    if (!(mu1 >= 0.0) || !(mu2 >= 0.0) || !std::isfinite(mu1 + mu2 + sigma + gx + gy + gz))
+        return fail(FLUTAS_ERR_INVALID_ARG, "viscosities must be non-negative; sigma and g finite");
+    if (!pl->ws_base) return fail(FLUTAS_ERR_INVALID_ARG, "the plan has no workspace (flutas_plan_set_workspace)");
+    return FLUTAS_OK;
+}
+
+extern "C" int flutas_momentum_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
+                                   const double *kappa, const double *p, const double *p_old, const double *m_old_u,
+                                   const double *m_old_v, const double *m_old_w, double *m_new_u, double *m_new_v,
+                                   double *m_new_w, double mu1, double mu2, double sigma, double gx, double gy, double gz,
+                                   double dt, double dt_ratio, double *us_out, double *vs_out, double *ws_out,
+                                   double *rhs_out, void *stream) {
+    if (int rc = check_momentum_args(pl, mu1, mu2, sigma, gx, gy, gz, dt, dt_ratio)) return rc;
+    if ((p == nullptr) != (p_old == nullptr)) return fail(FLUTAS_ERR_INVALID_ARG, "p and p_old must both be given or both be NULL");
+    const void *ptrs[17] = {u, v, w, phi, m_old_u, m_old_v, m_old_w, m_new_u, m_new_v, m_new_w, us_out, vs_out, ws_out, rhs_out, kappa, p, p_old};
+    int n = 14;
+    if (kappa) ptrs[n++] = kappa;
+    if (p) { ptrs[n++] = p; ptrs[n++] = p_old; }
+    if (int rc = check_fields(pl, ptrs, n)) return rc;
+    const double *mo[3] = {m_old_u, m_old_v, m_old_w};
+    double *mn[3] = {m_new_u, m_new_v, m_new_w};
+    const double prm[6] = {mu1, mu2, sigma, gx, gy, gz};
+    return enqueue_momentum(pl, u, v, w, phi, kappa, p, p_old, mo, mn, prm, dt, dt_ratio, us_out, vs_out, ws_out, rhs_out,
+                            (cudaStream_t)stream);
+}
+
+extern "C" int flutas_time_step(flutas_plan *pl, double *u, double *v, double *w, const double *phi, const double *kappa,
+                                const double *p, const double *p_old, double *p_out, const double *m_old_u,
+                                const double *m_old_v, const double *m_old_w, double *m_new_u, double *m_new_v,
+                                double *m_new_w, double mu1, double mu2, double sigma, double gx, double gy, double gz,
+                                double dt, double dt_ratio, void *stream) {
+    if (int rc = check_momentum_args(pl, mu1, mu2, sigma, gx, gy, gz, dt, dt_ratio)) return rc;
+    const void *ptrs[14] = {u, v, w, phi, p, p_old, m_old_u, m_old_v, m_old_w, m_new_u, m_new_v, m_new_w, kappa, p_out};
+    int n = 12;
+    if (kappa) ptrs[n++] = kappa;
+    if (p_out != p && p_out != p_old) ptrs[n++] = p_out;
+    if (!p_out) return fail(FLUTAS_ERR_INVALID_ARG, "NULL field pointer (p_out)");
+    if (int rc = check_fields(pl, ptrs, n)) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    StepTimer tm(pl, st);
+    const double *mo[3] = {m_old_u, m_old_v, m_old_w};
+    double *mn[3] = {m_new_u, m_new_v, m_new_w};
+    const double prm[6] = {mu1, mu2, sigma, gx, gy, gz};
+    tm.mark();
+    if (int rc = enqueue_momentum(pl, u, v, w, phi, kappa, p, p_old, mo, mn, prm, dt, dt_ratio, pl->up, pl->vp, pl->wp, pl->rhs, st)) return rc;
+    tm.mark();
+    if (int rc = check_launch(launch_r2c(pl, pl->rhs, st, 0, pl->nz), "fft_x_r2c")) return rc;
+    tm.mark();
+    if (int rc = enqueue_y<MODE_FWD>(pl, st, 0, pl->nz)) return rc;
+    tm.mark();
+    if (int rc = enqueue_z(pl, st, &tm)) return rc;
+    if (int rc = enqueue_y<MODE_INV>(pl, st, 0, pl->nz)) return rc;
+    tm.mark();
+    if (int rc = check_launch(launch_c2r(pl, p_out, norm_scale(pl), st, 0, pl->nz), "fft_x_c2r")) return rc;
+    tm.mark();
+    if (int rc = enqueue_correction(pl, dt, p_out, u, v, w, st, 0, pl->nz)) return rc;
     tm.mark();
     tm.done();
     return FLUTAS_OK;
