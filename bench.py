@@ -8,6 +8,7 @@ batch of synthetic input.  Workloads (BASELINE.json `metric` names both):
   cfg4  512^3 triply periodic, box (2 pi)^3, drops at 5 % volume fraction, rho2/rho1 = 50   [primary line]
   cfg5  1024 x 1024 x 512 wall-bounded, box 4 x 4 x 1, two-layer, rho2/rho1 = 1000          [under "also"]
   cavity 512 x 512 x 256 closed box, walls in x, y, z (cosine expansions; NEXT-2)           [under "also"]
+  cfg4ts the cfg4 fields through flutas_time_step (momentum prediction fused in; NEXT-5)    [under "also"]
 N > 1 (torchrun): N independent replicas, one per GPU, no data-path collective ("replicas only").
 Prints ONE JSON line on rank 0.  --impl reference times the CPU oracle (tests' ground truth) on the same workload
 (one or two steps of the full 512^3 box); it is a deliberately slow baseline, not a target.
@@ -31,6 +32,9 @@ WORKLOAD_DESC = {
     "cfg5": "cfg5: 1024x1024x512 wall-bounded (Neumann p, Thomas in z), box 4x4x1, two-layer, rho2/rho1=1000, dt=1e-3",
     "cavity": "cavity: 512x512x256 closed box, walls (Neumann p, no-slip) in x, y and z: cosine expansions in x, y + Thomas in z "
               "(PAPER.md:287 shape, extruded; SURVEY sec. 8(f) NEXT-2), two-layer, rho2/rho1=5, dt=1e-3",
+    "cfg4ts": "cfg4ts: the cfg4 fields (512^3 triply periodic, rho2/rho1=50) through flutas_time_step: momentum prediction "
+              "(eq. 15: mu2/mu1=15, surface tension with a synthetic curvature field, gravity) fused with the projection "
+              "(SURVEY sec. 8(f) NEXT-5)",
     "cfg2": "cfg2: 128^3 triply periodic emulsion-shaped (small case)",
     "cfg3": "cfg3: 256x256x128 wall-bounded two-layer (small case)",
 }
@@ -38,7 +42,7 @@ WORKLOAD_DESC = {
 
 def make_workload(name, ratio=None):
     import workloads as wl          # top-level module: loads neither the CUDA library nor the oracle
-    if name == "cfg4":
+    if name in ("cfg4", "cfg4ts"):
         return wl.config4(512, 50.0 if ratio is None else ratio)
     if name == "cfg5":
         return wl.config5()
@@ -142,9 +146,29 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     host = list(W.fields())
     dev = [torch.from_numpy(a).cuda() for a in host]
     torch.cuda.synchronize()
+    timestep = name.endswith("ts")
+    if timestep:
+        # whole velocity / pressure update: seven more resident fields (curvature, M of two time levels); the velocity
+        # stays bounded over the timed steps because every step ends with the projection
+        gen = torch.Generator(device="cuda").manual_seed(5)
+        kappa = torch.randn(dev[0].shape, dtype=torch.float64, device="cuda", generator=gen)
+        kappa *= 0.1
+        mbuf = [torch.zeros_like(dev[0]) for _ in range(6)]
+        state = {"flip": 0}
+
+        def one_step():
+            # a real time loop: M and p ping-pong (p^(n+1) is written over p^(n-1), then the roles swap)
+            f = state["flip"]
+            a, b = (mbuf[:3], mbuf[3:]) if f == 0 else (mbuf[3:], mbuf[:3])
+            pn, po = (dev[4], dev[5]) if f == 0 else (dev[5], dev[4])
+            state["flip"] ^= 1
+            plan.time_step(dev[0], dev[1], dev[2], dev[3], kappa, pn, po, po, a, b, 0.01, 0.15, 0.05, (0.0, 0.0, -1.0), 1e-4)
+    else:
+        def one_step():
+            plan.projection_step(*dev, W.dt)
 
     for _ in range(args.warmup):
-        plan.projection_step(*dev, W.dt)
+        one_step()
     torch.cuda.synchronize()
     # ---- the headline: K steps back to back, per-kernel event recording OFF, one event pair around them
     sampler = ClockSampler(visible_gpu_index(local_rank))
@@ -154,7 +178,7 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     sampler.start()
     ev0.record()
     for _ in range(args.steps):
-        plan.projection_step(*dev, W.dt)
+        one_step()
     ev1.record()
     torch.cuda.synchronize()
     replicas.barrier()
@@ -166,16 +190,19 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     kv0, kv1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     kv0.record()
     for _ in range(k_steps):
-        plan.projection_step(*dev, W.dt)
+        one_step()
     kv1.record()
     torch.cuda.synchronize()
     kms, ksteps = plan.read_timing()
     plan.set_timing(False)
     instrumented_ms = kv0.elapsed_time(kv1) / k_steps
-    finite = bool(torch.isfinite(dev[4]).all().item() and torch.isfinite(dev[0]).all().item())
+    finite = bool(torch.isfinite(dev[4]).all().item() and torch.isfinite(dev[5]).all().item() and torch.isfinite(dev[0]).all().item())
     units, ms = replicas.aggregate_throughput(float(W.npts) * args.steps, ms_local)
 
     names, kbytes = plan.kernel_names, plan.kernel_bytes
+    if timestep:     # the first kernel is the fused prediction: reads u, v, w, phi, kappa, p, p_old, M_old (3); writes M (3), u', v', w', rhs
+        names = ["momentum_rhs"] + names[1:]
+        kbytes = [17 * 8.0 * W.npts] + kbytes[1:]
     kernels = []
     for n_, b_, t_ in zip(names, kbytes, kms):
         avg = t_ / max(ksteps, 1)
@@ -184,7 +211,7 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     dom = max(kernels, key=lambda k: k["ms"])
     # DRAM bytes of the dominant kernel from the committed ncu capture -- only if that capture is of the kernel
     # that ran here (same device symbol); a stale capture gives null instead of a wrong number
-    symbols = dict(zip(names, plan.kernel_symbols))
+    symbols = dict(zip(names, (["momentum_rhs_kernel"] + plan.kernel_symbols[1:]) if timestep else plan.kernel_symbols))
     tr = traffic.get(name, {}).get(dom["name"])
     if traffic.get("_symbols", {}).get(name, {}).get(dom["name"]) != symbols[dom["name"]]:
         tr = None
@@ -196,6 +223,8 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     step_ms = ms_local / args.steps
     model_bytes = sum(kbytes)
     step = {"ms": round(step_ms, 4), "model_bytes_per_pt": round(model_bytes / W.npts, 1), "min_bytes_per_pt": 80,
+            "min_bytes_note": "80 B/pt = north_star's minimum for the projection step alone" if not timestep else
+                              "the whole update reads 10 and writes 7 more fields than that minimum counts",
             "model_gbs": round(model_bytes / (step_ms * 1e-3) / 1e9, 1),
             "frac_of_peak_model_bytes": round(model_bytes / (step_ms * 1e-3) / 1e9 / peak_gbs, 4),
             "frac_of_peak_min_bytes": round(80.0 * W.npts / (step_ms * 1e-3) / 1e9 / peak_gbs, 4),
@@ -224,7 +253,7 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
         del fresh
         torch.cuda.empty_cache()
 
-    if with_e2e:
+    if with_e2e and not timestep:
         # end to end through the host entry point of the C ABI: pinned host buffers, H2D of the six inputs
         # and D2H of u, v, w, p inside the timed region, every step
         e_steps = max(1, min(args.steps, args.e2e_steps))
@@ -394,7 +423,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workloads", default="cfg4,cfg5,cavity")
+    ap.add_argument("--workloads", default="cfg4,cfg5,cavity,cfg4ts")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-all", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

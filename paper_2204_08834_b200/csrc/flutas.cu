@@ -1103,7 +1103,7 @@ static int enqueue_momentum(flutas_plan *pl, const double *u, const double *v, c
     g.c_po = dt_ratio;
     MomentumParams mp{prm[0], prm[1], prm[2], prm[3], prm[4], prm[5], 1.0 + 0.5 * dt_ratio, 0.5 * dt_ratio, kappa ? 1 : 0, p ? 1 : 0};
     const int kc = pl->nz < 32 ? pl->nz : 32;
-    const dim3 block(MomTile::TX, MomTile::TY), grid(pl->nx / MomTile::TX, pl->ny / MomTile::TY, (pl->nz + kc - 1) / kc);
+    const dim3 block(MomTile::TX, MomTile::TY + 1), grid(pl->nx / MomTile::TX, pl->ny / MomTile::TY, (pl->nz + kc - 1) / kc);
     momentum_rhs_kernel<<<grid, block, 0, st>>>(g, mp, dt, kc, u, v, w, phi, kappa, p, po, m_old[0], m_old[1], m_old[2],
                                                 m_new[0], m_new[1], m_new[2], rhs, us, vs, ws);
     return check_launch(cudaGetLastError(), "momentum_rhs");

@@ -13,9 +13,9 @@
 //
 // Triply periodic.  A block owns a tile of 32 x 8 cells and marches in z.  Per plane it evaluates the face values u' on
 // 33 x 8 east faces (its own and the column to the west), v' on 32 x 9 north faces (its own and the row to the south)
-// and w' on its 32 x 8 top faces as three lists of work items spread over the 256 threads (the halo costs one extra
-// item for 8 (u) and 32 (v) threads instead of a divergent second pass in every warp), leaves them in shared memory, and
-// then every thread takes the divergence of its cell; w' of the plane below stays in shared memory from the previous
+// and w' on its 32 x 8 top faces as three lists of work items spread over 32 x 9 = 288 threads (one round per list: the
+// halo costs a ninth warp instead of a second, almost empty round in every warp), leaves them in shared memory, and
+// then the first 256 threads take the divergence of their cells; w' of the plane below stays in shared memory from the previous
 // step.  Operands come through L1 / L2 (read-only path): this is the first, plain form of the kernel.
 #pragma once
 #include "kernels.cuh"
@@ -29,7 +29,7 @@ struct MomentumParams {
 };
 
 struct MomTile {
-    static constexpr int TX = 32, TY = 8, NT = TX * TY;
+    static constexpr int TX = 32, TY = 8, NT = TX * (TY + 1);   // one more row of threads than cells: every item list fits in ONE round
 };
 
 // everything one face evaluation needs to find its neighbours: wrapped indices around (i, j, k)
@@ -110,7 +110,7 @@ face_component(const double *__restrict__ a, const double *__restrict__ b, const
     return o;
 }
 
-__global__ void __launch_bounds__(MomTile::NT, 2)
+__global__ void __launch_bounds__(MomTile::NT, 3)
 momentum_rhs_kernel(GridParams g, MomentumParams mp, double dt, int kc, const double *__restrict__ u, const double *__restrict__ v,
                     const double *__restrict__ w, const double *__restrict__ phi, const double *__restrict__ kappa,
                     const double *__restrict__ p, const double *__restrict__ po, const double *__restrict__ mu_old,
@@ -143,6 +143,7 @@ momentum_rhs_kernel(GridParams g, MomentumParams mp, double dt, int kc, const do
         if (jj >= 0) { mv_new[n.c] = o.m; vp[n.c] = o.up; }
     };
     auto do_w = [&](int k, int slot, bool store) {
+        if (threadIdx.y >= T::TY) return;
         const int kk = k < 0 ? g.nz - 1 : k;
         const Nbr n = neighbours(g, x0 + threadIdx.x, j0 + threadIdx.y, kk);
         const FaceOut o = face_component(w, u, v, phi, kappa, p, po, mw_old, n.c, AxisOff{n.zm, n.zp, n.zpp}, AxisOff{n.xm, n.xp, n.xpp},
@@ -156,14 +157,16 @@ momentum_rhs_kernel(GridParams g, MomentumParams mp, double dt, int kc, const do
     do_w(k0 - 1, 0, false);                       // top faces of the plane below the chunk
     int cur = 1;
     for (int k = k0; k < k1; ++k, cur ^= 1) {
-        for (int item = tid; item < (T::TX + 1) * T::TY; item += T::NT) do_u(item, k);
-        for (int item = tid; item < T::TX * (T::TY + 1); item += T::NT) do_v(item, k);
+        if (tid < (T::TX + 1) * T::TY) do_u(tid, k);
+        do_v(tid, k);                              // 32 x 9 items = all threads
         do_w(k, cur, true);
         __syncthreads();
         const int tx = threadIdx.x, ty = threadIdx.y;
-        const long long q = (x0 + tx) + (long long)g.nx * ((j0 + ty) + (long long)g.ny * k);
-        rhs[q] = c_div * ((su[ty][tx + 1] - su[ty][tx]) * g.inv_dx + (sv[ty + 1][tx] - sv[ty][tx]) * g.inv_dy +
-                          (sw[cur][ty][tx] - sw[cur ^ 1][ty][tx]) * g.inv_dz);
+        if (ty < T::TY) {
+            const long long q = (x0 + tx) + (long long)g.nx * ((j0 + ty) + (long long)g.ny * k);
+            rhs[q] = c_div * ((su[ty][tx + 1] - su[ty][tx]) * g.inv_dx + (sv[ty + 1][tx] - sv[ty][tx]) * g.inv_dy +
+                              (sw[cur][ty][tx] - sw[cur ^ 1][ty][tx]) * g.inv_dz);
+        }
         __syncthreads();
     }
 }
