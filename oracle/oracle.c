@@ -787,3 +787,167 @@ int oracle_momentum_prediction(int nx, int ny, int nz, double lx, double ly, dou
 #undef MU
     return 0;
 }
+
+/* ------------------------------------------------------ MTHINC volume of fluid */
+
+/* SURVEY.md sec. 8(f) NEXT-4.  PAPER.md:104-132 (sec. 3.1, eqs. 8-12) and Appendix A, triply periodic,
+ * with the LINEAR reconstruction T(x~) = n . x~ (the curvature tensor of eqs. A.3-A.5 set to zero) -- readings
+ * R21-R26 of DESIGN.md.  One step, directional splitting x -> y -> z (Algorithm 2):
+ *   for p = x, y, z  (s = n, x, y):
+ *     in every cell reconstruct  H^(x~) = 1/2 [1 + tanh(beta (n . x~ + d))]  from phi^s          (eq. 10)
+ *        n  = m~ / |m~|,  m~ = the Youngs gradient of phi^s in cell units (corner values averaged)  (A.6)
+ *        d  from the volume constraint  int_cell H^ = phi^s  (A.8), the integral being exact along the direction of the
+ *           largest |n| and a 2 x 2 Gauss quadrature across it (A.9-A.13)
+ *        cells with phi^s outside (eps, 1 - eps) or without a gradient keep the constant state H^ = phi^s
+ *     on every face along p the flux is the integral of the UPWIND cell's H^ over the part of that cell swept through the face
+ *        in dt, exact along p and 2 x 2 Gauss across it (A.23-A.31)
+ *     phi^p = [phi^s - (F_+ - F_-) / dl] / [1 - dt/dl (u_+ - u_-)]                                   (eq. 11)
+ *   phi^(n+1) = phi^z - sum_p dt/dl_p phi^p (u^p_+ - u^p_-)                                            (eq. 12)
+ * d is found here by bisection on the constraint itself (the definition; the paper's route is the quartic A.15). */
+#define VOF_EPS 1e-8
+
+/* ln cosh(x), stable for large |x| */
+static double ln_cosh(double x) {
+    double a = fabs(x);
+    return a + log1p(exp(-2.0 * a)) - 0.69314718055994530941723212145818;
+}
+/* int_a^b 1/2 [1 + tanh(beta (alpha x + gamma))] dx */
+static double tanh_integral(double a, double b, double alpha, double gamma, double beta) {
+    if (fabs(alpha) < 1e-12) return (b - a) * 0.5 * (1.0 + tanh(beta * gamma));
+    return 0.5 * ((b - a) + (ln_cosh(beta * (alpha * b + gamma)) - ln_cosh(beta * (alpha * a + gamma))) / (beta * alpha));
+}
+static const double GAUSS2[2] = {0.5 - 0.28867513459481288225457439025098, 0.5 + 0.28867513459481288225457439025098};
+
+/* mean of H^ over x~_dir in [a, b] and the full unit square across: exact along dir, 2 x 2 Gauss across (n: normal, d: offset) */
+static double hat_integral(const double n[3], double d, int dir, double a, double b, double beta) {
+    int t1 = (dir + 1) % 3, t2 = (dir + 2) % 3;
+    double s = 0.0;
+    for (int p = 0; p < 2; ++p)
+        for (int q = 0; q < 2; ++q) s += tanh_integral(a, b, n[dir], n[t1] * GAUSS2[p] + n[t2] * GAUSS2[q] + d, beta);
+    return 0.25 * s;
+}
+
+typedef struct { double n[3]; double d; int flat; } recon_t;   /* flat: H^ is the constant phi of the cell */
+
+static void reconstruct_cell(const grid_t *g, const double *phi, int i, int j, int k, double beta, recon_t *r) {
+    const int nx = g->nx, ny = g->ny, nz = g->nz;
+    const double f = phi[at(g, i, j, k)];
+    r->flat = 1; r->d = 0.0; r->n[0] = r->n[1] = r->n[2] = 0.0;
+    if (!(f > VOF_EPS && f < 1.0 - VOF_EPS)) return;
+    /* Youngs: the gradient at each of the 8 corners of the cell from the 8 cells around that corner (differences in
+     * cell units: the reconstruction lives in the unit cube), then the mean of the 8 corner values */
+    double m[3] = {0.0, 0.0, 0.0};
+    for (int ck = 0; ck < 2; ++ck)
+        for (int cj = 0; cj < 2; ++cj)
+            for (int ci = 0; ci < 2; ++ci) {
+                /* corner between cells (i-1+ci .. i+ci) x (j-1+cj .. j+cj) x (k-1+ck .. k+ck) */
+                int i0 = wrap(i - 1 + ci, nx), i1 = wrap(i + ci, nx);
+                int j0 = wrap(j - 1 + cj, ny), j1 = wrap(j + cj, ny);
+                int k0 = wrap(k - 1 + ck, nz), k1 = wrap(k + ck, nz);
+                double p000 = phi[at(g, i0, j0, k0)], p100 = phi[at(g, i1, j0, k0)], p010 = phi[at(g, i0, j1, k0)], p110 = phi[at(g, i1, j1, k0)];
+                double p001 = phi[at(g, i0, j0, k1)], p101 = phi[at(g, i1, j0, k1)], p011 = phi[at(g, i0, j1, k1)], p111 = phi[at(g, i1, j1, k1)];
+                m[0] += 0.25 * ((p100 - p000) + (p110 - p010) + (p101 - p001) + (p111 - p011));
+                m[1] += 0.25 * ((p010 - p000) + (p110 - p100) + (p011 - p001) + (p111 - p101));
+                m[2] += 0.25 * ((p001 - p000) + (p101 - p100) + (p011 - p010) + (p111 - p110));
+            }
+    m[0] *= 0.125; m[1] *= 0.125; m[2] *= 0.125;
+    double mag = sqrt(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+    if (!(mag > 1e-12)) return;
+    r->flat = 0;
+    for (int c = 0; c < 3; ++c) r->n[c] = m[c] / mag;
+    /* direction of the exact integration: the largest |n|, ties to x, then y (cases 1-3) */
+    double ax = fabs(r->n[0]), ay = fabs(r->n[1]), az = fabs(r->n[2]);
+    int dir = (ax >= ay && ax >= az) ? 0 : ((ay >= az) ? 1 : 2);
+    /* volume constraint (A.8, A.10): the cell mean of H^ equals phi; monotone in d -> bisection */
+    double lo = -(2.0 + 40.0 / beta), hi = 2.0 + 40.0 / beta;
+    for (int it = 0; it < 200; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (hat_integral(r->n, mid, dir, 0.0, 1.0, beta) < f) lo = mid; else hi = mid;
+    }
+    r->d = 0.5 * (lo + hi);
+}
+
+/* the flux (phase-1 volume per unit face area) through the face between cell (i,j,k) and its next neighbour along dir */
+static double face_flux_vof(const grid_t *g, const double *phi, const recon_t *rec, int i, int j, int k, int dir,
+                            double vel, double dl, double dt, double beta) {
+    double c = vel * dt / dl;                                   /* local CFL number, A.26 / A.30 / A.31 */
+    int iu = i, ju = j, ku = k;
+    double a, b, sign;
+    if (c >= 0.0) { a = 1.0 - c; b = 1.0; sign = 1.0; }          /* donor = this cell, its last c of the way */
+    else {
+        if (dir == 0) iu = wrap(i + 1, g->nx); else if (dir == 1) ju = wrap(j + 1, g->ny); else ku = wrap(k + 1, g->nz);
+        a = 0.0; b = -c; sign = -1.0;                            /* donor = the next cell, its first |c| */
+    }
+    const recon_t *r = &rec[at(g, iu, ju, ku)];
+    double vol = r->flat ? (b - a) * phi[at(g, iu, ju, ku)] : hat_integral(r->n, r->d, dir, a, b, beta);
+    return sign * dl * vol;
+}
+
+int oracle_vof_step(int nx, int ny, int nz, double lx, double ly, double lz, double beta, double dt,
+                    const double *phi, const double *u, const double *v, const double *w, double *phi_out, int nthreads) {
+    grid_t g;
+    if (grid_init(&g, nx, ny, nz, lx, ly, lz, ORACLE_BC_Z_PERIODIC, 1.0, 1.0, dt)) return 1;
+    if (!(beta > 0.0) || !(dt > 0.0)) return 1;
+    set_threads(nthreads);
+    const size_t n = (size_t)nx * ny * nz;
+    recon_t *rec = (recon_t *)malloc(sizeof(recon_t) * n);
+    double *cur = (double *)malloc(sizeof(double) * n), *flux = (double *)malloc(sizeof(double) * n);
+    double *ps[3] = {(double *)malloc(sizeof(double) * n), (double *)malloc(sizeof(double) * n), (double *)malloc(sizeof(double) * n)};
+    int rc = 0;
+    if (!rec || !cur || !flux || !ps[0] || !ps[1] || !ps[2]) { rc = 2; goto done; }
+    memcpy(cur, phi, sizeof(double) * n);
+    const double *vel[3] = {u, v, w};
+    const double dl[3] = {g.dx, g.dy, g.dz};
+    for (int dir = 0; dir < 3; ++dir) {
+#pragma omp parallel for collapse(2) schedule(static)
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j)
+                for (int i = 0; i < nx; ++i) reconstruct_cell(&g, cur, i, j, k, beta, &rec[at(&g, i, j, k)]);
+#pragma omp parallel for collapse(2) schedule(static)
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j)
+                for (int i = 0; i < nx; ++i)
+                    flux[at(&g, i, j, k)] = face_flux_vof(&g, cur, rec, i, j, k, dir, vel[dir][at(&g, i, j, k)], dl[dir], dt, beta);
+#pragma omp parallel for collapse(2) schedule(static)
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j)
+                for (int i = 0; i < nx; ++i) {
+                    size_t q = at(&g, i, j, k);
+                    size_t qm = dir == 0 ? at(&g, wrap(i - 1, nx), j, k) : (dir == 1 ? at(&g, i, wrap(j - 1, ny), k) : at(&g, i, j, wrap(k - 1, nz)));
+                    double du = vel[dir][q] - vel[dir][qm];
+                    ps[dir][q] = (cur[q] - (flux[q] - flux[qm]) / dl[dir]) / (1.0 - dt / dl[dir] * du);      /* eq. (11) */
+                }
+        memcpy(cur, ps[dir], sizeof(double) * n);
+    }
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                size_t q = at(&g, i, j, k);
+                double du = u[q] - u[at(&g, wrap(i - 1, nx), j, k)], dv = v[q] - v[at(&g, i, wrap(j - 1, ny), k)];
+                double dw = w[q] - w[at(&g, i, j, wrap(k - 1, nz))];
+                phi_out[q] = ps[2][q] - (dt / g.dx * ps[0][q] * du + dt / g.dy * ps[1][q] * dv + dt / g.dz * ps[2][q] * dw);   /* eq. (12) */
+            }
+done:
+    free(rec); free(cur); free(flux); free(ps[0]); free(ps[1]); free(ps[2]);
+    return rc;
+}
+
+/* the reconstruction alone, for the pins: n (3 doubles per cell, x fastest over cells), d and the flat flag per cell */
+int oracle_vof_reconstruct(int nx, int ny, int nz, double beta, const double *phi, double *n_out, double *d_out, int *flat_out, int nthreads) {
+    grid_t g;
+    if (grid_init(&g, nx, ny, nz, 1.0, 1.0, 1.0, ORACLE_BC_Z_PERIODIC, 1.0, 1.0, 1.0)) return 1;
+    if (!(beta > 0.0)) return 1;
+    set_threads(nthreads);
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                recon_t r;
+                reconstruct_cell(&g, phi, i, j, k, beta, &r);
+                size_t q = at(&g, i, j, k);
+                n_out[3 * q] = r.n[0]; n_out[3 * q + 1] = r.n[1]; n_out[3 * q + 2] = r.n[2];
+                d_out[q] = r.d; flat_out[q] = r.flat;
+            }
+    return 0;
+}

@@ -160,6 +160,16 @@ int oracle_momentum_prediction(int nx, int ny, int nz, double lx, double ly, dou
                                double *us, double *vs, double *ws,
                                double *mnew_u, double *mnew_v, double *mnew_w, int nthreads);
 
+/* ---- MTHINC volume-of-fluid step (eqs. 8-12; Appendix A),
+ * triply periodic, linear reconstruction T = n . x~, directional splitting x -> y -> z, one step:
+ * phi (cell centres) and u, v, w (faces) in, phi_out = phi^(n+1).  See oracle.c for every formula and DESIGN.md R21-R26
+ * for the readings (Gauss points, flat cells, normalised normal, flux quadrature). */
+int oracle_vof_step(int nx, int ny, int nz, double lx, double ly, double lz, double beta, double dt,
+                    const double *phi, const double *u, const double *v, const double *w, double *phi_out, int nthreads);
+/* the reconstruction of every cell alone: unit normal (3 per cell), offset d, and whether the cell keeps a constant state */
+int oracle_vof_reconstruct(int nx, int ny, int nz, double beta, const double *phi, double *n_out, double *d_out,
+                           int *flat_out, int nthreads);
+
 /* number of OpenMP threads a call with this nthreads argument would use */
 int oracle_threads(int nthreads);
 

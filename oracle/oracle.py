@@ -43,6 +43,10 @@ for _f in ("oracle_r2r_axis", "oracle_eigenvalues", "oracle_divergence_bc", "ora
     getattr(_lib, _f).restype = _ci
 _lib.oracle_momentum_prediction.argtypes = [_ci, _ci, _ci, _cd, _cd, _cd] + [_cd] * 10 + [_dp] * 14 + [_ci]
 _lib.oracle_momentum_prediction.restype = _ci
+_lib.oracle_vof_step.argtypes = [_ci, _ci, _ci, _cd, _cd, _cd, _cd, _cd] + [_dp] * 5 + [_ci]
+_lib.oracle_vof_step.restype = _ci
+_lib.oracle_vof_reconstruct.argtypes = [_ci, _ci, _ci, _cd, _dp, _dp, _dp, ctypes.POINTER(_ci), _ci]
+_lib.oracle_vof_reconstruct.restype = _ci
 _lib.oracle_threads.argtypes = [_ci]
 for _f in ("oracle_rhs_vdt", "oracle_projection_step_vdt", "oracle_rhs", "oracle_poisson", "oracle_projection_step", "oracle_projection_step_paper",
            "oracle_dft_axis", "oracle_divergence", "oracle_laplacian", "oracle_threads"):
@@ -262,3 +266,26 @@ def momentum_prediction(u, v, w, phi, kappa, m_old, box, rho1, rho2, mu1, mu2, s
                                            *[_p(a) for a in mo], *[_p(a) for a in out], nthreads),
            "oracle_momentum_prediction")
     return tuple(out[:3]), tuple(out[3:])
+
+
+def vof_step(phi, u, v, w, box, beta, dt, nthreads=0):
+    """one MTHINC step (x -> y -> z), triply periodic; returns phi^(n+1)"""
+    phi = _field(phi)
+    u, v, w = (_field(a, phi.shape) for a in (u, v, w))
+    out = np.empty_like(phi)
+    nz, ny, nx = phi.shape
+    _check(_lib.oracle_vof_step(nx, ny, nz, float(box[0]), float(box[1]), float(box[2]), float(beta), float(dt),
+                                _p(phi), _p(u), _p(v), _p(w), _p(out), nthreads), "oracle_vof_step")
+    return out
+
+
+def vof_reconstruct(phi, beta, nthreads=0):
+    """per cell: unit normal (nz, ny, nx, 3), offset d, flat flag"""
+    phi = _field(phi)
+    nz, ny, nx = phi.shape
+    n = np.empty(phi.shape + (3,))
+    d = np.empty_like(phi)
+    flat = np.empty(phi.shape, dtype=np.int32)
+    _check(_lib.oracle_vof_reconstruct(nx, ny, nz, float(beta), _p(phi), _p(n), _p(d),
+                                       flat.ctypes.data_as(ctypes.POINTER(_ci)), nthreads), "oracle_vof_reconstruct")
+    return n, d, flat

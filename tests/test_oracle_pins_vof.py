@@ -1,0 +1,137 @@
+"""Pins for the oracle's MTHINC volume-of-fluid step (oracle.vof_step / vof_reconstruct; SURVEY.md sec. 8(f) NEXT-4;
+PAPER.md:104-132, Appendix A).  The paper prints no worked numbers for one step, so the pins are what the method fixes:
+  V1  the reconstruction satisfies its own definition: the cell mean of H^ (A.8) -- evaluated with an INDEPENDENT
+      64-point Gauss-Legendre rule along the direction of exact integration -- equals phi to round-off; n is a unit vector
+      pointing towards phase 1; pure cells and cells without a gradient are flat
+  V2  Youngs' gradient is exact for a linear field (and so is the choice of the integration direction)
+  V3  "the mass of each phase [is] conserved up to machine precision" when div u = 0 discretely
+  V4  CFL = +-1 along the interface normal moves the profile by exactly one cell (flux = the whole donor cell), in
+      each direction: pins upwinding, signs, the swept interval and which velocity component drives which sweep
+  V5  a drop in a uniform diagonal flow: 0 <= phi <= 1, volume conserved, centroid moves by u t (consistency)
+  V6  a uniform phi stays uniform in a solenoidal flow; donor-cell fluxes for pure cells
+"""
+import numpy as np
+import pytest
+
+from tests import np_ops as ops
+
+BETA = 2.0
+
+
+def _drop(shape, centre, radius, width):
+    nz, ny, nx = shape
+    z, y, x = np.meshgrid(np.arange(nz) + 0.5, np.arange(ny) + 0.5, np.arange(nx) + 0.5, indexing="ij")
+    d = [np.minimum(np.abs(a - c), n - np.abs(a - c)) for a, c, n in ((x, centre[0], nx), (y, centre[1], ny), (z, centre[2], nz))]
+    r = np.sqrt(d[0] ** 2 + d[1] ** 2 + d[2] ** 2)
+    return 0.5 * (1.0 - np.tanh((r - radius) / width))
+
+
+def _solenoidal(shape, box, seed):
+    """u = curl of a random vector potential living on the cell edges: discretely divergence free on the MAC grid"""
+    rng = np.random.default_rng(seed)
+    dx, dy, dz = ops.spacings(shape, box)
+    ax, ay, az = (rng.standard_normal(shape) for _ in range(3))
+    d = lambda f, axis, h: (f - np.roll(f, 1, axis=axis)) / h
+    u = d(az, 1, dy) - d(ay, 0, dz)
+    v = d(ax, 0, dz) - d(az, 2, dx)
+    w = d(ay, 2, dx) - d(ax, 1, dy)
+    assert np.abs(ops.div(u, v, w, box, False)).max() < 1e-10 * np.abs(u).max() / dx
+    return u, v, w
+
+
+def test_v1_reconstruction_satisfies_the_volume_constraint(oracle_mod):
+    shape = (12, 14, 16)
+    phi = _drop(shape, (8.3, 6.1, 5.7), 4.0, 0.8)
+    phi[0, 0, 0] = 0.4                                            # an isolated blip: has a gradient of its own
+    n, d, flat = oracle_mod.vof_reconstruct(phi, BETA)
+    inter = flat == 0
+    assert inter.sum() > 200 and np.all(flat[(phi <= 1e-8) | (phi >= 1 - 1e-8)] == 1)
+    assert np.allclose(np.linalg.norm(n[inter], axis=-1), 1.0, atol=1e-14)
+    xs, ws = np.polynomial.legendre.leggauss(64)
+    xs, ws = 0.5 * (xs + 1.0), 0.5 * ws                           # on [0, 1]
+    g2 = np.array([0.5 - 0.5 / np.sqrt(3.0), 0.5 + 0.5 / np.sqrt(3.0)])
+    worst = 0.0
+    idx = np.argwhere(inter)
+    for (k, j, i) in idx[:: max(1, len(idx) // 300)]:
+        nn, dd = n[k, j, i], d[k, j, i]
+        a = np.abs(nn)
+        dr = 0 if (a[0] >= a[1] and a[0] >= a[2]) else (1 if a[1] >= a[2] else 2)
+        t1, t2 = (dr + 1) % 3, (dr + 2) % 3
+        tot = 0.0
+        for p in g2:
+            for q in g2:
+                tot += 0.25 * np.sum(ws * 0.5 * (1.0 + np.tanh(BETA * (nn[dr] * xs + nn[t1] * p + nn[t2] * q + dd))))
+        worst = max(worst, abs(tot - phi[k, j, i]))
+    assert worst < 1e-12
+    # n points towards phase 1 (phi = 1 inside the drop): against the radial direction
+    k, j, i = 6, 6, 12                                            # a cell on the +x side of the drop
+    assert flat[k, j, i] == 0 and n[k, j, i, 0] < -0.5
+
+
+def test_v2_youngs_gradient_is_exact_for_a_linear_field(oracle_mod):
+    shape = (8, 9, 10)
+    z, y, x = np.meshgrid(np.arange(8.0), np.arange(9.0), np.arange(10.0), indexing="ij")
+    for g in ((0.03, 0.01, -0.02), (0.0, -0.04, 0.01), (0.01, 0.01, 0.05), (-0.02, 0.02, 0.02)):
+        phi = 0.5 + g[0] * (x - 4.5) + g[1] * (y - 4.0) + g[2] * (z - 3.5)
+        n, d, flat = oracle_mod.vof_reconstruct(phi, BETA)
+        want = np.array(g) / np.linalg.norm(g)
+        inner = n[1:-1, 1:-1, 1:-1]                                # the periodic wrap breaks linearity in the outer layer
+        assert np.all(flat[1:-1, 1:-1, 1:-1] == 0) and np.abs(inner - want).max() < 1e-13
+
+
+@pytest.mark.parametrize("seed", [0, 1])
+def test_v3_volume_is_conserved_to_round_off_in_a_solenoidal_flow(oracle_mod, seed):
+    shape, box = (10, 12, 16), (1.6, 1.2, 1.0)
+    phi = _drop(shape, (7.2, 6.4, 4.9), 3.5, 0.7)
+    u, v, w = _solenoidal(shape, box, seed)
+    dt = 0.3 * min(ops.spacings(shape, box)) / max(np.abs(a).max() for a in (u, v, w))
+    out = oracle_mod.vof_step(phi, u, v, w, box, BETA, dt)
+    assert abs(out.sum() - phi.sum()) < 1e-13 * phi.sum()
+    assert np.abs(out - phi).max() > 1e-3                         # ... and the step did something
+    assert out.min() > -1e-3 and out.max() < 1.0 + 1e-3
+
+
+@pytest.mark.parametrize("axis,sign", [(2, 1), (2, -1), (1, 1), (1, -1), (0, 1), (0, -1)])
+def test_v4_unit_cfl_along_the_normal_is_an_exact_shift(oracle_mod, axis, sign):
+    shape, box = (8, 8, 8), (0.8, 1.6, 2.4)
+    n = 8
+    s = np.arange(n) + 0.5
+    prof = 0.5 * (np.tanh((s - 2.0) / 0.9) - np.tanh((s - 6.0) / 0.9))          # a slab, periodic
+    sh = [1, 1, 1]
+    sh[axis] = n
+    phi = np.ascontiguousarray(np.broadcast_to(prof.reshape(sh), shape))
+    h = ops.spacings(shape, box)[2 - axis]
+    dt = 0.01
+    vel = [np.zeros(shape) for _ in range(3)]
+    vel[2 - axis] = np.full(shape, sign * h / dt)                   # u dt / dl = +-1
+    out = oracle_mod.vof_step(phi, *vel, box, BETA, dt)
+    assert np.abs(out - np.roll(phi, sign, axis=axis)).max() < 1e-12
+
+
+def test_v5_drop_in_a_uniform_diagonal_flow(oracle_mod):
+    shape, box = (16, 16, 16), (1.0, 1.0, 1.0)
+    phi = _drop(shape, (6.0, 7.0, 8.0), 3.0, 0.7)
+    vel = (0.8, -0.5, 0.3)
+    u, v, w = (np.full(shape, c) for c in vel)
+    dt, steps = 0.25 / 16 / 0.8, 8
+    cur = phi
+    for _ in range(steps):
+        cur = oracle_mod.vof_step(cur, u, v, w, box, BETA, dt)
+        assert cur.min() > -1e-6 and cur.max() < 1.0 + 1e-6
+    assert abs(cur.sum() - phi.sum()) < 1e-12 * phi.sum()
+    z, y, x = np.meshgrid(*(np.arange(16) + 0.5,) * 3, indexing="ij")
+    cen = lambda f: np.array([(f * x).sum(), (f * y).sum(), (f * z).sum()]) / f.sum() / 16.0
+    shift = cen(cur) - cen(phi)
+    want = np.array(vel) * dt * steps
+    # the first moment is not an invariant of the scheme (the tanh profile sharpens to the width 1 / beta while it moves):
+    # the centroid follows u t to a few per cent -- a wrong component, sign or split order would be off by O(1)
+    assert np.all(np.abs(shift - want) < 0.03 * np.abs(want))
+
+
+def test_v6_uniform_and_pure_states(oracle_mod):
+    shape, box = (6, 8, 10), (1.0, 0.8, 0.6)
+    u, v, w = _solenoidal(shape, box, 5)
+    dt = 0.2 * min(ops.spacings(shape, box)) / max(np.abs(a).max() for a in (u, v, w))
+    for val in (0.3, 0.0, 1.0):
+        out = oracle_mod.vof_step(np.full(shape, val), u, v, w, box, BETA, dt)
+        assert np.abs(out - val).max() < 1e-13
