@@ -180,6 +180,19 @@ int flutas_momentum_rhs(flutas_plan *plan, const double *u, const double *v, con
                         double dt, double dt_ratio, double *us_out, double *vs_out, double *ws_out, double *rhs_out,
                         void *stream);
 
+/* One step of the MTHINC volume-of-fluid method (eqs. 8-12; Appendix A,
+ * PAPER.md:446-653; Algorithm 1 line 6, Algorithm 2): phi^n -> phi^(n+1) with the velocity u^n, directional splitting
+ * x -> y -> z, hyperbolic-tangent reconstruction with sharpness beta (the paper's runs use 2 and 3) and the
+ * LINEAR surface T = n . x~ (curvature tensor zero), Youngs normals, the volume constraint solved in the
+ * paper's polynomial form (A.14-A.16), fluxes by exact integration along the sweep and 2 x 2 Gauss points across it,
+ * the divergence correction of eq. (12).  Cells with phi outside (1e-8, 1 - 1e-8) or without a gradient carry a constant
+ * state (R21-R26).  Triply periodic plans only (FLUTAS_ERR_UNSUPPORTED_SIZE otherwise).
+ *   phi, u, v, w: N doubles each on the device (phi at cell centres, u / v / w on east / north / top faces); not modified
+ *   phi_out: N doubles; may be phi itself (in place).  beta > 0, dt > 0.
+ * Uses four fields of the plan's workspace (one step of anything in flight per plan).  Enqueues on `stream`. */
+int flutas_vof_step(flutas_plan *plan, const double *phi, const double *u, const double *v, const double *w,
+                    double *phi_out, double beta, double dt, void *stream);
+
 /* NULL is a no-op.  Frees every device and host resource of the plan (synchronises the device). */
 void flutas_plan_destroy(flutas_plan *plan);
 

@@ -32,6 +32,8 @@ lib.flutas_time_step.argtypes = [_vp] * 15 + [_cd] * 8 + [_vp]
 lib.flutas_time_step.restype = _ci
 lib.flutas_momentum_rhs.argtypes = [_vp] * 14 + [_cd] * 8 + [_vp] * 5
 lib.flutas_momentum_rhs.restype = _ci
+lib.flutas_vof_step.argtypes = [_vp] * 6 + [_cd, _cd, _vp]
+lib.flutas_vof_step.restype = _ci
 lib.flutas_plan_destroy.argtypes = [_vp]
 lib.flutas_plan_destroy.restype = None
 lib.flutas_projection_step.argtypes = [_vp] * 7 + [_cd, _vp]
@@ -72,7 +74,7 @@ EXPORTS = [
     "flutas_plan_set_timing", "flutas_plan_read_timing", "flutas_plan_kernel_bytes", "flutas_plan_set_option",
     "flutas_projection_step_ex", "flutas_splitting_rhs_ex",
     "flutas_plan_create_ex", "flutas_workspace_bytes", "flutas_plan_set_workspace", "flutas_plan_kernel_symbol",
-    "flutas_time_step", "flutas_momentum_rhs",
+    "flutas_time_step", "flutas_momentum_rhs", "flutas_vof_step",
 ]
 
 
@@ -192,6 +194,11 @@ class Plan:
         outs = [_dev_ptr(t, self.npts) for t in (us, vs, ws, rhs)]
         _check(lib.flutas_momentum_rhs(self._h, *ptrs, float(mu1), float(mu2), float(sigma), float(grav[0]), float(grav[1]),
                                        float(grav[2]), float(dt), float(dt_ratio), *outs, _stream() if stream is None else stream))
+
+    # --- one MTHINC volume-of-fluid step (phi_out may be phi)
+    def vof_step(self, phi, u, v, w, phi_out, beta, dt, stream=None):
+        ptrs = [_dev_ptr(t, self.npts) for t in (phi, u, v, w, phi_out)]
+        _check(lib.flutas_vof_step(self._h, *ptrs, float(beta), float(dt), _stream() if stream is None else stream))
 
     # --- the step for host arrays (numpy float64 or pinned torch CPU tensors), in place, synchronous
     def projection_step_host(self, u, v, w, phi, p, p_old, dt, stream=None):

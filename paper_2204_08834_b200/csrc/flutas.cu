@@ -19,6 +19,7 @@
 #include "kernels_rhs.cuh"
 #include "kernels_thomas.cuh"
 #include "kernels_tma.cuh"
+#include "kernels_vof.cuh"
 #include "kernels_x.cuh"
 #include "kernels_y16.cuh"
 
@@ -1176,6 +1177,31 @@ extern "C" int flutas_time_step(flutas_plan *pl, double *u, double *v, double *w
     tm.mark();
     tm.done();
     return FLUTAS_OK;
+}
+
+// ---- MTHINC volume-of-fluid step (kernels_vof.cuh): three sweeps (flux, update) and the divergence correction
+extern "C" int flutas_vof_step(flutas_plan *pl, const double *phi, const double *u, const double *v, const double *w,
+                               double *phi_out, double beta, double dt, void *stream) {
+    if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
+    if (pl->bc[0] != FLUTAS_BC_PERIODIC || pl->bc[1] != FLUTAS_BC_PERIODIC || pl->bc[2] != FLUTAS_BC_PERIODIC)
+        return fail(FLUTAS_ERR_UNSUPPORTED_SIZE, "the volume-of-fluid step takes triply periodic plans");
+    if (!(beta > 0.0) || !std::isfinite(beta) || !(dt > 0.0) || !std::isfinite(dt))
+        return fail(FLUTAS_ERR_INVALID_ARG, "beta and dt must be positive and finite");
+    const void *ptrs[5] = {phi, u, v, w, phi_out};
+    if (int rc = check_fields(pl, ptrs, phi_out == phi ? 4 : 5)) return rc;
+    if (!pl->ws_base) return fail(FLUTAS_ERR_INVALID_ARG, "the plan has no workspace (flutas_plan_set_workspace)");
+    cudaStream_t st = (cudaStream_t)stream;
+    const GridParams g = pl->grid;
+    const unsigned nb = (unsigned)((pl->npts + 255) / 256);
+    double *flux = pl->rhs, *px = pl->up, *py = pl->vp, *pz = pl->wp;
+    vof_flux_kernel<0><<<nb, 256, 0, st>>>(g, beta, dt, phi, u, flux);
+    vof_update_kernel<0><<<nb, 256, 0, st>>>(g, dt, phi, u, flux, px);
+    vof_flux_kernel<1><<<nb, 256, 0, st>>>(g, beta, dt, px, v, flux);
+    vof_update_kernel<1><<<nb, 256, 0, st>>>(g, dt, px, v, flux, py);
+    vof_flux_kernel<2><<<nb, 256, 0, st>>>(g, beta, dt, py, w, flux);
+    vof_update_kernel<2><<<nb, 256, 0, st>>>(g, dt, py, w, flux, pz);
+    vof_final_kernel<<<nb, 256, 0, st>>>(g, dt, px, py, pz, u, v, w, phi_out);
+    return check_launch(cudaGetLastError(), "vof_step");
 }
 
 extern "C" int flutas_projection_step(flutas_plan *pl, double *u, double *v, double *w, const double *phi, double *p,

@@ -1,0 +1,169 @@
+// kernels_vof.cuh -- SURVEY.md sec. 8(f) NEXT-4: one step of the MTHINC volume-of-fluid method (sec. 3.1,
+// eqs. 8-12; Appendix A), triply periodic, linear reconstruction T(x~) = n . x~ (the curvature tensor of
+// A.3-A.5 set to zero), directional splitting x -> y -> z (Algorithm 2):
+//
+//   per sweep p (s = n, x, y):   reconstruct  H^ = 1/2 [1 + tanh(beta (n . x~ + d))]  in every interface cell of phi^s
+//                                flux through every face = integral of the UPWIND cell's H^ over the part swept in dt
+//                                phi^p = [phi^s - (F_+ - F_-) / dl] / [1 - dt/dl (u_+ - u_-)]                       eq. (11)
+//   finally                      phi^(n+1) = phi^z - sum_p dt/dl_p phi^p (u^p_+ - u^p_-)                             eq. (12)
+//
+//   n = m~ / |m~| with m~ the Youngs gradient in cell units (A.6): evaluated with explicitly rounded adds / multiplies in a
+//       fixed order, because n decides an INTEGER -- the direction of exact integration, argmax |n| (cases 1-3,
+//       PAPER.md:503-520) -- and that decision must not depend on fused multiply-adds;
+//   d  from the volume constraint A.8 / A.10 in the paper's polynomial form (A.14-A.16): with D = e^{2 beta d},
+//       A = e^{2 beta n_dir}, B_i = e^{2 beta a_i} (a_i = the transverse part of n . x~ at the four Gauss points) and
+//       Q = e^{8 beta n_dir phi}:   prod_i (A B_i D + 1) = Q prod_i (B_i D + 1),  a quartic in D with exactly one positive
+//       root, found by bisection on ln D (robust for every phi in (eps, 1 - eps); the closed-form route A.17-A.21 is not used);
+//   fluxes: exact integration of tanh along the sweep direction, 2 x 2 Gauss points across it (A.23-A.31).
+//
+// vof_flux_kernel<DIR>: one thread per cell; a cell writes the flux of the faces it is the donor of (its + face when
+// the velocity there is >= 0, its - face when the velocity there is < 0): every face is written exactly once.
+// vof_update_kernel<DIR>: eq. (11).  vof_final_kernel: eq. (12).
+#pragma once
+#include "kernels.cuh"
+
+namespace flutas {
+
+constexpr double kVofEps = 1e-8;
+constexpr double kGauss0 = 0.5 - 0.28867513459481288225457439025098, kGauss1 = 0.5 + 0.28867513459481288225457439025098;
+
+__device__ __forceinline__ double ln_cosh_dev(double x) {
+    const double a = fabs(x);
+    return a + log1p(exp(-2.0 * a)) - 0.69314718055994530941723212145818;
+}
+// int_a^b 1/2 [1 + tanh(beta (alpha x + gamma))] dx
+__device__ __forceinline__ double tanh_integral_dev(double a, double b, double alpha, double gamma, double beta) {
+    if (fabs(alpha) < 1e-12) return (b - a) * 0.5 * (1.0 + tanh(beta * gamma));
+    return 0.5 * ((b - a) + (ln_cosh_dev(beta * (alpha * b + gamma)) - ln_cosh_dev(beta * (alpha * a + gamma))) / (beta * alpha));
+}
+// mean of H^ over x~_dir in [a, b] x the unit square across it
+__device__ __forceinline__ double hat_integral_dev(double nd, double n1, double n2, double d, double a, double b, double beta) {
+    double s = tanh_integral_dev(a, b, nd, n1 * kGauss0 + n2 * kGauss0 + d, beta);
+    s += tanh_integral_dev(a, b, nd, n1 * kGauss0 + n2 * kGauss1 + d, beta);
+    s += tanh_integral_dev(a, b, nd, n1 * kGauss1 + n2 * kGauss0 + d, beta);
+    s += tanh_integral_dev(a, b, nd, n1 * kGauss1 + n2 * kGauss1 + d, beta);
+    return 0.25 * s;
+}
+
+struct VofRecon { double n[3]; double d; bool flat; };
+
+// reconstruction of cell (i, j, k) from the field f (periodic)
+__device__ __forceinline__ void vof_reconstruct(const GridParams &g, const double *__restrict__ f, int i, int j, int k, double beta,
+                                                VofRecon &r) {
+    const long long sy = g.nx, sz = (long long)g.nx * g.ny;
+    const double fc = f[i + sy * j + sz * k];
+    r.flat = true; r.d = 0.0; r.n[0] = r.n[1] = r.n[2] = 0.0;
+    if (!(fc > kVofEps && fc < 1.0 - kVofEps)) return;
+    int ii[3] = {i == 0 ? g.nx - 1 : i - 1, i, i == g.nx - 1 ? 0 : i + 1};
+    int jj[3] = {j == 0 ? g.ny - 1 : j - 1, j, j == g.ny - 1 ? 0 : j + 1};
+    int kk[3] = {k == 0 ? g.nz - 1 : k - 1, k, k == g.nz - 1 ? 0 : k + 1};
+    double p[3][3][3];   // [dk][dj][di]
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) p[c][b][a] = __ldg(f + ii[a] + sy * jj[b] + sz * kk[c]);
+    // Youngs: the gradient at the 8 corners from the 8 cells around each, then their mean.  Explicitly rounded operations
+    // in a fixed order (corner order k, j, i): no fused multiply-add may change n, which decides the integration direction.
+    double m0 = 0.0, m1 = 0.0, m2 = 0.0;
+#pragma unroll
+    for (int ck = 0; ck < 2; ++ck)
+#pragma unroll
+        for (int cj = 0; cj < 2; ++cj)
+#pragma unroll
+            for (int ci = 0; ci < 2; ++ci) {
+                const double p000 = p[ck][cj][ci], p100 = p[ck][cj][ci + 1], p010 = p[ck][cj + 1][ci], p110 = p[ck][cj + 1][ci + 1];
+                const double p001 = p[ck + 1][cj][ci], p101 = p[ck + 1][cj][ci + 1], p011 = p[ck + 1][cj + 1][ci], p111 = p[ck + 1][cj + 1][ci + 1];
+                auto sum4 = [](double a, double b, double c, double d) { return __dadd_rn(__dadd_rn(__dadd_rn(a, b), c), d); };
+                m0 = __dadd_rn(m0, __dmul_rn(0.25, sum4(__dsub_rn(p100, p000), __dsub_rn(p110, p010), __dsub_rn(p101, p001), __dsub_rn(p111, p011))));
+                m1 = __dadd_rn(m1, __dmul_rn(0.25, sum4(__dsub_rn(p010, p000), __dsub_rn(p110, p100), __dsub_rn(p011, p001), __dsub_rn(p111, p101))));
+                m2 = __dadd_rn(m2, __dmul_rn(0.25, sum4(__dsub_rn(p001, p000), __dsub_rn(p101, p100), __dsub_rn(p011, p010), __dsub_rn(p111, p110))));
+            }
+    m0 = __dmul_rn(m0, 0.125); m1 = __dmul_rn(m1, 0.125); m2 = __dmul_rn(m2, 0.125);
+    const double mag = sqrt(__dadd_rn(__dadd_rn(__dmul_rn(m0, m0), __dmul_rn(m1, m1)), __dmul_rn(m2, m2)));
+    if (!(mag > 1e-12)) return;
+    r.flat = false;
+    r.n[0] = m0 / mag; r.n[1] = m1 / mag; r.n[2] = m2 / mag;
+    const double ax = fabs(r.n[0]), ay = fabs(r.n[1]), az = fabs(r.n[2]);
+    const int dir = (ax >= ay && ax >= az) ? 0 : ((ay >= az) ? 1 : 2);
+    const double nd = r.n[dir], n1 = r.n[(dir + 1) % 3], n2 = r.n[(dir + 2) % 3];
+    // prod_i (A B_i D + 1) = Q prod_i (B_i D + 1)   (A.14-A.16 with Q here = A^2 Q_paper)
+    const double tb = 2.0 * beta;
+    const double A = exp(tb * nd), Q = exp(4.0 * tb * nd * fc);
+    const double B0 = exp(tb * (n1 * kGauss0 + n2 * kGauss0)), B1 = exp(tb * (n1 * kGauss0 + n2 * kGauss1));
+    const double B2 = exp(tb * (n1 * kGauss1 + n2 * kGauss0)), B3 = exp(tb * (n1 * kGauss1 + n2 * kGauss1));
+    const double AB0 = A * B0, AB1 = A * B1, AB2 = A * B2, AB3 = A * B3;
+    // the left side minus the right side increases with D when A > 1 and decreases when A < 1
+    double lo = -tb * (2.0 + 40.0 / beta), hi = -lo;                       // ln D = 2 beta d
+    const bool rising = nd > 0.0;
+    for (int it = 0; it < 64; ++it) {
+        const double mid = 0.5 * (lo + hi), D = exp(mid);
+        const double num = fma(AB0, D, 1.0) * fma(AB1, D, 1.0) * (fma(AB2, D, 1.0) * fma(AB3, D, 1.0));
+        const double den = fma(B0, D, 1.0) * fma(B1, D, 1.0) * (fma(B2, D, 1.0) * fma(B3, D, 1.0));
+        const bool below = rising ? (num < Q * den) : (num > Q * den);     // the root lies above mid
+        if (below) lo = mid; else hi = mid;
+    }
+    r.d = 0.5 * (lo + hi) / tb;
+}
+
+template <int DIR>
+__global__ void __launch_bounds__(256)
+vof_flux_kernel(GridParams g, double beta, double dt, const double *__restrict__ phi, const double *__restrict__ vel,
+                double *__restrict__ flux) {
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long npts = (long long)g.nx * g.ny * g.nz;
+    if (q >= npts) return;
+    const int i = (int)(q % g.nx), j = (int)((q / g.nx) % g.ny), k = (int)(q / ((long long)g.nx * g.ny));
+    const long long sy = g.nx, sz = (long long)g.nx * g.ny;
+    const long long qm = DIR == 0 ? (i == 0 ? q + (g.nx - 1) : q - 1)
+                       : DIR == 1 ? (j == 0 ? q + (g.ny - 1) * sy : q - sy) : (k == 0 ? q + (g.nz - 1) * sz : q - sz);
+    const double dl = 1.0 / (DIR == 0 ? g.inv_dx : (DIR == 1 ? g.inv_dy : g.inv_dz));
+    const double cp = vel[q] * dt / dl, cm = vel[qm] * dt / dl;             // local CFL numbers on the + and - face (A.26)
+    const bool give_p = cp >= 0.0, give_m = cm < 0.0;
+    if (!give_p && !give_m) return;
+    VofRecon r;
+    vof_reconstruct(g, phi, i, j, k, beta, r);
+    const double fc = phi[q];
+    const double nd = r.n[DIR], n1 = r.n[(DIR + 1) % 3], n2 = r.n[(DIR + 2) % 3];
+    if (give_p) {                                                            // the last cp of the way through this cell
+        const double a = 1.0 - cp, b = 1.0;
+        flux[q] = dl * (r.flat ? (b - a) * fc : hat_integral_dev(nd, n1, n2, r.d, a, b, beta));
+    }
+    if (give_m) {                                                            // the first |cm| of it, leaving backwards
+        const double a = 0.0, b = -cm;
+        flux[qm] = -dl * (r.flat ? (b - a) * fc : hat_integral_dev(nd, n1, n2, r.d, a, b, beta));
+    }
+}
+
+template <int DIR>
+__global__ void __launch_bounds__(256)
+vof_update_kernel(GridParams g, double dt, const double *__restrict__ phi, const double *__restrict__ vel,
+                  const double *__restrict__ flux, double *__restrict__ out) {
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long npts = (long long)g.nx * g.ny * g.nz;
+    if (q >= npts) return;
+    const int i = (int)(q % g.nx), j = (int)((q / g.nx) % g.ny), k = (int)(q / ((long long)g.nx * g.ny));
+    const long long sy = g.nx, sz = (long long)g.nx * g.ny;
+    const long long qm = DIR == 0 ? (i == 0 ? q + (g.nx - 1) : q - 1)
+                       : DIR == 1 ? (j == 0 ? q + (g.ny - 1) * sy : q - sy) : (k == 0 ? q + (g.nz - 1) * sz : q - sz);
+    const double inv_dl = DIR == 0 ? g.inv_dx : (DIR == 1 ? g.inv_dy : g.inv_dz);
+    const double du = vel[q] - vel[qm];
+    out[q] = (phi[q] - (flux[q] - flux[qm]) * inv_dl) / (1.0 - dt * inv_dl * du);     // eq. (11)
+}
+
+__global__ void __launch_bounds__(256)
+vof_final_kernel(GridParams g, double dt, const double *__restrict__ px, const double *__restrict__ py, const double *__restrict__ pz,
+                 const double *__restrict__ u, const double *__restrict__ v, const double *__restrict__ w, double *__restrict__ out) {
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long npts = (long long)g.nx * g.ny * g.nz;
+    if (q >= npts) return;
+    const int i = (int)(q % g.nx), j = (int)((q / g.nx) % g.ny), k = (int)(q / ((long long)g.nx * g.ny));
+    const long long sy = g.nx, sz = (long long)g.nx * g.ny;
+    const double du = u[q] - u[i == 0 ? q + (g.nx - 1) : q - 1];
+    const double dv = v[q] - v[j == 0 ? q + (g.ny - 1) * sy : q - sy];
+    const double dw = w[q] - w[k == 0 ? q + (g.nz - 1) * sz : q - sz];
+    out[q] = pz[q] - (dt * g.inv_dx * px[q] * du + dt * g.inv_dy * py[q] * dv + dt * g.inv_dz * pz[q] * dw);   // eq. (12)
+}
+
+}  // namespace flutas
