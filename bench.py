@@ -9,6 +9,7 @@ batch of synthetic input.  Workloads (BASELINE.json `metric` names both):
   cfg5  1024 x 1024 x 512 wall-bounded, box 4 x 4 x 1, two-layer, rho2/rho1 = 1000          [under "also"]
   cavity 512 x 512 x 256 closed box, walls in x, y, z (cosine expansions; NEXT-2)           [under "also"]
   cfg4ts the cfg4 fields through flutas_time_step (momentum prediction fused in; NEXT-5)    [under "also"]
+  cfg4vof the cfg4 colour function through flutas_vof_step (one MTHINC step; NEXT-4)        [under "also"]
 N > 1 (torchrun): N independent replicas, one per GPU, no data-path collective ("replicas only").
 Prints ONE JSON line on rank 0.  --impl reference times the CPU oracle (tests' ground truth) on the same workload
 (one or two steps of the full 512^3 box); it is a deliberately slow baseline, not a target.
@@ -35,6 +36,8 @@ WORKLOAD_DESC = {
     "cfg4ts": "cfg4ts: the cfg4 fields (512^3 triply periodic, rho2/rho1=50) through flutas_time_step: momentum prediction "
               "(eq. 15: mu2/mu1=15, surface tension with a synthetic curvature field, gravity) fused with the projection "
               "(SURVEY sec. 8(f) NEXT-5)",
+    "cfg4vof": "cfg4vof: the cfg4 colour function and velocity (512^3 triply periodic, 391 drops of radius 16 cells) through "
+               "flutas_vof_step: one MTHINC step, beta = 2, CFL 0.3 (SURVEY sec. 8(f) NEXT-4)",
     "cfg2": "cfg2: 128^3 triply periodic emulsion-shaped (small case)",
     "cfg3": "cfg3: 256x256x128 wall-bounded two-layer (small case)",
 }
@@ -42,7 +45,7 @@ WORKLOAD_DESC = {
 
 def make_workload(name, ratio=None):
     import workloads as wl          # top-level module: loads neither the CUDA library nor the oracle
-    if name in ("cfg4", "cfg4ts"):
+    if name in ("cfg4", "cfg4ts", "cfg4vof"):
         return wl.config4(512, 50.0 if ratio is None else ratio)
     if name == "cfg5":
         return wl.config5()
@@ -147,7 +150,16 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     dev = [torch.from_numpy(a).cuda() for a in host]
     torch.cuda.synchronize()
     timestep = name.endswith("ts")
-    if timestep:
+    vof = name.endswith("vof")
+    if vof:
+        # phi^n -> phi^(n+1) out of place on the same resident fields every step (speed depends on the interface area,
+        # which the drops of cfg4 fix); dt from CFL 0.3 on the largest velocity component
+        cfl_dt = 0.3 / max(float(dev[c].abs().max()) * n_ / l_ for c, n_, l_ in zip(range(3), (W.nx, W.ny, W.nz), W.box))
+        phi_next = torch.empty_like(dev[3])
+
+        def one_step():
+            plan.vof_step(dev[3], dev[0], dev[1], dev[2], phi_next, 2.0, cfl_dt)
+    elif timestep:
         # whole velocity / pressure update: seven more resident fields (curvature, M of two time levels); the velocity
         # stays bounded over the timed steps because every step ends with the projection
         gen = torch.Generator(device="cuda").manual_seed(5)
@@ -196,6 +208,13 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     kms, ksteps = plan.read_timing()
     plan.set_timing(False)
     instrumented_ms = kv0.elapsed_time(kv1) / k_steps
+    if vof:
+        band = float(((dev[3] > 1e-8) & (dev[3] < 1.0 - 1e-8)).double().mean().item())
+        return vof_result(name, W, args, world, units_ms=replicas.aggregate_throughput(float(W.npts) * args.steps, ms_local),
+                          clocks=clocks, peak_gbs=peak_gbs, peak_label=peak_label, gen_s=gen_s,
+                          finite=bool(torch.isfinite(phi_next).all().item()),
+                          drift=float((phi_next.sum() - dev[3].sum()).abs() / dev[3].sum()), plan=plan, band=band,
+                          sm_count=torch.cuda.get_device_properties(0).multi_processor_count)
     finite = bool(torch.isfinite(dev[4]).all().item() and torch.isfinite(dev[5]).all().item() and torch.isfinite(dev[0]).all().item())
     units, ms = replicas.aggregate_throughput(float(W.npts) * args.steps, ms_local)
 
@@ -279,6 +298,35 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     if rank == 0 and world == 1 and with_cpu_baseline:
         out["cpu_baseline"] = oracle_full(W)
     return out
+
+
+def vof_result(name, W, args, world, units_ms, clocks, peak_gbs, peak_label, gen_s, finite, drift, plan, band, sm_count):
+    """the JSON block of the volume-of-fluid workload.  Seven launches per step (3 x flux + update, the correction).  The
+    flux kernels are bound by FP64 arithmetic in the cells that carry a reconstruction: algorithmic work
+    = 1100 fp64 operations per such cell and sweep (27-point Youngs gradient 230, 15 exponentials and 5 logarithms 425, the
+    root of the quartic 270, divisions and the flux arithmetic 175); peak = SMs x 64 fp64 lanes x the SM clock."""
+    units, ms = units_ms
+    step_ms = ms / args.steps
+    model_bytes = 28 * 8.0 * W.npts
+    ops = 1100.0 * 3 * band * W.npts
+    sm_ghz = (clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0) / 1e3
+    peak_ops = sm_count * 64 * sm_ghz            # G fp64 operations (instructions x lanes) per second
+    plan.destroy()
+    return {"metric": "fp64 volume-of-fluid step throughput", "value": round(units / (ms * 1e-3) / 1e6, 1), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(step_ms, 4), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_DESC[name], "grid": [W.nx, W.ny, W.nz], "input_generation_s": round(gen_s, 1),
+                       "cells_with_a_reconstruction": round(band, 4)},
+            "clocks": clocks, "gpu_launches": args.steps * 7, "launches_per_step": 7, "finite": finite,
+            "volume_drift_one_step": drift,
+            "step": {"ms": round(step_ms, 4), "model_bytes_per_pt": 224.0,
+                     "model_gbs": round(model_bytes / (step_ms * 1e-3) / 1e9, 1),
+                     "frac_of_peak_model_bytes": round(model_bytes / (step_ms * 1e-3) / 1e9 / peak_gbs, 4)},
+            "roofline": {"bound": "alu", "kernel": "vof_flux_kernel (3 launches, ~96 % of the step)",
+                         "achieved": round(ops / (step_ms * 1e-3) / 1e9, 1), "peak": round(peak_ops, 1), "unit": "G fp64 op/s",
+                         "frac": round(ops / (step_ms * 1e-3) / 1e9 / peak_ops, 4), "traffic": None,
+                         "peak_source": "derived: %d SMs x 64 fp64 lanes x %.3f GHz (DESIGN.md sec. 6)" % (sm_count, sm_ghz),
+                         "alg_ops_per_launch": ops / 3}}
 
 
 def torch_cufft_step(u, v, w, phi, p, po, box, rho1, rho2, dt):
@@ -423,7 +471,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workloads", default="cfg4,cfg5,cavity,cfg4ts")
+    ap.add_argument("--workloads", default="cfg4,cfg5,cavity,cfg4ts,cfg4vof")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-all", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -13,7 +13,8 @@
 //   d  from the volume constraint A.8 / A.10 in the paper's polynomial form (A.14-A.16): with D = e^{2 beta d},
 //       A = e^{2 beta n_dir}, B_i = e^{2 beta a_i} (a_i = the transverse part of n . x~ at the four Gauss points) and
 //       Q = e^{8 beta n_dir phi}:   prod_i (A B_i D + 1) = Q prod_i (B_i D + 1),  a quartic in D with exactly one positive
-//       root, found by bisection on ln D (robust for every phi in (eps, 1 - eps); the closed-form route A.17-A.21 is not used);
+//       root, found by a bracketed regula falsi started from the root of the untilted case (robust for every phi in
+//       (eps, 1 - eps), no transcendental function inside the iteration; the closed-form route A.17-A.21 is not used);
 //   fluxes: exact integration of tanh along the sweep direction, 2 x 2 Gauss points across it (A.23-A.31).
 //
 // vof_flux_kernel<DIR>: one thread per cell; a cell writes the flux of the faces it is the donor of (its + face when
@@ -27,14 +28,13 @@ namespace flutas {
 constexpr double kVofEps = 1e-8;
 constexpr double kGauss0 = 0.5 - 0.28867513459481288225457439025098, kGauss1 = 0.5 + 0.28867513459481288225457439025098;
 
-__device__ __forceinline__ double ln_cosh_dev(double x) {
-    const double a = fabs(x);
-    return a + log1p(exp(-2.0 * a)) - 0.69314718055994530941723212145818;
-}
 // int_a^b 1/2 [1 + tanh(beta (alpha x + gamma))] dx
 __device__ __forceinline__ double tanh_integral_dev(double a, double b, double alpha, double gamma, double beta) {
     if (fabs(alpha) < 1e-12) return (b - a) * 0.5 * (1.0 + tanh(beta * gamma));
-    return 0.5 * ((b - a) + (ln_cosh_dev(beta * (alpha * b + gamma)) - ln_cosh_dev(beta * (alpha * a + gamma))) / (beta * alpha));
+    // ln cosh(xb) - ln cosh(xa) with ln cosh(x) = |x| + ln(1 + e^(-2|x|)) - ln 2: one logarithm for the pair
+    const double xb = fabs(beta * (alpha * b + gamma)), xa = fabs(beta * (alpha * a + gamma));
+    const double lc = (xb - xa) + log((1.0 + exp(-2.0 * xb)) / (1.0 + exp(-2.0 * xa)));
+    return 0.5 * ((b - a) + lc / (beta * alpha));
 }
 // mean of H^ over x~_dir in [a, b] x the unit square across it
 __device__ __forceinline__ double hat_integral_dev(double nd, double n1, double n2, double d, double a, double b, double beta) {
@@ -94,17 +94,38 @@ __device__ __forceinline__ void vof_reconstruct(const GridParams &g, const doubl
     const double B0 = exp(tb * (n1 * kGauss0 + n2 * kGauss0)), B1 = exp(tb * (n1 * kGauss0 + n2 * kGauss1));
     const double B2 = exp(tb * (n1 * kGauss1 + n2 * kGauss0)), B3 = exp(tb * (n1 * kGauss1 + n2 * kGauss1));
     const double AB0 = A * B0, AB1 = A * B1, AB2 = A * B2, AB3 = A * B3;
-    // the left side minus the right side increases with D when A > 1 and decreases when A < 1
-    double lo = -tb * (2.0 + 40.0 / beta), hi = -lo;                       // ln D = 2 beta d
-    const bool rising = nd > 0.0;
-    for (int it = 0; it < 64; ++it) {
-        const double mid = 0.5 * (lo + hi), D = exp(mid);
+    // F(D) = +-[ prod (A B_i D + 1) - Q prod (B_i D + 1) ] S, signed so that it increases with D and scaled by S = 1 / (Q prod(B_i D0 + 1))
+    // so that it is O(1) around the root.  With no transverse tilt (B_i = 1) the root is D0 = (q - 1) / (A - q), q = Q^(1/4): the
+    // starting point.  Bracket it by factors of 4, then the Illinois variant of regula falsi (superlinear, bracket kept): no
+    // transcendental function and no division inside the loop.
+    double scale = 1.0;
+    auto F = [&](double D) {
         const double num = fma(AB0, D, 1.0) * fma(AB1, D, 1.0) * (fma(AB2, D, 1.0) * fma(AB3, D, 1.0));
         const double den = fma(B0, D, 1.0) * fma(B1, D, 1.0) * (fma(B2, D, 1.0) * fma(B3, D, 1.0));
-        const bool below = rising ? (num < Q * den) : (num > Q * den);     // the root lies above mid
-        if (below) lo = mid; else hi = mid;
+        return scale * fma(-Q, den, num);
+    };
+    const double qq = exp(tb * nd * fc);
+    double a = (qq - 1.0) / (A - qq), b = a;
+    scale = (nd > 0.0 ? 1.0 : -1.0) / (Q * (fma(B0, a, 1.0) * fma(B1, a, 1.0) * (fma(B2, a, 1.0) * fma(B3, a, 1.0))));
+    double fa = F(a), fb = fa;
+    for (int it = 0; it < 400 && fa > 0.0; ++it) { b = a; fb = fa; a *= 0.25; fa = F(a); }
+    for (int it = 0; it < 400 && fb < 0.0; ++it) { a = b; fa = fb; b *= 4.0; fb = F(b); }
+    int side = 0;
+    double root = 0.5 * (a + b), prev = -1.0;
+    for (int it = 0; it < 100; ++it) {
+        if (fa == 0.0) { root = a; break; }
+        if (fb == 0.0) { root = b; break; }
+        double c = (fa * b - fb * a) / (fa - fb);
+        if (!(c > a && c < b)) c = 0.5 * (a + b);
+        root = c;
+        if (fabs(c - prev) <= 1.0e-15 * c) break;        // the iterates have converged (the bracket need not shrink on both sides)
+        prev = c;
+        const double fcv = F(c);
+        if (fcv == 0.0) break;
+        if (fcv > 0.0) { b = c; fb = fcv; if (side == -1) fa *= 0.5; side = -1; }
+        else { a = c; fa = fcv; if (side == 1) fb *= 0.5; side = 1; }
     }
-    r.d = 0.5 * (lo + hi) / tb;
+    r.d = log(root) / tb;
 }
 
 template <int DIR>
