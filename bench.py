@@ -10,6 +10,7 @@ batch of synthetic input.  Workloads (BASELINE.json `metric` names both):
   cavity 512 x 512 x 256 closed box, walls in x, y, z (cosine expansions; NEXT-2)           [under "also"]
   cfg4ts the cfg4 fields through flutas_time_step (momentum prediction fused in; NEXT-5)    [under "also"]
   cfg4vof the cfg4 colour function through flutas_vof_step (one MTHINC step; NEXT-4)        [under "also"]
+  cfg4slab8 the cfg4 step on a z-slab decomposition over 8 ranks, all on one device (NEXT-3) [under "also"]
 N > 1 (torchrun): N independent replicas, one per GPU, no data-path collective ("replicas only").
 Prints ONE JSON line on rank 0.  --impl reference times the CPU oracle (tests' ground truth) on the same workload
 (one or two steps of the full 512^3 box); it is a deliberately slow baseline, not a target.
@@ -38,6 +39,11 @@ WORKLOAD_DESC = {
               "(SURVEY sec. 8(f) NEXT-5)",
     "cfg4vof": "cfg4vof: the cfg4 colour function and velocity (512^3 triply periodic, 391 drops of radius 16 cells) through "
                "flutas_vof_step: one MTHINC step, beta = 2, CFL 0.3 (SURVEY sec. 8(f) NEXT-4)",
+    "cfg4slab8": "cfg4slab8: the cfg4 step (512^3 triply periodic, rho2/rho1=50) on a z-slab decomposition over 8 ranks "
+                 "(SURVEY sec. 8(f) NEXT-3: the two all-to-all transposes are the store stages of the y transform and of the z "
+                 "stage, written straight into the peers' spectra); all 8 ranks driven phase by phase on ONE device",
+    "cfg5slab8": "cfg5slab8: the cfg5 step (1024x1024x512 wall-bounded, rho2/rho1=1000) on a z-slab decomposition over 8 ranks, "
+                 "all ranks on ONE device (SURVEY sec. 8(f) NEXT-3)",
     "cfg2": "cfg2: 128^3 triply periodic emulsion-shaped (small case)",
     "cfg3": "cfg3: 256x256x128 wall-bounded two-layer (small case)",
 }
@@ -45,7 +51,9 @@ WORKLOAD_DESC = {
 
 def make_workload(name, ratio=None):
     import workloads as wl          # top-level module: loads neither the CUDA library nor the oracle
-    if name in ("cfg4", "cfg4ts", "cfg4vof"):
+    if name == "cfg5slab8":
+        return wl.config5()
+    if name in ("cfg4", "cfg4ts", "cfg4vof", "cfg4slab8"):
         return wl.config4(512, 50.0 if ratio is None else ratio)
     if name == "cfg5":
         return wl.config5()
@@ -135,6 +143,8 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     import paper_2204_08834_b200 as fl
     from paper_2204_08834_b200 import replicas
 
+    if "slab" in name:
+        return bench_slab(name, args, local_rank, peak_gbs, peak_label)
     ratio = replicas.replica_density_ratio(rank) if (name == "cfg4" and world > 1) else None
     t0 = time.time()
     W = make_workload(name, ratio)
@@ -300,6 +310,122 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     return out
 
 
+def bench_slab(name, args, local_rank, peak_gbs, peak_label, n_ranks=8):
+    """NEXT-3 on one device: every rank of the decomposition is a plan of its own with its own buffers; the ranks are
+    driven phase by phase on one stream (their kernels never wait for one another), so the time of a step is the SUM of
+    the ranks' work -- what one GPU of an n_ranks-GPU node would do is 1 / n_ranks of it, plus the synchronisation and
+    the NVLink time of the bytes reported here, which this box cannot measure."""
+    import torch
+    import workloads as wl
+    from paper_2204_08834_b200 import slab
+    t0 = time.time()
+    W = make_workload(name)
+    gen_s = time.time() - t0
+    periodic = W.bc_z == 0
+    grp = slab.SlabGroup(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2, n_ranks)
+    parts = [wl.slab_split(a, n_ranks, periodic) for a in W.fields()]
+    dev = [[torch.from_numpy(parts[f][r]).cuda() for f in range(6)] for r in range(n_ranks)]
+    del parts
+    if not periodic:        # planes beyond a wall are never read; keep them finite for the checks below
+        for r in (0, n_ranks - 1):
+            for t in dev[r]:
+                torch.nan_to_num_(t, nan=0.0)
+    torch.cuda.synchronize()
+
+    def one_step(events=None):
+        for phase in range(3):
+            for r, pl in enumerate(grp.plans):
+                u, v, w, phi, p, po = dev[r]
+                pl.step_phase(phase, u, v, w, phi, p, po, p, W.dt, 1.0)
+            if events is not None:
+                events[phase].record()
+
+    for _ in range(args.warmup):
+        one_step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(visible_gpu_index(local_rank))
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    ev0.record()
+    for _ in range(args.steps):
+        one_step()
+    ev1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.result()
+    ms = ev0.elapsed_time(ev1)
+    # per phase, in a separate short loop
+    k_steps, phase_ms = 3, [0.0, 0.0, 0.0]
+    for _ in range(k_steps):
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        evs[0].record()
+        one_step(evs[1:])
+        torch.cuda.synchronize()
+        for i in range(3):
+            phase_ms[i] += evs[i].elapsed_time(evs[i + 1]) / k_steps
+    finite = all(bool(torch.isfinite(dev[r][f][1:-1]).all().item()) for r in range(n_ranks) for f in (0, 4))
+    step_ms = ms / args.steps
+    nxh, nzl, rpp = W.nx // 2 + 1, W.nz // n_ranks, W.ny // n_ranks
+    # bytes a rank sends to OTHER ranks per step: its share of the spectrum twice (forward rows, backward planes) + halo planes
+    fwd = 16.0 * nxh * (W.ny - rpp) * nzl
+    bwd = 16.0 * nxh * rpp * (W.nz - nzl) + 16.0 * nxh * rpp * 2
+    # algorithmic bytes of all ranks: the one-GPU model (216 / 218 B per point) with nzl + 2 instead of nzl planes in the
+    # inverse x, y transforms (the halo planes of p^(n+1))
+    model = (216.0 if periodic else 218.0) * W.npts + 2 * n_ranks * (16.0 * 2 + 8.0 + 16.0) * W.nx * W.ny
+    for pl in grp.plans:
+        pl.destroy()
+    return {"metric": METRIC + " (z-slab decomposition, all ranks on one device)", "value": round(W.npts * args.steps / (ms * 1e-3) / 1e6, 1),
+            "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(step_ms, 4),
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_DESC[name], "grid": [W.nx, W.ny, W.nz], "n_ranks": n_ranks, "planes_per_rank": nzl,
+                       "ky_rows_per_rank": rpp, "input_generation_s": round(gen_s, 1)},
+            "clocks": clocks, "gpu_launches": args.steps * n_ranks * (7 if periodic else 8), "finite": finite,
+            "phase_ms_all_ranks": [round(x, 4) for x in phase_ms],
+            "per_rank_ms": round(step_ms / n_ranks, 4),
+            "exchange_bytes_per_rank_per_step": {"forward": fwd, "backward": bwd,
+                                                 "at_900_GBs_ms": round((fwd + bwd) / 900e9 * 1e3, 4)},
+            "step": {"ms": round(step_ms, 4), "model_bytes_per_pt": round(model / W.npts, 1),
+                     "model_gbs": round(model / (step_ms * 1e-3) / 1e9, 1),
+                     "frac_of_peak_model_bytes": round(model / (step_ms * 1e-3) / 1e9 / peak_gbs, 4)},
+            "note": "one device runs all ranks one after the other: no NVLink transfer and no barrier is in this number"}
+
+
+def bench_slab_distributed(name, args, rank, local_rank, world):
+    """--slab under torchrun: ONE box decomposed over the N GPUs (strong scaling), one rank per GPU, exchange buffers in
+    torch symmetric memory, an NCCL all-reduce of one element as the barrier between phases.  NOT exercised in this
+    repository's runs (they have one GPU); the kernels and the index maps are the ones the one-device tests check."""
+    import torch
+    import workloads as wl
+    from paper_2204_08834_b200 import replicas, slab
+    W = make_workload(name)
+    periodic = W.bc_z == 0
+    sr = slab.SlabRank(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2)
+    dev = [torch.from_numpy(wl.slab_split(a, world, periodic)[rank]).cuda() for a in W.fields()]
+    for t in dev:
+        torch.nan_to_num_(t, nan=0.0)
+    for _ in range(args.warmup):
+        sr.step(*dev, W.dt)
+    sampler = ClockSampler(visible_gpu_index(local_rank))
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    replicas.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    ev0.record()
+    for _ in range(args.steps):
+        sr.step(*dev, W.dt)
+    ev1.record()
+    torch.cuda.synchronize()
+    replicas.barrier()
+    clocks = sampler.result()
+    _, ms = replicas.aggregate_throughput(0.0, ev0.elapsed_time(ev1))
+    return {"metric": METRIC, "value": round(W.npts * args.steps / (ms * 1e-3) / 1e6, 1), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms / args.steps, 4), "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_DESC[name], "grid": [W.nx, W.ny, W.nz],
+                       "parallelism": f"z-slabs x{world}, transposes fused into the transforms' stores over peer memory"},
+            "clocks": clocks, "gpu_launches": args.steps * (7 if periodic else 8),
+            "finite": bool(torch.isfinite(dev[4][1:-1]).all().item())}
+
+
 def vof_result(name, W, args, world, units_ms, clocks, peak_gbs, peak_label, gen_s, finite, drift, plan, band, sm_count):
     """the JSON block of the volume-of-fluid workload.  Seven launches per step (3 x flux + update, the correction).  The
     flux kernels are bound by FP64 arithmetic in the cells that carry a reconstruction: algorithmic work
@@ -425,6 +551,14 @@ def run_ours(args):
     peak_gbs, peak_label = load_peak()
     traffic = load_ncu_traffic()
     names = [w for w in args.workloads.split(",") if w]
+    if world > 1:       # all-ranks-on-one-device workloads are a one-GPU measurement
+        names = [n for n in names if "slab" not in n]
+    if args.slab and world > 1:
+        out = bench_slab_distributed(names[0], args, rank, local_rank, world)
+        if rank == 0:
+            print(json.dumps(out), flush=True)
+        replicas.barrier()
+        return
     results = [bench_workload(n, args, rank, local_rank, world, peak_gbs, peak_label, with_e2e=(not args.no_e2e) and (i == 0 or args.e2e_all),
                               traffic=traffic, with_cpu_baseline=(i == 0 and not args.no_cpu_baseline)) for i, n in enumerate(names)]
     out = results[0]
@@ -471,13 +605,15 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workloads", default="cfg4,cfg5,cavity,cfg4ts,cfg4vof")
+    ap.add_argument("--workloads", default="cfg4,cfg5,cavity,cfg4ts,cfg4vof,cfg4slab8")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-all", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--no-compare-torch", action="store_true", help="skip the torch/cuFFT statement of the periodic step (comparison only)")
     ap.add_argument("--opt", action="append", help="plan tuning knob name=value (experiments)")
+    ap.add_argument("--slab", action="store_true", help="N > 1 only: decompose ONE box over the N GPUs (z slabs, SURVEY sec. 8(f) "
+                                                        "NEXT-3) instead of running N replicas")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -257,6 +257,51 @@ double flutas_plan_kernel_bytes(const flutas_plan *plan, int idx);
  *   "overlap" = 0 | 1             chunked only: run the three kernels of a group on three internal streams */
 int flutas_plan_set_option(flutas_plan *plan, const char *name, int value);
 
+/* ---- the step on a z-slab decomposition over several GPUs ---------------------------
+ *
+ * PAPER.md:169-183 (sec. 3.3.1: slabs for the transforms along x and y, "all-to-all" transposes to make z local for the
+ * Gauss elimination and back), PAPER.md:313, 364-368 (the transposes are the measured bottleneck of the multi-GPU runs).
+ * Here the two all-to-alls are the STORE stage of the kernel before them: the last pass of the forward transform along
+ * y writes every row straight into the z-local spectrum of the rank that owns it, and the z stage writes every plane
+ * straight into the slab spectrum of the rank that owns it -- plain / TMA stores into peer memory over NVLink (or into
+ * the same device when ranks share one).  No transpose kernel, no pack / unpack buffer, no NCCL data path.
+ *
+ * Decomposition: rank r of n_ranks owns planes r*nzl .. (r+1)*nzl - 1, nzl = nz / n_ranks.  Every field argument is a
+ * LOCAL array of (nzl + 2) planes of nx*ny doubles (x fastest): plane 0 = the plane below the slab (owned by rank r-1),
+ * planes 1 .. nzl = the slab, plane nzl + 1 = the plane above (rank r+1); periodic z wraps around, beyond a wall the
+ * halo plane is never read.  On entry the halo planes of phi, p, p_old (both) and of w (plane 0) must hold the
+ * neighbours' values; u, v need none.  On exit u, v, w are corrected on planes 1 .. nzl and p_out holds p^(n+1) on ALL
+ * planes 0 .. nzl + 1 that exist (the z stage sends the two boundary planes of every slab to the neighbours as well), so
+ * a time loop never exchanges pressure halos; phi and w* arrive with the halos their producers gave them.
+ *
+ * Buffers (caller-owned device memory, 256-byte aligned):
+ *   workspace  flutas_slab_workspace_bytes: private to the rank;
+ *   exchange   flutas_slab_exchange_bytes: the rank's two spectra; PEERS WRITE INTO IT, so it must be mapped in every
+ *              rank's address space (CUDA IPC, torch symmetric memory, or one process) -- flutas_slab_plan_attach takes
+ *              the n_ranks device pointers as THIS process sees them (a HOST array; entry `rank` is the own buffer).
+ *              attach clears the own buffer: synchronise all ranks between attach and the first step.
+ * A step is three calls, phase = 0, 1, 2, each only enqueueing kernels on `stream`; BETWEEN phases 0 -> 1 and 1 -> 2 all
+ * ranks must have finished the earlier phase before any starts the later one (a stream-ordered barrier, e.g. an NCCL
+ * all-reduce of one element; nothing when the ranks are driven phase by phase on one stream of one device):
+ *   phase 0  right-hand side, transform along x, transform along y -> rows to their owners
+ *   phase 1  z stage on the own rows of ky -> planes to their owners
+ *   phase 2  inverse transforms along y and x, correction
+ * Phases 0 and 2 take the fields (p_out may be p, p_old or a seventh array, as in flutas_projection_step_ex); phase 1
+ * ignores them (NULL allowed).
+ * Sizes: n_ranks a power of two <= 16 dividing ny and nz, nz / n_ranks a power of two; nx a power of two in [128, 1024];
+ *        ny a power of two in [8, 1024]; periodic z: nz a power of two in [8, 1024]; wall z: nz <= 512.
+ * Results equal flutas_projection_step on the assembled fields up to round-off (same kernels, same arithmetic). */
+typedef struct flutas_slab_plan flutas_slab_plan;
+flutas_slab_plan *flutas_slab_plan_create(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
+                                          double rho1, double rho2, int n_ranks, int rank);
+size_t flutas_slab_workspace_bytes(int nx, int ny, int nz, int bc_z, int n_ranks);   /* 0: unsupported decomposition */
+size_t flutas_slab_exchange_bytes(int nx, int ny, int nz, int bc_z, int n_ranks);
+int flutas_slab_plan_attach(flutas_slab_plan *plan, void *workspace, size_t workspace_bytes,
+                            void *const *exchange /* HOST array of n_ranks DEVICE pointers */, size_t exchange_bytes);
+int flutas_slab_step_phase(flutas_slab_plan *plan, int phase, double *u, double *v, double *w, const double *phi,
+                           const double *p, const double *p_old, double *p_out, double dt, double dt_ratio, void *stream);
+void flutas_slab_plan_destroy(flutas_slab_plan *plan);
+
 #ifdef __cplusplus
 }
 #endif

@@ -67,6 +67,19 @@ lib.flutas_plan_read_timing.restype = _ci
 lib.flutas_plan_set_option.argtypes = [_vp, ctypes.c_char_p, _ci]
 lib.flutas_plan_set_option.restype = _ci
 
+lib.flutas_slab_plan_create.argtypes = [_ci, _ci, _ci, _cd, _cd, _cd, _ci, _cd, _cd, _ci, _ci]
+lib.flutas_slab_plan_create.restype = _vp
+lib.flutas_slab_workspace_bytes.argtypes = [_ci] * 5
+lib.flutas_slab_workspace_bytes.restype = ctypes.c_size_t
+lib.flutas_slab_exchange_bytes.argtypes = [_ci] * 5
+lib.flutas_slab_exchange_bytes.restype = ctypes.c_size_t
+lib.flutas_slab_plan_attach.argtypes = [_vp, _vp, ctypes.c_size_t, ctypes.POINTER(_vp), ctypes.c_size_t]
+lib.flutas_slab_plan_attach.restype = _ci
+lib.flutas_slab_step_phase.argtypes = [_vp, _ci] + [_vp] * 7 + [_cd, _cd, _vp]
+lib.flutas_slab_step_phase.restype = _ci
+lib.flutas_slab_plan_destroy.argtypes = [_vp]
+lib.flutas_slab_plan_destroy.restype = None
+
 EXPORTS = [
     "flutas_plan_create", "flutas_projection_step", "flutas_projection_step_host", "flutas_plan_destroy",
     "flutas_splitting_rhs", "flutas_poisson_solve", "flutas_last_error", "flutas_last_error_code",
@@ -75,6 +88,8 @@ EXPORTS = [
     "flutas_projection_step_ex", "flutas_splitting_rhs_ex",
     "flutas_plan_create_ex", "flutas_workspace_bytes", "flutas_plan_set_workspace", "flutas_plan_kernel_symbol",
     "flutas_time_step", "flutas_momentum_rhs", "flutas_vof_step",
+    "flutas_slab_plan_create", "flutas_slab_workspace_bytes", "flutas_slab_exchange_bytes", "flutas_slab_plan_attach",
+    "flutas_slab_step_phase", "flutas_slab_plan_destroy",
 ]
 
 
@@ -247,6 +262,53 @@ class Plan:
 
     def set_option(self, name, value):
         _check(lib.flutas_plan_set_option(self._h, name.encode(), int(value)))
+
+
+class SlabPlan:
+    """flutas_slab_plan_create / _attach / _step_phase / _destroy for ONE rank of a z-slab decomposition (include/flutas.h).
+    Fields are local tensors of (nz / n_ranks + 2) * ny * nx doubles (one halo plane below and above the slab).
+    `exchange_ptrs`: the device addresses of every rank's exchange buffer as this process sees them (entry `rank` is the
+    own one); slab.py builds them for ranks that share a process and for torchrun ranks (symmetric memory)."""
+
+    def __init__(self, nx, ny, nz, lx, ly, lz, bc_z, rho1, rho2, n_ranks, rank):
+        self._h = None
+        h = lib.flutas_slab_plan_create(int(nx), int(ny), int(nz), float(lx), float(ly), float(lz), int(bc_z), float(rho1),
+                                        float(rho2), int(n_ranks), int(rank))
+        if not h:
+            _raise_last()
+        self._h = h
+        self.nx, self.ny, self.nz, self.bc_z, self.n_ranks, self.rank = int(nx), int(ny), int(nz), int(bc_z), int(n_ranks), int(rank)
+        self.nzl = self.nz // self.n_ranks
+        self.npts_local = self.nx * self.ny * (self.nzl + 2)
+        self.workspace_bytes = lib.flutas_slab_workspace_bytes(self.nx, self.ny, self.nz, self.bc_z, self.n_ranks)
+        self.exchange_bytes = lib.flutas_slab_exchange_bytes(self.nx, self.ny, self.nz, self.bc_z, self.n_ranks)
+        self._keep = None
+
+    def attach(self, workspace, exchange_ptrs, keep=None):
+        """workspace: uint8 CUDA tensor of workspace_bytes; exchange_ptrs: n_ranks ints; keep: objects to keep alive"""
+        arr = (_vp * self.n_ranks)(*[int(q) for q in exchange_ptrs])
+        _check(lib.flutas_slab_plan_attach(self._h, workspace.data_ptr(), workspace.numel(), arr, self.exchange_bytes))
+        self._keep = (workspace, keep)
+
+    def step_phase(self, phase, u, v, w, phi, p, p_old, p_out, dt, dt_ratio=1.0, stream=None):
+        if phase == 1:
+            ptrs = [None] * 7
+        else:
+            ptrs = [_dev_ptr(t, self.npts_local) for t in (u, v, w, phi, p, p_old, p_out)]
+        _check(lib.flutas_slab_step_phase(self._h, int(phase), *ptrs, float(dt), float(dt_ratio),
+                                          _stream() if stream is None else stream))
+
+    def destroy(self):
+        if self._h:
+            lib.flutas_slab_plan_destroy(self._h)
+            self._h = None
+            self._keep = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
 
 
 def _host_ptr(a, npts):

@@ -102,7 +102,16 @@ struct flutas_plan {
     int timing;
     cudaEvent_t *events;         // kMaxPendingSteps * (n_launch + 1)
     int pending;
+    // z-slab decomposition (flutas_slab_plan, flutas_slab.inl): a rank owns two plans of reduced geometry
+    int role;                    // ROLE_FULL, ROLE_SLAB (nz = its planes + 2 halo planes: real-space kernels, x and y
+                                 // transforms), ROLE_ZLOCAL (ny = its share of the ky rows: the z stage)
+    int ny_full, row0;           // ROLE_ZLOCAL: rows of the whole spectrum and the first one this plan holds
+    double2 *spec_ext;           // ROLE_SLAB / ROLE_ZLOCAL: the spectrum lives in the exchange buffer, not in the workspace
+    PeerScatter *sc_dev;         // device copy of the store descriptor of the last forward y pass / of the z stage
+    ThomasPeerMaps *tpm;         // ROLE_ZLOCAL, wall: tensor maps of the peers' slab spectra (host)
+    int sc_nzl, sc_srows, sc_npeers;
 };
+enum { ROLE_FULL = 0, ROLE_SLAB = 1, ROLE_ZLOCAL = 2 };
 
 static const char *kKernelNames[K_MAX] = {"splitting_rhs", "fft_x_r2c", "fft_y_fwd", "z_solve", "z_singular",
                                           "fft_y_inv", "fft_x_c2r", "correction"};
@@ -158,10 +167,11 @@ static void host_wq(int n, std::vector<double2> &t) {
 // eigenvalues along y in the storage order of the transform in use (the 16 x 8 x 8 kernel has its own digit order)
 static int upload_lam_y(flutas_plan *pl) {
     std::vector<double> lam(pl->ny);
-    const double dy = pl->ly / pl->ny;
+    const int nyf = pl->ny_full;                 // == ny except for the z-local plan of a slab decomposition (rows row0 ..)
+    const double dy = pl->ly / nyf;
     for (int pos = 0; pos < pl->ny; ++pos) {
-        const int k = pl->y16 ? y1024_freq_of_pos(pos) : host_freq_of_pos(pl->ny, pos);
-        lam[pos] = pl->bc[1] == FLUTAS_BC_PERIODIC ? host_lambda(k, pl->ny, dy) : host_lambda_r2r(k, pl->ny, dy, pl->bc[1]);
+        const int k = pl->y16 ? y1024_freq_of_pos(pos) : host_freq_of_pos(nyf, pl->row0 + pos);
+        lam[pos] = pl->bc[1] == FLUTAS_BC_PERIODIC ? host_lambda(k, nyf, dy) : host_lambda_r2r(k, nyf, dy, pl->bc[1]);
     }
     CUDA_TRY(cudaMemcpy(pl->lam_y, lam.data(), sizeof(double) * pl->ny, cudaMemcpyHostToDevice));
     return FLUTAS_OK;
@@ -192,7 +202,8 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-static int make_spectrum_map(flutas_plan *pl, CUtensorMap *map, int cols, int line_dim, int n, int box_rows = 0) {
+static int make_spectrum_map(flutas_plan *pl, CUtensorMap *map, int cols, int line_dim, int n, int box_rows = 0,
+                             void *base = nullptr) {
     static EncodeTiledFn encode = nullptr;
     if (!encode) {
         void *fn = nullptr;
@@ -206,7 +217,7 @@ static int make_spectrum_map(flutas_plan *pl, CUtensorMap *map, int cols, int li
     const cuuint64_t gstride[2] = {(cuuint64_t)pl->pitch * 16, (cuuint64_t)pl->plane * 16};
     const cuuint32_t box[3] = {(cuuint32_t)(2 * cols), line_dim == 1 ? rows : 1u, line_dim == 2 ? rows : 1u};
     const cuuint32_t estr[3] = {1, 1, 1};
-    const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, pl->spec, gdim, gstride, box, estr,
+    const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base ? base : (void *)pl->spec, gdim, gstride, box, estr,
                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                               cols >= 8 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -215,7 +226,9 @@ static int make_spectrum_map(flutas_plan *pl, CUtensorMap *map, int cols, int li
 }
 
 static int plan_make_maps(flutas_plan *pl) {
-    if (int rc = make_spectrum_map(pl, &pl->map_y, pl->y16 ? Y16Geom::C : pl->y_cols, 1, pl->ny)) return rc;
+    if (pl->role != ROLE_ZLOCAL)
+        if (int rc = make_spectrum_map(pl, &pl->map_y, pl->y16 ? Y16Geom::C : pl->y_cols, 1, pl->ny)) return rc;
+    if (pl->role == ROLE_SLAB) return FLUTAS_OK;
     if (pl->bc_z == FLUTAS_BC_Z_PERIODIC) {
         if (int rc = make_spectrum_map(pl, &pl->map_z, pl->z_cols, 2, pl->nz)) return rc;
     } else if (pl->thomas_variant == 1) {
@@ -252,13 +265,13 @@ static WsLayout plan_layout(const flutas_plan *pl) {
     const size_t fb = sizeof(double) * (size_t)pl->npts, sb = sizeof(double2) * (size_t)pl->nspec;
     WsLayout w{};
     size_t o = 0;
-    w.spec = o; o += align_up(sb);
-    w.rhs = o; o += align_up(fb);
-    w.up = o; o += align_up(fb);
-    w.vp = o; o += align_up(fb);
-    w.wp = o; o += align_up(fb);
+    w.spec = o; if (pl->role == ROLE_FULL) o += align_up(sb);      // slab plans: the spectrum lives in the exchange buffer
+    w.rhs = o; if (pl->role != ROLE_ZLOCAL) o += align_up(fb);
+    w.up = o; if (pl->role != ROLE_ZLOCAL) o += align_up(fb);
+    w.vp = o; if (pl->role != ROLE_ZLOCAL) o += align_up(fb);
+    w.wp = o; if (pl->role != ROLE_ZLOCAL) o += align_up(fb);
     w.zaux = o;
-    if (pl->bc_z == FLUTAS_BC_Z_WALL) {
+    if (pl->bc_z == FLUTAS_BC_Z_WALL && pl->role != ROLE_SLAB) {
         if (ThomasGeom::smem_bytes(pl->nz, thomas_cw(pl)) <= 227 * 1024) {   // coefficient table of the one-pass solve
             const int n_tiles_x = (pl->nxh + ThomasGeom::C - 1) / ThomasGeom::C;
             o += align_up(sizeof(double) * ThomasGeom::tab_doubles(pl->nz, thomas_cw(pl)) * (size_t)n_tiles_x * pl->ny);
@@ -291,7 +304,7 @@ static int plan_attach_workspace(flutas_plan *pl, void *base, bool owned) {
     char *b = (char *)base;
     pl->ws_base = base;
     pl->ws_owned = owned;
-    pl->spec = (double2 *)(b + w.spec);
+    pl->spec = pl->role == ROLE_FULL ? (double2 *)(b + w.spec) : pl->spec_ext;
     pl->rhs = (double *)(b + w.rhs);
     pl->up = (double *)(b + w.up);
     pl->vp = (double *)(b + w.vp);
@@ -300,7 +313,7 @@ static int plan_attach_workspace(flutas_plan *pl, void *base, bool owned) {
     pl->ttab = nullptr;
     // padding columns / the pad row of the spectrum are read (never used) by the strided kernels: keep them finite
     CUDA_TRY(cudaMemset(pl->spec, 0, sizeof(double2) * (size_t)pl->nspec));
-    if (pl->bc_z == FLUTAS_BC_Z_WALL) {
+    if (pl->bc_z == FLUTAS_BC_Z_WALL && pl->role != ROLE_SLAB) {
         if (ThomasGeom::smem_bytes(pl->nz, thomas_cw(pl)) <= 227 * 1024) {
             pl->ttab = (double *)(b + w.zaux);
             if (int rc = build_thomas_table(pl)) return rc;
@@ -322,14 +335,15 @@ static void plan_detach_workspace(flutas_plan *pl) {
 
 static int plan_build(flutas_plan *pl, unsigned flags) {
     const int nx = pl->nx, ny = pl->ny, nz = pl->nz;
-    const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL;
-    const double dx = pl->lx / nx, dy = pl->ly / ny, dz = pl->lz / nz;
+    const bool wall = pl->bc_z == FLUTAS_BC_Z_WALL && pl->role != ROLE_SLAB;   // a slab plan has no z stage
+    const double dx = pl->lx / nx, dy = pl->ly / pl->ny_full, dz = pl->lz / nz;
     const bool same_rho = pl->rho1 == pl->rho2;    // (1 - rho0/rho_f) is then exactly 0 (flux_coef)
     pl->grid = GridParams{nx, ny, nz, pl->bc[2] == FLUTAS_BC_NEUMANN ? 1 : 0, 1.0 / dx, 1.0 / dy, 1.0 / dz, pl->rho1, pl->rho2,
                           pl->rho1 < pl->rho2 ? pl->rho1 : pl->rho2, 2.0, 1.0, same_rho ? 0.0 : 1.0,
                           pl->bc[0] == FLUTAS_BC_NEUMANN ? 1 : 0, pl->bc[1] == FLUTAS_BC_NEUMANN ? 1 : 0};
     plan_geometry(pl);
-    pl->has_null = pl->bc[0] != FLUTAS_BC_DIRICHLET && pl->bc[1] != FLUTAS_BC_DIRICHLET && pl->bc[2] != FLUTAS_BC_DIRICHLET;
+    pl->has_null = pl->bc[0] != FLUTAS_BC_DIRICHLET && pl->bc[1] != FLUTAS_BC_DIRICHLET && pl->bc[2] != FLUTAS_BC_DIRICHLET &&
+                   pl->row0 == 0;                  // the (0, 0) column is on the rank that holds row 0
     pl->end_coef_z = pl->bc[2] == FLUTAS_BC_DIRICHLET ? 3.0 : 1.0;
     pl->y_r2r = pl->bc[1] == FLUTAS_BC_NEUMANN ? 2 : (pl->bc[1] == FLUTAS_BC_DIRICHLET ? 3 : (pl->xsplit ? 1 : 0));
 
@@ -339,7 +353,7 @@ static int plan_build(flutas_plan *pl, unsigned flags) {
     if (int rc = upload(&pl->tw_x, t, &tb)) return rc;
     host_twiddles(ny, t);
     if (int rc = upload(&pl->tw_y, t, &tb)) return rc;
-    if (!wall) {
+    if (!wall && pl->role != ROLE_SLAB) {
         host_twiddles(nz, t);
         if (int rc = upload(&pl->tw_z, t, &tb)) return rc;
     }
@@ -365,10 +379,10 @@ static int plan_build(flutas_plan *pl, unsigned flags) {
         host_wq(ny, t);
         if (int rc = upload(&pl->wq_y, t, &tb)) return rc;
     }
-    pl->y16 = (ny == Y16Geom::N && pl->y_r2r == 0) ? 1 : 0;
+    pl->y16 = (ny == Y16Geom::N && pl->y_r2r == 0 && pl->role == ROLE_FULL) ? 1 : 0;
     CUDA_TRY(cudaMalloc((void **)&pl->lam_y, sizeof(double) * ny));
     if (int rc = upload_lam_y(pl)) return rc;
-    if (!wall) {
+    if (!wall && pl->role != ROLE_SLAB) {
         lam.assign(nz, 0.0);
         for (int pos = 0; pos < nz; ++pos) lam[pos] = host_lambda(host_freq_of_pos(nz, pos), nz, dz);
         if (int rc = upload(&pl->lam_z, lam, &tb)) return rc;
@@ -453,6 +467,7 @@ extern "C" flutas_plan *flutas_plan_create_ex(int nx, int ny, int nz, double lx,
     }
     memset(pl, 0, sizeof(*pl));
     pl->nx = nx; pl->ny = ny; pl->nz = nz;
+    pl->ny_full = ny;
     pl->bc[0] = bc_x; pl->bc[1] = bc_y; pl->bc[2] = bc_z;
     pl->bc_z = bc_z == FLUTAS_BC_PERIODIC ? FLUTAS_BC_Z_PERIODIC : FLUTAS_BC_Z_WALL;
     pl->lx = lx; pl->ly = ly; pl->lz = lz; pl->rho1 = rho1; pl->rho2 = rho2;
@@ -473,6 +488,7 @@ extern "C" size_t flutas_workspace_bytes(int nx, int ny, int nz, int bc_x, int b
     flutas_plan tmp;
     memset(&tmp, 0, sizeof(tmp));
     tmp.nx = nx; tmp.ny = ny; tmp.nz = nz;
+    tmp.ny_full = ny;
     tmp.bc[0] = bc_x; tmp.bc[1] = bc_y; tmp.bc[2] = bc_z;
     tmp.bc_z = bc_z == FLUTAS_BC_PERIODIC ? FLUTAS_BC_Z_PERIODIC : FLUTAS_BC_Z_WALL;
     plan_geometry(&tmp);
@@ -503,6 +519,8 @@ extern "C" void flutas_plan_destroy(flutas_plan *pl) {
     cudaFree(pl->lam_x); cudaFree(pl->lam_y); cudaFree(pl->lam_z); cudaFree(pl->lam_x2);
     cudaFree(pl->wq_x); cudaFree(pl->wq_y);
     cudaFree(pl->sing_coef);
+    cudaFree(pl->sc_dev);
+    delete pl->tpm;
     if (pl->cp_owned) cudaFree(pl->cp);
     plan_detach_workspace(pl);
     for (int i = 0; i < 6; ++i) cudaFree(pl->stage[i]);
@@ -628,7 +646,8 @@ static cudaError_t launch_tma_nc(const CUtensorMap &map, const TmaFftArgs &a, co
         }
     }
     // lines of 2048 (1024 butterflies per tile): the generic kernel, several butterflies per thread (complex transforms only)
-    if constexpr (MODE == MODE_R2R_FWD || MODE == MODE_R2R_INV) return cudaErrorInvalidValue;
+    if constexpr (MODE == MODE_R2R_FWD || MODE == MODE_R2R_INV || MODE == MODE_FWD_SCAT || MODE == MODE_SOLVE_SCAT)
+        return cudaErrorInvalidValue;
     else {
     constexpr int NT = tma_nt(N, C), NBUF = tma_nbuf(N, C);
     const size_t smem = (size_t)NBUF * N * C * 16 + 128;
@@ -663,7 +682,7 @@ static cudaError_t launch_tma(int n, int cols, const CUtensorMap &map, TmaFftArg
     a1.data = data; a1.row_stride = row_stride; a1.outer_stride = outer_stride;
     a1.n_outer = a.n_outer; a1.line_dim = a.line_dim; a1.nxh = a.nxh; a1.tw = a.tw;
     a1.lam_x = a.lam_x; a1.lam_outer = a.lam_outer; a1.lam_pos = a.lam_pos;
-    a1.wq = a.wq; a1.reorder = a.reorder; a1.neg = a.neg;
+    a1.wq = a.wq; a1.reorder = a.reorder; a1.neg = a.neg; a1.sc = a.sc;
     switch (n) {
         case 8: return launch_tma_n<8, MODE>(cols, map, a, a1, st, num_sms);
         case 16: return launch_tma_n<16, MODE>(cols, map, a, a1, st, num_sms);
@@ -841,10 +860,11 @@ static int check_launch(cudaError_t e, const char *what) {
 static bool rhs_takes_ranges(const flutas_plan *pl) {
     return pl->nx % Rhs3Geom::X == 0 && pl->ny % Rhs3Geom::TY == 0;
 }
-static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
-                       const double *p, const double *po, double dt, double dt_ratio, double *rhs, cudaStream_t st,
-                       int k0, int k1) {
-    GridParams g = pl->grid;
+// g: the grid as the kernel is to see it (a slab plan passes its own nz / wall; everyone else pl->grid); up, vp, wp: where
+// the half-corrected velocity goes
+static int enqueue_rhs_g(flutas_plan *pl, GridParams g, const double *u, const double *v, const double *w, const double *phi,
+                         const double *p, const double *po, double dt, double dt_ratio, double *rhs, double *up, double *vp,
+                         double *wp, cudaStream_t st, int k0, int k1) {
     g.c_pn = 1.0 + dt_ratio;    // p_hat = (1 + r) p^n - r p^(n-1)
     g.c_po = dt_ratio;
     const int nk = k1 - k0;
@@ -852,9 +872,9 @@ static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const 
     if (rhs_takes_ranges(pl)) {
         // bulk-copy-fed form: tile = 128 x 8 cells, three plane slabs in shared memory
         const dim3 b3(Rhs3Geom::NTX, Rhs3Geom::TY), g3(pl->nx / Rhs3Geom::X, pl->ny / Rhs3Geom::TY, (nk + kc - 1) / kc);
-        auto k3 = pl->bc_z == FLUTAS_BC_Z_WALL ? splitting_rhs_kernel3<true> : splitting_rhs_kernel3<false>;
+        auto k3 = g.wall ? splitting_rhs_kernel3<true> : splitting_rhs_kernel3<false>;
         if (set_smem(k3, Rhs3Geom::SMEM) != cudaSuccess) return check_launch(cudaGetLastError(), "splitting_rhs attr");
-        k3<<<g3, b3, Rhs3Geom::SMEM, st>>>(g, dt, kc, k0, k1, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+        k3<<<g3, b3, Rhs3Geom::SMEM, st>>>(g, dt, kc, k0, k1, u, v, w, phi, p, po, rhs, up, vp, wp);
         return check_launch(cudaGetLastError(), "splitting_rhs");
     }
     // small grids (nx < 128 or ny < 8 rows per tile): the register-marching form.
@@ -864,11 +884,16 @@ static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const 
     int ty = 256 / bx;
     if (ty > pl->ny) ty = pl->ny;
     dim3 block(bx, ty), grid(pl->nx / 2 / bx, pl->ny / ty, (nk + kc - 1) / kc);
-    if (pl->bc_z == FLUTAS_BC_Z_WALL)
-        splitting_rhs_kernel2<true><<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+    if (g.wall)
+        splitting_rhs_kernel2<true><<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, up, vp, wp);
     else
-        splitting_rhs_kernel2<false><<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, pl->up, pl->vp, pl->wp);
+        splitting_rhs_kernel2<false><<<grid, block, 0, st>>>(g, dt, kc, u, v, w, phi, p, po, rhs, up, vp, wp);
     return check_launch(cudaGetLastError(), "splitting_rhs");
+}
+static int enqueue_rhs(flutas_plan *pl, const double *u, const double *v, const double *w, const double *phi,
+                       const double *p, const double *po, double dt, double dt_ratio, double *rhs, cudaStream_t st,
+                       int k0, int k1) {
+    return enqueue_rhs_g(pl, pl->grid, u, v, w, phi, p, po, dt, dt_ratio, rhs, pl->up, pl->vp, pl->wp, st, k0, k1);
 }
 
 // transform along y (MODE_FWD or MODE_INV) of planes k0 .. k1 - 1 of the half-spectrum
@@ -899,6 +924,11 @@ template <int MODE> static int enqueue_y(flutas_plan *pl, cudaStream_t st, int k
         return check_launch(launch_tma<RMODE>(pl->ny, pl->y_cols, pl->map_y, ty, row_stride, outer_stride, pl->spec,
                                               st, pl->num_sms, k0, k1 - k0), what);
     }
+    if (MODE == MODE_FWD && pl->sc_dev) {   // slab decomposition: the last pass stores into the peers' z-local spectra
+        ty.sc = pl->sc_dev;
+        return check_launch(launch_tma<MODE_FWD_SCAT>(pl->ny, pl->y_cols, pl->map_y, ty, row_stride, outer_stride, pl->spec,
+                                                      st, pl->num_sms, k0, k1 - k0), what);
+    }
     return check_launch(launch_tma<MODE>(pl->ny, pl->y_cols, pl->map_y, ty, row_stride, outer_stride, pl->spec,
                                          st, pl->num_sms, k0, k1 - k0), what);
 }
@@ -915,8 +945,12 @@ static int enqueue_z(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
         tz.lam_x = pl->lam_x;
         tz.lam_outer = pl->lam_y;
         tz.lam_pos = pl->lam_z;
-        if (int rc = check_launch(launch_tma<MODE_SOLVE>(pl->nz, pl->z_cols, pl->map_z, tz, row_stride, outer_stride, pl->spec,
-                                                         st, pl->num_sms, 0, pl->ny), "z_solve")) return rc;
+        if (pl->sc_dev) {   // slab decomposition: the last inverse pass stores into the peers' slab spectra
+            tz.sc = pl->sc_dev;
+            if (int rc = check_launch(launch_tma<MODE_SOLVE_SCAT>(pl->nz, pl->z_cols, pl->map_z, tz, row_stride, outer_stride,
+                                                                  pl->spec, st, pl->num_sms, 0, pl->ny), "z_solve")) return rc;
+        } else if (int rc = check_launch(launch_tma<MODE_SOLVE>(pl->nz, pl->z_cols, pl->map_z, tz, row_stride, outer_stride, pl->spec,
+                                                                st, pl->num_sms, 0, pl->ny), "z_solve")) return rc;
         if (tm) tm->mark();
     } else {
         const long long ncol = (long long)pl->pitch * pl->ny;
@@ -930,12 +964,18 @@ static int enqueue_z(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
             ta.dz2 = 1.0 / inv_dz2;
             ta.has_null = pl->has_null;
             const size_t smem_t = ThomasGeom::smem_bytes(pl->nz, thomas_cw(pl));
-            auto kern = pl->xsplit ? (pl->thomas_warps == 2 ? thomas_tma_kernel<2, 16> : thomas_tma_kernel<1, 16>)
+            static const ThomasPeerMaps no_peers{};
+            if (pl->sc_dev) {   // slab decomposition: the solved tile goes to the ranks that own its planes
+                ta.n_peers = pl->sc_npeers; ta.nzl = pl->sc_nzl; ta.srows = pl->sc_srows;
+                ta.row0 = pl->row0; ta.nxh = pl->nxh; ta.sc = pl->sc_dev;
+            }
+            auto kern = pl->sc_dev ? (pl->thomas_warps == 2 ? thomas_tma_kernel<2, 8, true> : thomas_tma_kernel<1, 8, true>)
+                      : pl->xsplit ? (pl->thomas_warps == 2 ? thomas_tma_kernel<2, 16> : thomas_tma_kernel<1, 16>)
                                    : (pl->thomas_warps == 2 ? thomas_tma_kernel<2, 8> : thomas_tma_kernel<1, 8>);
             if (set_smem(kern, smem_t) != cudaSuccess) return check_launch(cudaGetLastError(), "z_solve attr");
             long long grid = pl->num_sms;
             if (grid > (long long)ta.n_tiles_x * ta.ny) grid = (long long)ta.n_tiles_x * ta.ny;
-            kern<<<(unsigned)grid, 32 * (pl->thomas_warps + 1), smem_t, st>>>(pl->map_z, ta);
+            kern<<<(unsigned)grid, 32 * (pl->thomas_warps + 1), smem_t, st>>>(pl->map_z, ta, pl->sc_dev ? *pl->tpm : no_peers);
         } else {
             thomas_kernel<<<(unsigned)((ncol + 127) / 128), 128, 0, st>>>(pl->spec, pl->cp, pl->pitch, pl->ny, pl->nz, pl->nxh,
                                                                         pl->lam_x, pl->lam_y, inv_dz2, pl->plane, pl->end_coef_z, pl->has_null);
@@ -946,7 +986,7 @@ static int enqueue_z(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
         const size_t smem = sizeof(double) * (4 * (size_t)pl->nz + 2);
         // nz <= 4096 (checked at plan creation): at most 128 KB
         if (set_smem(thomas_singular_kernel, smem) != cudaSuccess) return check_launch(cudaGetLastError(), "z_singular attr");
-        thomas_singular_kernel<<<1, 256, smem, st>>>(pl->spec, pl->plane, pl->nz, pl->sing_coef, pl->xsplit);
+        thomas_singular_kernel<<<1, 256, smem, st>>>(pl->spec, pl->plane, pl->nz, pl->sing_coef, pl->xsplit, pl->sc_dev);
         if (int rc = check_launch(cudaGetLastError(), "z_singular")) return rc;
         if (tm) tm->mark();
     }
@@ -954,13 +994,17 @@ static int enqueue_z(flutas_plan *pl, cudaStream_t st, StepTimer *tm) {
 }
 
 // planes k0 .. k1 - 1 of u, v, w (reads p^(n+1) of planes k0 .. k1, wrapped)
-static int enqueue_correction(flutas_plan *pl, double dt, const double *pn, double *u, double *v, double *w,
-                              cudaStream_t st, int k0, int k1) {
+static int enqueue_correction_g(flutas_plan *pl, const GridParams &g, double dt, const double *pn, double *u, double *v, double *w,
+                                cudaStream_t st, int k0, int k1) {
     if (k1 <= k0) return FLUTAS_OK;
     const long long plane = (long long)pl->nx * pl->ny, q0 = k0 * plane, q1 = k1 * plane;
     const unsigned nb = (unsigned)(((q1 - q0) / 2 + 255) / 256);   // two points per thread
-    correction_kernel<<<nb, 256, 0, st>>>(pl->grid, dt, q0, q1, pn, pl->up, pl->vp, pl->wp, u, v, w);
+    correction_kernel<<<nb, 256, 0, st>>>(g, dt, q0, q1, pn, pl->up, pl->vp, pl->wp, u, v, w);
     return check_launch(cudaGetLastError(), "correction");
+}
+static int enqueue_correction(flutas_plan *pl, double dt, const double *pn, double *u, double *v, double *w,
+                              cudaStream_t st, int k0, int k1) {
+    return enqueue_correction_g(pl, pl->grid, dt, pn, u, v, w, st, k0, k1);
 }
 
 static double norm_scale(const flutas_plan *pl) {
@@ -1293,3 +1337,6 @@ extern "C" int flutas_plan_read_timing(flutas_plan *pl, float *ms_out, int n_out
     pl->pending = 0;
     return FLUTAS_OK;
 }
+
+// -------------------------------------------------------------------------------------- z-slab decomposition (NEXT-3)
+#include "flutas_slab.inl"

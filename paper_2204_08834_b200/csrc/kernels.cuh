@@ -244,7 +244,56 @@ __device__ __forceinline__ void tile_fft(double2 *s, const double2 *__restrict__
 }
 
 // modes of the strided transform kernels (kernels_tma.cuh, kernels_y16.cuh)
-enum { MODE_FWD = 0, MODE_INV = 1, MODE_SOLVE = 2, MODE_R2R_FWD = 3, MODE_R2R_INV = 4 };
+enum { MODE_FWD = 0, MODE_INV = 1, MODE_SOLVE = 2, MODE_R2R_FWD = 3, MODE_R2R_INV = 4,
+       MODE_FWD_SCAT = 5, MODE_SOLVE_SCAT = 6 };   // MODE_FWD / MODE_SOLVE whose last pass stores into the peers' arrays
+
+// ------------------------------------------------------------------------------------------------
+// z-slab decomposition over several GPUs: the two all-to-all
+// transposes around the z stage are the STORE stage of the transform before them.  The last pass of a transform
+// along a line whose positions are dealt out to the ranks in equal blocks writes position r of the line
+//     to   base[r / rows_per_peer] + ((r % rows_per_peer) + lead) * row_stride + (outer + outer_off) * outer_stride + kx
+// (base[]: the same array of every rank, mapped into this process: NVLink peer memory, or plain device memory when
+// the ranks share a device).  halo = 1: the first / last position of every block is also written one row past the
+// end / before the start of the neighbouring rank's block (the plane above / below a slab: what the velocity
+// correction and the next step's right-hand side need from the neighbour), wrapping around when wrap = 1.
+// ------------------------------------------------------------------------------------------------
+constexpr int kMaxRanks = 16;
+struct PeerScatter {
+    int shift;                 // log2(rows_per_peer)
+    int lead;                  // rows before a rank's block in its array (1 with halo planes, else 0)
+    int halo, wrap, n_peers;
+    long long row_stride, outer_stride, outer_off;   // of the destination arrays, in elements
+    double2 *base[kMaxRanks];
+};
+// the scalar members live in registers (ScatterRegs), the peers' base pointers are fetched through the read-only path
+struct ScatterRegs {
+    int shift, lead, halo, wrap, n_peers;
+    long long row_stride, outer_stride, outer_off;
+    const PeerScatter *desc;
+    __device__ __forceinline__ void load(const PeerScatter *d) {
+        desc = d;
+        shift = d->shift; lead = d->lead; halo = d->halo; wrap = d->wrap; n_peers = d->n_peers;
+        row_stride = d->row_stride; outer_stride = d->outer_stride; outer_off = d->outer_off;
+    }
+    __device__ __forceinline__ double2 *base(int peer) const {
+        return reinterpret_cast<double2 *>(__ldg(reinterpret_cast<const unsigned long long *>(&desc->base[peer])));
+    }
+};
+__device__ __forceinline__ void scatter_store(const ScatterRegs &sc, int r, long long outer, int kx, double2 v) {
+    const int rpp = 1 << sc.shift, peer = r >> sc.shift, loc = r & (rpp - 1);
+    const long long off = (outer + sc.outer_off) * sc.outer_stride + kx;
+    sc.base(peer)[(long long)(loc + sc.lead) * sc.row_stride + off] = v;
+    if (sc.halo) {
+        if (loc == 0) {                                    // the plane above the slab of the rank below
+            const int q = peer > 0 ? peer - 1 : (sc.wrap ? sc.n_peers - 1 : -1);
+            if (q >= 0) sc.base(q)[(long long)(rpp + sc.lead) * sc.row_stride + off] = v;
+        }
+        if (loc == rpp - 1) {                              // the plane below the slab of the rank above
+            const int q = peer + 1 < sc.n_peers ? peer + 1 : (sc.wrap ? 0 : -1);
+            if (q >= 0) sc.base(q)[off] = v;
+        }
+    }
+}
 
 // ------------------------------------------------------------------------------------------------
 // Cooperative copy of TOT contiguous elements with B loads in flight per thread: all loads of a batch are
@@ -412,8 +461,10 @@ thomas_kernel(double2 *__restrict__ spec, double *__restrict__ cp, int pitch, in
 // The (kx,ky) = (0,0) column: lam_xy = 0, the system is singular (pure Neumann).  Eliminate rows
 // 0..nz-2, pin x_{nz-1} = 0, back-substitute, then remove the mean over k (zero-mean gauge, R5).
 // re_only: with non-periodic x the imaginary part of column 0 is another (regular) mode and is left alone.
+// sc != nullptr (z-slab decomposition): the solved column goes to the ranks that own its planes instead of back in place.
 __global__ void thomas_singular_kernel(double2 *__restrict__ spec, long long col_stride, int nz,
-                                       const double *__restrict__ coef /* inv_k, c'_k interleaved: 2 nz doubles */, int re_only) {
+                                       const double *__restrict__ coef /* inv_k, c'_k interleaved: 2 nz doubles */, int re_only,
+                                       const PeerScatter *__restrict__ sc) {
     extern __shared__ double sm[];
     double *dr = sm, *di = sm + nz, *cf = sm + 2 * nz, *mean = sm + 4 * nz;
     for (int k = threadIdx.x; k < nz; k += blockDim.x) {
@@ -445,6 +496,12 @@ __global__ void thomas_singular_kernel(double2 *__restrict__ spec, long long col
     }
     __syncthreads();
     const double mr = mean[0], mi = mean[1];
+    if (sc) {
+        ScatterRegs scr;
+        scr.load(sc);
+        for (int k = threadIdx.x; k < nz; k += blockDim.x) scatter_store(scr, k, 0, 0, make_double2(dr[k] - mr, di[k] - mi));
+        return;
+    }
     for (int k = threadIdx.x; k < nz; k += blockDim.x)
         spec[(long long)k * col_stride] = make_double2(dr[k] - mr, di[k] - mi);
 }

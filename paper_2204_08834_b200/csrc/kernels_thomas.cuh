@@ -101,10 +101,16 @@ struct ThomasArgs {
     int n_tiles_x, ny, nz;
     double dz2;               // 1 / a
     int has_null;             // the (0, 0) mode is left to thomas_singular_kernel
+    // SCAT (z-slab decomposition, kernels.cuh PeerScatter): the solved tile goes to the ranks that own its planes
+    int n_peers, nzl, srows;  // ranks, planes per rank, rows per store box (divides nzl, <= 256)
+    int row0, nxh;            // this rank's first row of ky in the peers' slab spectra; valid kx columns
+    const PeerScatter *sc;    // row_stride = plane of a slab spectrum (for the two halo planes, written with plain stores)
 };
+struct ThomasPeerMaps { CUtensorMap m[kMaxRanks]; };   // the peers' slab spectra, box {16, 1, srows}
 
-template <int NWARP, int CW>
-__global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const __grid_constant__ CUtensorMap tmap, ThomasArgs a) {
+template <int NWARP, int CW, bool SCAT = false>
+__global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const __grid_constant__ CUtensorMap tmap, ThomasArgs a,
+                                                                         const __grid_constant__ ThomasPeerMaps pm) {
     using G = ThomasGeom;
     static_assert(CW == 8 || CW == 16, "coefficient columns per tile");
     extern __shared__ unsigned char smem_raw[];
@@ -152,9 +158,35 @@ __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const _
         const long long tile = tile_of(n);
         const int tx = (int)(tile % a.n_tiles_x), jy = (int)(tile / a.n_tiles_x);
         const int b = (int)(n % G::NBUF);
-        for (int c = 0; c < nbox; ++c)
-            tma_store_3d(&tmap, base + b * buf_stride + c * box_bytes, tx * 2 * G::C, jy, c * rows);
+        if constexpr (SCAT) {
+            // rows r nzl .. (r + 1) nzl - 1 of the tile are planes 1 .. nzl of rank r's slab spectrum
+            for (int r = 0; r < a.n_peers; ++r)
+                for (int c = 0; c < a.nzl; c += a.srows)
+                    tma_store_3d(&pm.m[r], base + b * buf_stride + (uint32_t)(r * a.nzl + c) * (G::C * 16u), tx * 2 * G::C,
+                                 a.row0 + jy, 1 + c);
+        } else {
+            for (int c = 0; c < nbox; ++c)
+                tma_store_3d(&tmap, base + b * buf_stride + c * box_bytes, tx * 2 * G::C, jy, c * rows);
+        }
         bulk_commit();
+    };
+    // SCAT: the planes next to a slab boundary also go to the neighbour's halo planes (walls: no wrap-around); 8 columns
+    // x 2 (P - 1) rows, plain stores by the lanes of the copy warp
+    auto store_halos = [&](long long n) {
+        const long long tile = tile_of(n);
+        const int tx = (int)(tile % a.n_tiles_x), jy = (int)(tile / a.n_tiles_x);
+        const int b = (int)(n % G::NBUF);
+        const double2 *sd = reinterpret_cast<const double2 *>(base + b * buf_stride);
+        const long long plane_s = a.sc->row_stride, row_off = (long long)(a.row0 + jy) * a.sc->outer_stride;
+        for (int item = threadIdx.x & 31; item < 2 * (a.n_peers - 1) * G::C; item += 32) {
+            const int c = item % G::C, e = item / G::C, r = e >> 1, up = e & 1;   // boundary between ranks r and r + 1
+            const int kx = tx * G::C + c;
+            if (kx >= a.nxh) continue;
+            // up = 0: the last plane of rank r -> plane 0 (below) of rank r + 1; up = 1: the first plane of rank r + 1 -> plane nzl + 1 of rank r
+            const int row = (r + 1) * a.nzl - 1 + up;
+            double2 *dst = up ? a.sc->base[r] + (long long)(a.nzl + 1) * plane_s : a.sc->base[r + 1];
+            dst[row_off + kx] = sd[row * G::C + c];
+        }
     };
 
     if (threadIdx.x == 0) {
@@ -169,17 +201,24 @@ __global__ void __launch_bounds__(32 * (NWARP + 1), 1) thomas_tma_kernel(const _
     if (warp == NWARP) {
         // ---- the copy warp: as tiles are reported solved (in order), write them back, refill the table buffer at
         //      once and the data buffer as soon as the store has drained it.  The solving warps never wait for a drain.
-        if (lane == 0) {
+        if (SCAT || lane == 0) {
             for (long long n = 0; n < my_tiles; ++n) {
                 mbar_wait(&done[n % G::NBUF], (uint32_t)(n / G::NBUF) & 1);
-                issue_store(n);
-                if (n + G::NTAB < my_tiles) issue_table(n + G::NTAB);
-                if (n + G::NBUF < my_tiles) {
-                    bulk_wait_read<0>();
-                    issue_data(n + G::NBUF);
+                if constexpr (SCAT) {
+                    store_halos(n);
+                    __syncwarp();          // every lane has read its halo rows before the buffer can be refilled
                 }
+                if (lane == 0) {
+                    issue_store(n);
+                    if (n + G::NTAB < my_tiles) issue_table(n + G::NTAB);
+                    if (n + G::NBUF < my_tiles) {
+                        bulk_wait_read<0>();
+                        issue_data(n + G::NBUF);
+                    }
+                }
+                if constexpr (SCAT) __syncwarp();
             }
-            bulk_wait_all<0>();
+            if (lane == 0) bulk_wait_all<0>();
         }
         return;
     }

@@ -40,6 +40,7 @@ struct TmaFftArgs {
     const double *lam_x, *lam_outer, *lam_pos;    // SOLVE: eigenvalues in storage (permuted) order
     const double2 *wq;                            // MODE_R2R_*: see Tma1Args
     int reorder, neg;
+    const PeerScatter *sc;                        // MODE_*_SCAT: see Tma1Args
 };
 
 // reciprocal of a normal, non-zero double (either sign): hardware seed + two Newton steps, <= ~1 ulp
@@ -213,6 +214,7 @@ struct Tma1Args {
     const double2 *wq;       // e^{-i pi k / (2N)}, k = 0 .. N/2 (cosine / sine expansion); nullptr = half-complex (w = 1)
     int reorder;             // 1: rows enter as v[n] = z[2n], v[N-1-n] = z[2n+1] (cosine / sine), 0: as they are
     int neg;                 // 1: the odd rows change sign (sine expansion)
+    const PeerScatter *sc;   // MODE_FWD_SCAT / MODE_SOLVE_SCAT: where the last pass stores (device memory, plan-owned)
 };
 
 template <int N, int P_IDX> struct PassGeom {     // geometry of pass P_IDX (1-based) for one thread
@@ -266,9 +268,11 @@ template <int N, int C, int P_IDX> __device__ __forceinline__ void exchange_sync
     else asm volatile("bar.sync %0, %1;" ::"r"(1 + tid / GS), "n"(GS) : "memory");
 }
 
-template <int N, int C, int MODE, int NT, int NCACHE>
+template <int N, int C, int MODE_T, int NT, int NCACHE>
 __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__ CUtensorMap tmap, Tma1Args a) {
     static_assert(NT == N * C / 8 || (N * C / 8 < 32 && NT == 32), "one butterfly per thread");
+    constexpr bool SCAT = MODE_T == MODE_FWD_SCAT || MODE_T == MODE_SOLVE_SCAT;
+    constexpr int MODE = MODE_T == MODE_FWD_SCAT ? MODE_FWD : (MODE_T == MODE_SOLVE_SCAT ? MODE_SOLVE : MODE_T);
     extern __shared__ unsigned char smem_raw[];
     constexpr int P = Fact<N>::P;
     constexpr int ROWS = N < 256 ? N : 256, NBOX = N / ROWS;
@@ -340,14 +344,22 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
 #pragma unroll
         for (int e = 0; e < 8; ++e) sp[e * G::M * C] = v[e];
     };
+    ScatterRegs sc;                       // the peers' arrays (distributed spectrum)
+    if constexpr (SCAT) sc.load(a.sc);
+    int st_outer = 0, st_kx = 0;          // outer index and column of the tile being stored (SCAT)
     auto global_store = [&](auto pidx, double2 *gp, bool valid, const double2 *v) {
         constexpr int PI = decltype(pidx)::value;
         using G = PassGeom<N, PI>;
         if (valid) {
-            double2 *q = gp + (long long)G::base(t) * a.row_stride;
-            const long long step = (long long)G::M * a.row_stride;
+            if constexpr (SCAT) {
 #pragma unroll
-            for (int e = 0; e < 8; ++e) q[e * step] = v[e];
+                for (int e = 0; e < 8; ++e) scatter_store(sc, G::base(t) + e * G::M, st_outer, st_kx, v[e]);
+            } else {
+                double2 *q = gp + (long long)G::base(t) * a.row_stride;
+                const long long step = (long long)G::M * a.row_stride;
+#pragma unroll
+                for (int e = 0; e < 8; ++e) q[e * step] = v[e];
+            }
         }
     };
 
@@ -366,6 +378,7 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
         const int kx = tx * C + l;
         const bool valid = active && kx < a.nxh;
         double2 *gp = a.data + (long long)outer * a.outer_stride + kx;
+        st_outer = outer; st_kx = kx;
         double2 *s = bufs + b * TILE_ELEMS;
         mbar_wait(&full[b], (it >> 1) & 1);
 

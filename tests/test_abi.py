@@ -89,7 +89,7 @@ def test_product_never_imports_the_oracle():
     pkg = os.path.join(ROOT, "paper_2204_08834_b200")
     for dirpath, _, files in os.walk(pkg):
         for f in files:
-            if f.endswith((".py", ".cu", ".cuh", ".h")):
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".inl")):
                 text = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in text.lower(), f
     text = open(os.path.join(ROOT, "workloads.py")).read()          # the shared input generators import neither side

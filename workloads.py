@@ -326,4 +326,31 @@ def cavity(nx=256, ny=256, nz=64, ratio=1.0, seed=6):
     return _zero_wall_faces(W)
 
 
+# ------------------------------------------------------------------- z-slab decomposition
+
+def slab_split(a, n_ranks, periodic):
+    """Cut a field of shape (nz, ny, nx) into n_ranks local arrays of shape (nz / n_ranks + 2, ny, nx): plane 0 is the
+    plane below the slab, planes 1 .. nzl the slab, plane nzl + 1 the plane above (wrapped around when `periodic`, NaN
+    beyond a wall so that a kernel that reads it is found out).  Pure data movement: no arithmetic of the method."""
+    nz = a.shape[0]
+    assert nz % n_ranks == 0
+    nzl = nz // n_ranks
+    out = []
+    for r in range(n_ranks):
+        loc = np.full((nzl + 2,) + a.shape[1:], np.nan)
+        loc[1:nzl + 1] = a[r * nzl:(r + 1) * nzl]
+        lo, hi = r * nzl - 1, (r + 1) * nzl
+        if lo >= 0 or periodic:
+            loc[0] = a[lo % nz]
+        if hi < nz or periodic:
+            loc[nzl + 1] = a[hi % nz]
+        out.append(loc)
+    return out
+
+
+def slab_gather(parts):
+    """the inverse of slab_split for the owned planes: concatenates planes 1 .. nzl of every local array"""
+    return np.concatenate([q[1:-1] for q in parts], axis=0)
+
+
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
