@@ -265,31 +265,27 @@ struct PeerScatter {
     long long row_stride, outer_stride, outer_off;   // of the destination arrays, in elements
     double2 *base[kMaxRanks];
 };
-// the scalar members live in registers (ScatterRegs), the peers' base pointers are fetched through the read-only path
+// The descriptor is read where it is used, through a volatile pointer (shared memory in the transform kernels), so that
+// it does not sit in registers across the butterfly passes (those kernels are at their register limit).
 struct ScatterRegs {
-    int shift, lead, halo, wrap, n_peers;
-    long long row_stride, outer_stride, outer_off;
-    const PeerScatter *desc;
-    __device__ __forceinline__ void load(const PeerScatter *d) {
-        desc = d;
-        shift = d->shift; lead = d->lead; halo = d->halo; wrap = d->wrap; n_peers = d->n_peers;
-        row_stride = d->row_stride; outer_stride = d->outer_stride; outer_off = d->outer_off;
-    }
-    __device__ __forceinline__ double2 *base(int peer) const {
-        return reinterpret_cast<double2 *>(__ldg(reinterpret_cast<const unsigned long long *>(&desc->base[peer])));
-    }
+    const volatile PeerScatter *d;
+    __device__ __forceinline__ void load(const PeerScatter *desc) { d = desc; }
+    __device__ __forceinline__ double2 *base(int peer) const { return d->base[peer]; }
 };
 __device__ __forceinline__ void scatter_store(const ScatterRegs &sc, int r, long long outer, int kx, double2 v) {
-    const int rpp = 1 << sc.shift, peer = r >> sc.shift, loc = r & (rpp - 1);
-    const long long off = (outer + sc.outer_off) * sc.outer_stride + kx;
-    sc.base(peer)[(long long)(loc + sc.lead) * sc.row_stride + off] = v;
-    if (sc.halo) {
+    const int shift = sc.d->shift, lead = sc.d->lead;
+    const int rpp = 1 << shift, peer = r >> shift, loc = r & (rpp - 1);
+    const long long row_stride = sc.d->row_stride;
+    const long long off = (outer + sc.d->outer_off) * sc.d->outer_stride + kx;
+    sc.base(peer)[(long long)(loc + lead) * row_stride + off] = v;
+    if (sc.d->halo) {
+        const int n_peers = sc.d->n_peers, wrap = sc.d->wrap;
         if (loc == 0) {                                    // the plane above the slab of the rank below
-            const int q = peer > 0 ? peer - 1 : (sc.wrap ? sc.n_peers - 1 : -1);
-            if (q >= 0) sc.base(q)[(long long)(rpp + sc.lead) * sc.row_stride + off] = v;
+            const int q = peer > 0 ? peer - 1 : (wrap ? n_peers - 1 : -1);
+            if (q >= 0) sc.base(q)[(long long)(rpp + lead) * row_stride + off] = v;
         }
         if (loc == rpp - 1) {                              // the plane below the slab of the rank above
-            const int q = peer + 1 < sc.n_peers ? peer + 1 : (sc.wrap ? 0 : -1);
+            const int q = peer + 1 < n_peers ? peer + 1 : (wrap ? 0 : -1);
             if (q >= 0) sc.base(q)[off] = v;
         }
     }

@@ -285,6 +285,12 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
     const int l = tid % C, t = tid / C;
     const bool active = t < N / 8;           // only false for the tiny sizes padded to one warp
     const int ntiles = a.n_tiles_x * a.n_outer;
+    __shared__ PeerScatter sc_s;             // the peers' arrays (distributed spectrum), copied once per CTA
+    if constexpr (SCAT) {
+        static_assert(sizeof(PeerScatter) % 8 == 0, "copied as 8-byte words");
+        for (int i = tid; i < (int)(sizeof(PeerScatter) / 8); i += NT)
+            reinterpret_cast<unsigned long long *>(&sc_s)[i] = reinterpret_cast<const unsigned long long *>(a.sc)[i];
+    }
     if (tid == 0) {
         mbar_init(&full[0], 1);
         mbar_init(&full[1], 1);
@@ -344,8 +350,8 @@ __global__ void __launch_bounds__(NT, 1) fft_tma1_kernel(const __grid_constant__
 #pragma unroll
         for (int e = 0; e < 8; ++e) sp[e * G::M * C] = v[e];
     };
-    ScatterRegs sc;                       // the peers' arrays (distributed spectrum)
-    if constexpr (SCAT) sc.load(a.sc);
+    ScatterRegs sc;
+    sc.load(&sc_s);
     int st_outer = 0, st_kx = 0;          // outer index and column of the tile being stored (SCAT)
     auto global_store = [&](auto pidx, double2 *gp, bool valid, const double2 *v) {
         constexpr int PI = decltype(pidx)::value;
