@@ -1236,13 +1236,13 @@ extern "C" int flutas_vof_step(flutas_plan *pl, const double *phi, const double 
     if (!pl->ws_base) return fail(FLUTAS_ERR_INVALID_ARG, "the plan has no workspace (flutas_plan_set_workspace)");
     cudaStream_t st = (cudaStream_t)stream;
     const GridParams g = pl->grid;
-    const unsigned nb = (unsigned)((pl->npts + 255) / 256);
+    const unsigned nb = (unsigned)((pl->npts + 255) / 256), nbf = (unsigned)((pl->npts + VofTile::CELLS - 1) / VofTile::CELLS);
     double *flux = pl->rhs, *px = pl->up, *py = pl->vp, *pz = pl->wp;
-    vof_flux_kernel<0><<<nb, 256, 0, st>>>(g, beta, dt, phi, u, flux);
+    vof_flux_kernel<0><<<nbf, VofTile::NT, 0, st>>>(g, beta, dt, phi, u, flux);
     vof_update_kernel<0><<<nb, 256, 0, st>>>(g, dt, phi, u, flux, px);
-    vof_flux_kernel<1><<<nb, 256, 0, st>>>(g, beta, dt, px, v, flux);
+    vof_flux_kernel<1><<<nbf, VofTile::NT, 0, st>>>(g, beta, dt, px, v, flux);
     vof_update_kernel<1><<<nb, 256, 0, st>>>(g, dt, px, v, flux, py);
-    vof_flux_kernel<2><<<nb, 256, 0, st>>>(g, beta, dt, py, w, flux);
+    vof_flux_kernel<2><<<nbf, VofTile::NT, 0, st>>>(g, beta, dt, py, w, flux);
     vof_update_kernel<2><<<nb, 256, 0, st>>>(g, dt, py, w, flux, pz);
     vof_final_kernel<<<nb, 256, 0, st>>>(g, dt, px, py, pz, u, v, w, phi_out);
     return check_launch(cudaGetLastError(), "vof_step");

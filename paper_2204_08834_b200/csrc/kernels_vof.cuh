@@ -17,8 +17,9 @@
 //       (eps, 1 - eps), no transcendental function inside the iteration; the closed-form route A.17-A.21 is not used);
 //   fluxes: exact integration of tanh along the sweep direction, 2 x 2 Gauss points across it (A.23-A.31).
 //
-// vof_flux_kernel<DIR>: one thread per cell; a cell writes the flux of the faces it is the donor of (its + face when
-// the velocity there is >= 0, its - face when the velocity there is < 0): every face is written exactly once.
+// vof_flux_kernel<DIR>: a cell writes the flux of the faces it is the donor of (its + face when the velocity there is >= 0,
+// its - face when the velocity there is < 0): every face is written exactly once.  The cells that carry a reconstruction
+// are compacted per block before they are worked on (see the kernel).
 // vof_update_kernel<DIR>: eq. (11).  vof_final_kernel: eq. (12).
 #pragma once
 #include "kernels.cuh"
@@ -28,32 +29,27 @@ namespace flutas {
 constexpr double kVofEps = 1e-8;
 constexpr double kGauss0 = 0.5 - 0.28867513459481288225457439025098, kGauss1 = 0.5 + 0.28867513459481288225457439025098;
 
-// int_a^b 1/2 [1 + tanh(beta (alpha x + gamma))] dx
-__device__ __forceinline__ double tanh_integral_dev(double a, double b, double alpha, double gamma, double beta) {
-    if (fabs(alpha) < 1e-12) return (b - a) * 0.5 * (1.0 + tanh(beta * gamma));
-    // ln cosh(xb) - ln cosh(xa) with ln cosh(x) = |x| + ln(1 + e^(-2|x|)) - ln 2: one logarithm for the pair
-    const double xb = fabs(beta * (alpha * b + gamma)), xa = fabs(beta * (alpha * a + gamma));
-    const double lc = (xb - xa) + log((1.0 + exp(-2.0 * xb)) / (1.0 + exp(-2.0 * xa)));
-    return 0.5 * ((b - a) + lc / (beta * alpha));
-}
-// mean of H^ over x~_dir in [a, b] x the unit square across it
-__device__ __forceinline__ double hat_integral_dev(double nd, double n1, double n2, double d, double a, double b, double beta) {
-    double s = tanh_integral_dev(a, b, nd, n1 * kGauss0 + n2 * kGauss0 + d, beta);
-    s += tanh_integral_dev(a, b, nd, n1 * kGauss0 + n2 * kGauss1 + d, beta);
-    s += tanh_integral_dev(a, b, nd, n1 * kGauss1 + n2 * kGauss0 + d, beta);
-    s += tanh_integral_dev(a, b, nd, n1 * kGauss1 + n2 * kGauss1 + d, beta);
-    return 0.25 * s;
-}
+// Everything transcendental in a cell is an exponential of 2 beta n_c x~_c at a Gauss point or a cell face, so the
+// reconstruction keeps the six numbers E[c][g] = e^{2 beta n_c g_g} (c = x, y, z; g_0, g_1 the Gauss points) and
+// D = e^{2 beta d} instead of d itself:
+//   * e^{2 beta (n . x~ + d)} at a Gauss point across a direction is a product of two E's and D;
+//   * the volume constraint (A.14-A.16) is a polynomial in D whose coefficients are such products;
+//   * with T(x) = e^{2 beta (alpha x + gamma)}:  int_a^b 1/2 [1 + tanh(beta (alpha x + gamma))] dx = ln[(1 + T(b)) / (1 + T(a))] / (2 beta alpha)
+//     (ln cosh z = ln(e^{2z} + 1) - z - ln 2), so the mean over the four Gauss points across the sweep is ONE logarithm, of
+//     the product of the four ratios, and T(a), T(b) are E_a G_i D, E_b G_i D with one new exponential per face.
+// Per reconstructed cell and sweep: 8 exponentials and 1 logarithm (the first form of this kernel: 15 and 5).
+struct VofRecon {
+    double n[3];
+    double E[3][2];      // e^{2 beta n_c g0}, e^{2 beta n_c g1}
+    double D;            // e^{2 beta d}
+    bool flat;           // no reconstruction: the cell carries the constant state phi
+};
 
-struct VofRecon { double n[3]; double d; bool flat; };
-
-// reconstruction of cell (i, j, k) from the field f (periodic)
-__device__ __forceinline__ void vof_reconstruct(const GridParams &g, const double *__restrict__ f, int i, int j, int k, double beta,
-                                                VofRecon &r) {
+// reconstruction of cell (i, j, k), phi(i, j, k) = fc in (eps, 1 - eps), from the field f (periodic)
+__device__ __forceinline__ void vof_reconstruct(const GridParams &g, const double *__restrict__ f, int i, int j, int k, double fc,
+                                                double beta, VofRecon &r) {
     const long long sy = g.nx, sz = (long long)g.nx * g.ny;
-    const double fc = f[i + sy * j + sz * k];
-    r.flat = true; r.d = 0.0; r.n[0] = r.n[1] = r.n[2] = 0.0;
-    if (!(fc > kVofEps && fc < 1.0 - kVofEps)) return;
+    r.flat = true; r.D = 1.0; r.n[0] = r.n[1] = r.n[2] = 0.0;
     int ii[3] = {i == 0 ? g.nx - 1 : i - 1, i, i == g.nx - 1 ? 0 : i + 1};
     int jj[3] = {j == 0 ? g.ny - 1 : j - 1, j, j == g.ny - 1 ? 0 : j + 1};
     int kk[3] = {k == 0 ? g.nz - 1 : k - 1, k, k == g.nz - 1 ? 0 : k + 1};
@@ -85,15 +81,22 @@ __device__ __forceinline__ void vof_reconstruct(const GridParams &g, const doubl
     if (!(mag > 1e-12)) return;
     r.flat = false;
     r.n[0] = m0 / mag; r.n[1] = m1 / mag; r.n[2] = m2 / mag;
-    const double ax = fabs(r.n[0]), ay = fabs(r.n[1]), az = fabs(r.n[2]);
-    const int dir = (ax >= ay && ax >= az) ? 0 : ((ay >= az) ? 1 : 2);
-    const double nd = r.n[dir], n1 = r.n[(dir + 1) % 3], n2 = r.n[(dir + 2) % 3];
-    // prod_i (A B_i D + 1) = Q prod_i (B_i D + 1)   (A.14-A.16 with Q here = A^2 Q_paper)
     const double tb = 2.0 * beta;
-    const double A = exp(tb * nd), Q = exp(4.0 * tb * nd * fc);
-    const double B0 = exp(tb * (n1 * kGauss0 + n2 * kGauss0)), B1 = exp(tb * (n1 * kGauss0 + n2 * kGauss1));
-    const double B2 = exp(tb * (n1 * kGauss1 + n2 * kGauss0)), B3 = exp(tb * (n1 * kGauss1 + n2 * kGauss1));
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        r.E[c][0] = exp(tb * r.n[c] * kGauss0);
+        r.E[c][1] = exp(tb * r.n[c] * kGauss1);
+    }
+    const double ax = fabs(r.n[0]), ay = fabs(r.n[1]), az = fabs(r.n[2]);
+    const int dir = (ax >= ay && ax >= az) ? 0 : ((ay >= az) ? 1 : 2);     // direction of exact integration (cases 1-3)
+    const double nd = dir == 0 ? r.n[0] : (dir == 1 ? r.n[1] : r.n[2]);
+    const double A = dir == 0 ? r.E[0][0] * r.E[0][1] : (dir == 1 ? r.E[1][0] * r.E[1][1] : r.E[2][0] * r.E[2][1]);   // e^{2 beta n_dir}
+    const double P0 = dir == 0 ? r.E[1][0] : (dir == 1 ? r.E[2][0] : r.E[0][0]), P1 = dir == 0 ? r.E[1][1] : (dir == 1 ? r.E[2][1] : r.E[0][1]);
+    const double R0 = dir == 0 ? r.E[2][0] : (dir == 1 ? r.E[0][0] : r.E[1][0]), R1 = dir == 0 ? r.E[2][1] : (dir == 1 ? r.E[0][1] : r.E[1][1]);
+    // prod_i (A B_i D + 1) = Q prod_i (B_i D + 1)   (A.14-A.16 with Q here = A^2 Q_paper), B_i = e^{2 beta a_i}
+    const double B0 = P0 * R0, B1 = P0 * R1, B2 = P1 * R0, B3 = P1 * R1;
     const double AB0 = A * B0, AB1 = A * B1, AB2 = A * B2, AB3 = A * B3;
+    const double qq = exp(tb * nd * fc), q2 = qq * qq, Q = q2 * q2;
     // F(D) = +-[ prod (A B_i D + 1) - Q prod (B_i D + 1) ] S, signed so that it increases with D and scaled by S = 1 / (Q prod(B_i D0 + 1))
     // so that it is O(1) around the root.  With no transverse tilt (B_i = 1) the root is D0 = (q - 1) / (A - q), q = Q^(1/4): the
     // starting point.  Bracket it by factors of 4, then the Illinois variant of regula falsi (superlinear, bracket kept): no
@@ -104,7 +107,6 @@ __device__ __forceinline__ void vof_reconstruct(const GridParams &g, const doubl
         const double den = fma(B0, D, 1.0) * fma(B1, D, 1.0) * (fma(B2, D, 1.0) * fma(B3, D, 1.0));
         return scale * fma(-Q, den, num);
     };
-    const double qq = exp(tb * nd * fc);
     double a = (qq - 1.0) / (A - qq), b = a;
     scale = (nd > 0.0 ? 1.0 : -1.0) / (Q * (fma(B0, a, 1.0) * fma(B1, a, 1.0) * (fma(B2, a, 1.0) * fma(B3, a, 1.0))));
     double fa = F(a), fb = fa;
@@ -125,35 +127,90 @@ __device__ __forceinline__ void vof_reconstruct(const GridParams &g, const doubl
         if (fcv > 0.0) { b = c; fb = fcv; if (side == -1) fa *= 0.5; side = -1; }
         else { a = c; fa = fcv; if (side == 1) fb *= 0.5; side = 1; }
     }
-    r.d = log(root) / tb;
+    r.D = root;
 }
 
+// mean of H^ over x~_DIR in [a, b] x the unit square across DIR, times (b - a) -- i.e. the volume of fluid in that slice
 template <int DIR>
-__global__ void __launch_bounds__(256)
+__device__ __forceinline__ double vof_slice(const VofRecon &r, double a, double b, double beta) {
+    constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
+    const double alpha = r.n[DIR], tb = 2.0 * beta;
+    // e^{2 beta gamma_i} at the four Gauss points across DIR
+    const double G0 = r.E[T1][0] * r.E[T2][0] * r.D, G1 = r.E[T1][0] * r.E[T2][1] * r.D;
+    const double G2 = r.E[T1][1] * r.E[T2][0] * r.D, G3 = r.E[T1][1] * r.E[T2][1] * r.D;
+    if (fabs(alpha) < 1e-12)      // 1/2 (1 + tanh z) = e^{2z} / (1 + e^{2z})
+        return (b - a) * 0.25 * (G0 / (1.0 + G0) + G1 / (1.0 + G1) + G2 / (1.0 + G2) + G3 / (1.0 + G3));
+    const double Ea = a == 0.0 ? 1.0 : exp(tb * alpha * a);
+    const double Eb = b == 1.0 ? r.E[DIR][0] * r.E[DIR][1] : exp(tb * alpha * b);
+    const double num = fma(Eb, G0, 1.0) * fma(Eb, G1, 1.0) * (fma(Eb, G2, 1.0) * fma(Eb, G3, 1.0));
+    const double den = fma(Ea, G0, 1.0) * fma(Ea, G1, 1.0) * (fma(Ea, G2, 1.0) * fma(Ea, G3, 1.0));
+    return log(num / den) / (4.0 * tb * alpha);
+}
+
+// A block owns VofTile::CELLS consecutive cells.  Pass 1: every cell finds out which of its faces it is the donor of (its +
+// face when the velocity there is >= 0, its - face when the velocity there is < 0: every face is written exactly once) and
+// either writes the flux of a constant state at once or -- phi in (eps, 1 - eps) -- joins the block's work list.  Pass 2:
+// the list is worked off with every lane busy (the cells that carry a reconstruction are a band around the interfaces:
+// one cell in a warp of consecutive cells here, ten there).
+struct VofTile { static constexpr int NT = 256, PER = 4, CELLS = NT * PER; };
+
+template <int DIR>
+__global__ void __launch_bounds__(VofTile::NT)
 vof_flux_kernel(GridParams g, double beta, double dt, const double *__restrict__ phi, const double *__restrict__ vel,
                 double *__restrict__ flux) {
-    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long npts = (long long)g.nx * g.ny * g.nz;
-    if (q >= npts) return;
-    const int i = (int)(q % g.nx), j = (int)((q / g.nx) % g.ny), k = (int)(q / ((long long)g.nx * g.ny));
+    using T = VofTile;
+    __shared__ int list[T::CELLS];
+    __shared__ int n_list;
+    const long long npts = (long long)g.nx * g.ny * g.nz, base = (long long)blockIdx.x * T::CELLS;
     const long long sy = g.nx, sz = (long long)g.nx * g.ny;
-    const long long qm = DIR == 0 ? (i == 0 ? q + (g.nx - 1) : q - 1)
-                       : DIR == 1 ? (j == 0 ? q + (g.ny - 1) * sy : q - sy) : (k == 0 ? q + (g.nz - 1) * sz : q - sz);
     const double dl = 1.0 / (DIR == 0 ? g.inv_dx : (DIR == 1 ? g.inv_dy : g.inv_dz));
-    const double cp = vel[q] * dt / dl, cm = vel[qm] * dt / dl;             // local CFL numbers on the + and - face (A.26)
-    const bool give_p = cp >= 0.0, give_m = cm < 0.0;
-    if (!give_p && !give_m) return;
-    VofRecon r;
-    vof_reconstruct(g, phi, i, j, k, beta, r);
-    const double fc = phi[q];
-    const double nd = r.n[DIR], n1 = r.n[(DIR + 1) % 3], n2 = r.n[(DIR + 2) % 3];
-    if (give_p) {                                                            // the last cp of the way through this cell
-        const double a = 1.0 - cp, b = 1.0;
-        flux[q] = dl * (r.flat ? (b - a) * fc : hat_integral_dev(nd, n1, n2, r.d, a, b, beta));
+    const double dt_dl = dt / dl;
+    auto minus_of = [&](long long q, int i, int j, int k) {
+        return DIR == 0 ? (i == 0 ? q + (g.nx - 1) : q - 1) : DIR == 1 ? (j == 0 ? q + (g.ny - 1) * sy : q - sy) : (k == 0 ? q + (g.nz - 1) * sz : q - sz);
+    };
+    if (threadIdx.x == 0) n_list = 0;
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c < T::PER; ++c) {
+        const int loc = c * T::NT + threadIdx.x;
+        const long long q = base + loc;
+        bool queued = false;
+        if (q < npts) {
+            const int i = (int)(q % g.nx), j = (int)((q / g.nx) % g.ny), k = (int)(q / sz);
+            const long long qm = minus_of(q, i, j, k);
+            const double cp = vel[q] * dt_dl, cm = vel[qm] * dt_dl;              // local CFL numbers on the + and - face (A.26)
+            const bool give_p = cp >= 0.0, give_m = cm < 0.0;
+            if (give_p || give_m) {
+                const double fc = phi[q];
+                if (fc > kVofEps && fc < 1.0 - kVofEps) queued = true;
+                else {
+                    if (give_p) flux[q] = dl * (cp * fc);
+                    if (give_m) flux[qm] = -dl * (-cm * fc);
+                }
+            }
+        }
+        // warp-aggregated append
+        const unsigned m = __ballot_sync(0xffffffffu, queued);
+        int pos = 0;
+        if ((threadIdx.x & 31) == 0 && m) pos = atomicAdd(&n_list, __popc(m));
+        pos = __shfl_sync(0xffffffffu, pos, 0);
+        if (queued) list[pos + __popc(m & ((1u << (threadIdx.x & 31)) - 1u))] = loc;
     }
-    if (give_m) {                                                            // the first |cm| of it, leaving backwards
-        const double a = 0.0, b = -cm;
-        flux[qm] = -dl * (r.flat ? (b - a) * fc : hat_integral_dev(nd, n1, n2, r.d, a, b, beta));
+    __syncthreads();
+    const int n = n_list;
+    for (int it = threadIdx.x; it < n; it += T::NT) {
+        const long long q = base + list[it];
+        const int i = (int)(q % g.nx), j = (int)((q / g.nx) % g.ny), k = (int)(q / sz);
+        const long long qm = minus_of(q, i, j, k);
+        const double cp = vel[q] * dt_dl, cm = vel[qm] * dt_dl;
+        const bool give_p = cp >= 0.0, give_m = cm < 0.0;
+        const double fc = phi[q];
+        VofRecon r;
+        vof_reconstruct(g, phi, i, j, k, fc, beta, r);
+        if (give_p)                                                              // the last cp of the way through this cell
+            flux[q] = dl * (r.flat ? cp * fc : vof_slice<DIR>(r, 1.0 - cp, 1.0, beta));
+        if (give_m)                                                              // the first |cm| of it, leaving backwards
+            flux[qm] = -dl * (r.flat ? -cm * fc : vof_slice<DIR>(r, 0.0, -cm, beta));
     }
 }
 
