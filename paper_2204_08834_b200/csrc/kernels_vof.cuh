@@ -13,8 +13,9 @@
 //   d  from the volume constraint A.8 / A.10 in the paper's polynomial form (A.14-A.16): with D = e^{2 beta d},
 //       A = e^{2 beta n_dir}, B_i = e^{2 beta a_i} (a_i = the transverse part of n . x~ at the four Gauss points) and
 //       Q = e^{8 beta n_dir phi}:   prod_i (A B_i D + 1) = Q prod_i (B_i D + 1),  a quartic in D with exactly one positive
-//       root, found by a bracketed regula falsi started from the root of the untilted case (robust for every phi in
-//       (eps, 1 - eps), no transcendental function inside the iteration; the closed-form route A.17-A.21 is not used);
+//       root, found by a bracketed Newton iteration on the polynomial, started from the root of the untilted case (robust
+//       for every phi in (eps, 1 - eps), no transcendental function inside the iteration; the closed-form route A.17-A.21
+//       is not used);
 //   fluxes: exact integration of tanh along the sweep direction, 2 x 2 Gauss points across it (A.23-A.31).
 //
 // vof_flux_kernel<DIR>: a cell writes the flux of the faces it is the donor of (its + face when the velocity there is >= 0,
@@ -97,36 +98,40 @@ __device__ __forceinline__ void vof_reconstruct(const GridParams &g, const doubl
     const double B0 = P0 * R0, B1 = P0 * R1, B2 = P1 * R0, B3 = P1 * R1;
     const double AB0 = A * B0, AB1 = A * B1, AB2 = A * B2, AB3 = A * B3;
     const double qq = exp(tb * nd * fc), q2 = qq * qq, Q = q2 * q2;
-    // F(D) = +-[ prod (A B_i D + 1) - Q prod (B_i D + 1) ] S, signed so that it increases with D and scaled by S = 1 / (Q prod(B_i D0 + 1))
-    // so that it is O(1) around the root.  With no transverse tilt (B_i = 1) the root is D0 = (q - 1) / (A - q), q = Q^(1/4): the
-    // starting point.  Bracket it by factors of 4, then the Illinois variant of regula falsi (superlinear, bracket kept): no
-    // transcendental function and no division inside the loop.
-    double scale = 1.0;
-    auto F = [&](double D) {
-        const double num = fma(AB0, D, 1.0) * fma(AB1, D, 1.0) * (fma(AB2, D, 1.0) * fma(AB3, D, 1.0));
-        const double den = fma(B0, D, 1.0) * fma(B1, D, 1.0) * (fma(B2, D, 1.0) * fma(B3, D, 1.0));
-        return scale * fma(-Q, den, num);
-    };
-    double a = (qq - 1.0) / (A - qq), b = a;
-    scale = (nd > 0.0 ? 1.0 : -1.0) / (Q * (fma(B0, a, 1.0) * fma(B1, a, 1.0) * (fma(B2, a, 1.0) * fma(B3, a, 1.0))));
-    double fa = F(a), fb = fa;
-    for (int it = 0; it < 400 && fa > 0.0; ++it) { b = a; fb = fa; a *= 0.25; fa = F(a); }
-    for (int it = 0; it < 400 && fb < 0.0; ++it) { a = b; fa = fb; b *= 4.0; fb = F(b); }
-    int side = 0;
-    double root = 0.5 * (a + b), prev = -1.0;
-    for (int it = 0; it < 100; ++it) {
-        if (fa == 0.0) { root = a; break; }
-        if (fb == 0.0) { root = b; break; }
-        double c = (fa * b - fb * a) / (fa - fb);
-        if (!(c > a && c < b)) c = 0.5 * (a + b);
-        root = c;
-        if (fabs(c - prev) <= 1.0e-15 * c) break;        // the iterates have converged (the bracket need not shrink on both sides)
-        prev = c;
-        const double fcv = F(c);
-        if (fcv == 0.0) break;
-        if (fcv > 0.0) { b = c; fb = fcv; if (side == -1) fa *= 0.5; side = -1; }
-        else { a = c; fa = fcv; if (side == 1) fb *= 0.5; side = 1; }
+    // F(D) = sgn [ prod (A B_i D + 1) - Q prod (B_i D + 1) ], sgn = sign(n_dir): increasing in D, F(0) < 0 < F(inf), exactly one
+    // positive root (ln of the ratio of the two products rises monotonically from 0 to 4 ln A).  Newton's iteration on the
+    // polynomial and its derivative (product rule, no division), kept inside a bracket (a step that would leave it is replaced
+    // by a bisection).  With no transverse tilt (B_i = 1) the root is c = (q - 1) / (A - q), q = Q^(1/4).  One reciprocal
+    // (hardware seed + two Newton steps on it) and about 35 multiply-adds per iteration, 4-6 iterations on average, no
+    // transcendental function.
+    // The root is bracketed rigorously: every factor (A B_i D + 1) / (B_i D + 1) is monotone in B_i D, so with all B_i replaced
+    // by the largest (smallest) one the root is c / B_max (c / B_min); the geometric mean of the B_i gives the starting point.
+    const double sgn = nd > 0.0 ? 1.0 : -1.0;
+    const double c0 = (qq - 1.0) / (A - qq);
+    const double bmin = fmin(fmin(B0, B1), fmin(B2, B3)), bmax = fmax(fmax(B0, B1), fmax(B2, B3));
+    double lo = c0 / bmax * (1.0 - 1.0e-15), hi = c0 / bmin * (1.0 + 1.0e-15), x = c0 / sqrt(B0 * B3), prev_step = 1.0e300;
+    for (int it = 0; it < 64; ++it) {
+        const double f0 = fma(AB0, x, 1.0), f1 = fma(AB1, x, 1.0), f2 = fma(AB2, x, 1.0), f3 = fma(AB3, x, 1.0);
+        const double g0 = fma(B0, x, 1.0), g1 = fma(B1, x, 1.0), g2 = fma(B2, x, 1.0), g3 = fma(B3, x, 1.0);
+        const double n01 = f0 * f1, n23 = f2 * f3, m01 = g0 * g1, m23 = g2 * g3;
+        const double Fv = sgn * fma(-Q, m01 * m23, n01 * n23);
+        const double dN = fma(fma(AB0, f1, AB1 * f0), n23, n01 * fma(AB2, f3, AB3 * f2));
+        const double dM = fma(fma(B0, g1, B1 * g0), m23, m01 * fma(B2, g3, B3 * g2));
+        const double dF = sgn * fma(-Q, dM, dN);
+        if (Fv == 0.0) break;
+        if (Fv < 0.0) lo = x; else hi = x;
+        double xn = dF > 0.0 ? fma(-Fv, rcp_density(dF), x) : -1.0;
+        if (dF > 0.0 && fabs(xn - x) <= 4.0e-16 * x) { x = xn; break; }          // the step is below the resolution of x
+        const bool fallback = !(xn > lo) || !(xn < hi);                          // left the bracket (or no usable derivative)
+        if (fallback) xn = Fv < 0.0 ? 0.5 * (x + hi) : 0.5 * (lo + x);
+        const double step = fabs(xn - x);
+        x = xn;
+        if (step <= 4.0e-16 * x) break;
+        // Newton's steps shrink faster than geometrically until they reach round-off level: the first one that does not is noise
+        if (!fallback && step <= 1.0e-3 * x && step >= 0.5 * prev_step) break;
+        prev_step = fallback ? 1.0e300 : step;
     }
+    const double root = x;
     r.D = root;
 }
 
