@@ -24,6 +24,7 @@
 // vof_update_kernel<DIR>: eq. (11).  vof_final_kernel: eq. (12).
 #pragma once
 #include "kernels.cuh"
+#include "kernels_tma.cuh"   // rcp_normal
 
 namespace flutas {
 
@@ -90,14 +91,23 @@ __device__ __forceinline__ void vof_reconstruct(const GridParams &g, const doubl
     }
     const double ax = fabs(r.n[0]), ay = fabs(r.n[1]), az = fabs(r.n[2]);
     const int dir = (ax >= ay && ax >= az) ? 0 : ((ay >= az) ? 1 : 2);     // direction of exact integration (cases 1-3)
-    const double nd = dir == 0 ? r.n[0] : (dir == 1 ? r.n[1] : r.n[2]);
-    const double A = dir == 0 ? r.E[0][0] * r.E[0][1] : (dir == 1 ? r.E[1][0] * r.E[1][1] : r.E[2][0] * r.E[2][1]);   // e^{2 beta n_dir}
-    const double P0 = dir == 0 ? r.E[1][0] : (dir == 1 ? r.E[2][0] : r.E[0][0]), P1 = dir == 0 ? r.E[1][1] : (dir == 1 ? r.E[2][1] : r.E[0][1]);
-    const double R0 = dir == 0 ? r.E[2][0] : (dir == 1 ? r.E[0][0] : r.E[1][0]), R1 = dir == 0 ? r.E[2][1] : (dir == 1 ? r.E[0][1] : r.E[1][1]);
+    double nd = dir == 0 ? r.n[0] : (dir == 1 ? r.n[1] : r.n[2]);
+    double A = dir == 0 ? r.E[0][0] * r.E[0][1] : (dir == 1 ? r.E[1][0] * r.E[1][1] : r.E[2][0] * r.E[2][1]);   // e^{2 beta n_dir}
+    double P0 = dir == 0 ? r.E[1][0] : (dir == 1 ? r.E[2][0] : r.E[0][0]), P1 = dir == 0 ? r.E[1][1] : (dir == 1 ? r.E[2][1] : r.E[0][1]);
+    double R0 = dir == 0 ? r.E[2][0] : (dir == 1 ? r.E[0][0] : r.E[1][0]), R1 = dir == 0 ? r.E[2][1] : (dir == 1 ? r.E[0][1] : r.E[1][1]);
+    double qq = exp(tb * nd * fc);
+    // Cells more than half full are solved as their mirror image (n -> -n, phi -> 1 - phi, D -> 1 / D: the same polynomial with
+    // every coefficient replaced by its reciprocal and Q by Q / A^4): the iteration below converges in 4-5 steps from the
+    // dilute side and needs about twice as many from the other.
+    const bool mirror = fc > 0.5;
+    if (mirror) {
+        A = rcp_normal(A); P0 = rcp_normal(P0); P1 = rcp_normal(P1); R0 = rcp_normal(R0); R1 = rcp_normal(R1);
+        qq *= A; nd = -nd;
+    }
     // prod_i (A B_i D + 1) = Q prod_i (B_i D + 1)   (A.14-A.16 with Q here = A^2 Q_paper), B_i = e^{2 beta a_i}
     const double B0 = P0 * R0, B1 = P0 * R1, B2 = P1 * R0, B3 = P1 * R1;
     const double AB0 = A * B0, AB1 = A * B1, AB2 = A * B2, AB3 = A * B3;
-    const double qq = exp(tb * nd * fc), q2 = qq * qq, Q = q2 * q2;
+    const double q2 = qq * qq, Q = q2 * q2;
     // F(D) = sgn [ prod (A B_i D + 1) - Q prod (B_i D + 1) ], sgn = sign(n_dir): increasing in D, F(0) < 0 < F(inf), exactly one
     // positive root (ln of the ratio of the two products rises monotonically from 0 to 4 ln A).  Newton's iteration on the
     // polynomial and its derivative (product rule, no division), kept inside a bracket (a step that would leave it is replaced
@@ -107,9 +117,10 @@ __device__ __forceinline__ void vof_reconstruct(const GridParams &g, const doubl
     // The root is bracketed rigorously: every factor (A B_i D + 1) / (B_i D + 1) is monotone in B_i D, so with all B_i replaced
     // by the largest (smallest) one the root is c / B_max (c / B_min); the geometric mean of the B_i gives the starting point.
     const double sgn = nd > 0.0 ? 1.0 : -1.0;
-    const double c0 = (qq - 1.0) / (A - qq);
+    // (reciprocals by rcp_normal: <= ~1 ulp, the bracket is widened by far more than that)
+    const double c0 = (qq - 1.0) * rcp_normal(A - qq);
     const double bmin = fmin(fmin(B0, B1), fmin(B2, B3)), bmax = fmax(fmax(B0, B1), fmax(B2, B3));
-    double lo = c0 / bmax * (1.0 - 1.0e-15), hi = c0 / bmin * (1.0 + 1.0e-15), x = c0 / sqrt(B0 * B3), prev_step = 1.0e300;
+    double lo = c0 * rcp_normal(bmax) * (1.0 - 1.0e-14), hi = c0 * rcp_normal(bmin) * (1.0 + 1.0e-14), x = c0 * rsqrt(B0 * B3), prev_step = 1.0e300;
     for (int it = 0; it < 64; ++it) {
         const double f0 = fma(AB0, x, 1.0), f1 = fma(AB1, x, 1.0), f2 = fma(AB2, x, 1.0), f3 = fma(AB3, x, 1.0);
         const double g0 = fma(B0, x, 1.0), g1 = fma(B1, x, 1.0), g2 = fma(B2, x, 1.0), g3 = fma(B3, x, 1.0);
@@ -118,9 +129,9 @@ __device__ __forceinline__ void vof_reconstruct(const GridParams &g, const doubl
         const double dN = fma(fma(AB0, f1, AB1 * f0), n23, n01 * fma(AB2, f3, AB3 * f2));
         const double dM = fma(fma(B0, g1, B1 * g0), m23, m01 * fma(B2, g3, B3 * g2));
         const double dF = sgn * fma(-Q, dM, dN);
-        if (Fv == 0.0) break;
+        if (fabs(Fv) <= 2.0e-15 * (n01 * n23)) break;        // the two products agree to round-off: nothing left to gain
         if (Fv < 0.0) lo = x; else hi = x;
-        double xn = dF > 0.0 ? fma(-Fv, rcp_density(dF), x) : -1.0;
+        double xn = dF > 0.0 ? fma(-Fv, rcp_normal(dF), x) : -1.0;
         if (dF > 0.0 && fabs(xn - x) <= 4.0e-16 * x) { x = xn; break; }          // the step is below the resolution of x
         const bool fallback = !(xn > lo) || !(xn < hi);                          // left the bracket (or no usable derivative)
         if (fallback) xn = Fv < 0.0 ? 0.5 * (x + hi) : 0.5 * (lo + x);
@@ -131,7 +142,7 @@ __device__ __forceinline__ void vof_reconstruct(const GridParams &g, const doubl
         if (!fallback && step <= 1.0e-3 * x && step >= 0.5 * prev_step) break;
         prev_step = fallback ? 1.0e300 : step;
     }
-    const double root = x;
+    const double root = mirror ? rcp_normal(x) : x;
     r.D = root;
 }
 
@@ -144,12 +155,12 @@ __device__ __forceinline__ double vof_slice(const VofRecon &r, double a, double 
     const double G0 = r.E[T1][0] * r.E[T2][0] * r.D, G1 = r.E[T1][0] * r.E[T2][1] * r.D;
     const double G2 = r.E[T1][1] * r.E[T2][0] * r.D, G3 = r.E[T1][1] * r.E[T2][1] * r.D;
     if (fabs(alpha) < 1e-12)      // 1/2 (1 + tanh z) = e^{2z} / (1 + e^{2z})
-        return (b - a) * 0.25 * (G0 / (1.0 + G0) + G1 / (1.0 + G1) + G2 / (1.0 + G2) + G3 / (1.0 + G3));
+        return (b - a) * 0.25 * (G0 * rcp_normal(1.0 + G0) + G1 * rcp_normal(1.0 + G1) + G2 * rcp_normal(1.0 + G2) + G3 * rcp_normal(1.0 + G3));
     const double Ea = a == 0.0 ? 1.0 : exp(tb * alpha * a);
     const double Eb = b == 1.0 ? r.E[DIR][0] * r.E[DIR][1] : exp(tb * alpha * b);
     const double num = fma(Eb, G0, 1.0) * fma(Eb, G1, 1.0) * (fma(Eb, G2, 1.0) * fma(Eb, G3, 1.0));
     const double den = fma(Ea, G0, 1.0) * fma(Ea, G1, 1.0) * (fma(Ea, G2, 1.0) * fma(Ea, G3, 1.0));
-    return log(num / den) / (4.0 * tb * alpha);
+    return log(num * rcp_normal(den)) * rcp_normal(4.0 * tb * alpha);
 }
 
 // A block owns VofTile::CELLS consecutive cells.  Pass 1: every cell finds out which of its faces it is the donor of (its +
