@@ -429,12 +429,13 @@ def bench_slab_distributed(name, args, rank, local_rank, world):
 def vof_result(name, W, args, world, units_ms, clocks, peak_gbs, peak_label, gen_s, finite, drift, plan, band, sm_count):
     """the JSON block of the volume-of-fluid workload.  Seven launches per step (3 x flux + update, the correction).  The
     flux kernels are bound by FP64 arithmetic in the cells that carry a reconstruction: algorithmic work
-    = 1100 fp64 operations per such cell and sweep (27-point Youngs gradient 230, 15 exponentials and 5 logarithms 425, the
-    root of the quartic 270, divisions and the flux arithmetic 175); peak = SMs x 64 fp64 lanes x the SM clock."""
+    = 775 fp64 instructions per such cell and sweep with the algorithm as built (27-point Youngs gradient 230; 8 exponentials
+    224 and 1 logarithm 40; 3 divisions, a square root and a reciprocal square root 56; fast reciprocals 32; coefficients of
+    the quartic 25; 3.5 Newton iterations of 40; the flux 28); peak = SMs x 64 fp64 lanes x the SM clock."""
     units, ms = units_ms
     step_ms = ms / args.steps
     model_bytes = 28 * 8.0 * W.npts
-    ops = 1100.0 * 3 * band * W.npts
+    ops = 775.0 * 3 * band * W.npts
     sm_ghz = (clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0) / 1e3
     peak_ops = sm_count * 64 * sm_ghz            # G fp64 operations (instructions x lanes) per second
     plan.destroy()

@@ -171,7 +171,7 @@ __device__ __forceinline__ double vof_slice(const VofRecon &r, double a, double 
 struct VofTile { static constexpr int NT = 256, PER = 4, CELLS = NT * PER; };
 
 template <int DIR>
-__global__ void __launch_bounds__(VofTile::NT)
+__global__ void __launch_bounds__(VofTile::NT, 4)
 vof_flux_kernel(GridParams g, double beta, double dt, const double *__restrict__ phi, const double *__restrict__ vel,
                 double *__restrict__ flux) {
     using T = VofTile;
