@@ -110,6 +110,7 @@ struct flutas_plan {
     PeerScatter *sc_dev;         // device copy of the store descriptor of the last forward y pass / of the z stage
     ThomasPeerMaps *tpm;         // ROLE_ZLOCAL, wall: tensor maps of the peers' slab spectra (host)
     int sc_nzl, sc_srows, sc_npeers;
+    int mom_ty16;                // momentum kernel: tiles of 32 x 16 cells (one CTA per SM) instead of 32 x 8 (two)
 };
 enum { ROLE_FULL = 0, ROLE_SLAB = 1, ROLE_ZLOCAL = 2 };
 
@@ -605,6 +606,7 @@ extern "C" int flutas_plan_set_option(flutas_plan *pl, const char *name, int val
         return pl->ws_base ? plan_make_maps(pl) : FLUTAS_OK;
     }
     if (!strcmp(name, "thomas_warps") && (value == 1 || value == 2)) { pl->thomas_warps = value; return FLUTAS_OK; }
+    if (!strcmp(name, "mom_ty16") && (value == 0 || value == 1)) { pl->mom_ty16 = value; return FLUTAS_OK; }
     if (!strcmp(name, "chunk") && value >= 0) { pl->chunk = value; return FLUTAS_OK; }
     if (!strcmp(name, "overlap") && (value == 0 || value == 1)) { pl->overlap = value; return FLUTAS_OK; }
     return fail(FLUTAS_ERR_INVALID_ARG, "unknown option or value: %s = %d", name, value);
@@ -1148,9 +1150,19 @@ static int enqueue_momentum(flutas_plan *pl, const double *u, const double *v, c
     g.c_po = dt_ratio;
     MomentumParams mp{prm[0], prm[1], prm[2], prm[3], prm[4], prm[5], 1.0 + 0.5 * dt_ratio, 0.5 * dt_ratio, kappa ? 1 : 0, p ? 1 : 0};
     const int kc = pl->nz < 32 ? pl->nz : 32;
-    const dim3 block(MomTile::TX, MomTile::TY + 1), grid(pl->nx / MomTile::TX, pl->ny / MomTile::TY, (pl->nz + kc - 1) / kc);
-    momentum_rhs_kernel<<<grid, block, 0, st>>>(g, mp, dt, kc, u, v, w, phi, kappa, p, po, m_old[0], m_old[1], m_old[2],
-                                                m_new[0], m_new[1], m_new[2], rhs, us, vs, ws);
+    if (pl->ny % 16 == 0 && pl->mom_ty16) {      // tiles of 32 x 16 cells (one CTA of 736 threads per SM); 32 x 8 when ny is not a multiple of 16
+        using T = MomTile<16>;
+        const dim3 grid(pl->nx / T::TX, pl->ny / T::TY, (pl->nz + kc - 1) / kc);
+        if (set_smem(momentum_rhs_kernel<16>, T::SMEM) != cudaSuccess) return check_launch(cudaGetLastError(), "momentum_rhs attr");
+        momentum_rhs_kernel<16><<<grid, T::NT, T::SMEM, st>>>(g, mp, dt, kc, u, v, w, phi, kappa, p, po, m_old[0], m_old[1], m_old[2],
+                                                              m_new[0], m_new[1], m_new[2], rhs, us, vs, ws);
+    } else {
+        using T = MomTile<8>;
+        const dim3 grid(pl->nx / T::TX, pl->ny / T::TY, (pl->nz + kc - 1) / kc);
+        if (set_smem(momentum_rhs_kernel<8>, T::SMEM) != cudaSuccess) return check_launch(cudaGetLastError(), "momentum_rhs attr");
+        momentum_rhs_kernel<8><<<grid, T::NT, T::SMEM, st>>>(g, mp, dt, kc, u, v, w, phi, kappa, p, po, m_old[0], m_old[1], m_old[2],
+                                                             m_new[0], m_new[1], m_new[2], rhs, us, vs, ws);
+    }
     return check_launch(cudaGetLastError(), "momentum_rhs");
 }
 
@@ -1158,7 +1170,7 @@ static int check_momentum_args(const flutas_plan *pl, double mu1, double mu2, do
                                double dt, double dt_ratio) {
     if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
     if (pl->bc[0] != FLUTAS_BC_PERIODIC || pl->bc[1] != FLUTAS_BC_PERIODIC || pl->bc[2] != FLUTAS_BC_PERIODIC ||
-        pl->nx % MomTile::TX != 0 || pl->ny % MomTile::TY != 0)
+        pl->nx % MomTile<8>::TX != 0 || pl->ny % MomTile<8>::TY != 0)
         return fail(FLUTAS_ERR_UNSUPPORTED_SIZE, "the momentum prediction takes triply periodic plans with nx a multiple of 32");
     if (!(dt > 0.0) || !std::isfinite(dt) || !(dt_ratio > 0.0) || !std::isfinite(dt_ratio))
         return fail(FLUTAS_ERR_INVALID_ARG, "dt and dt_ratio must be positive and finite");
