@@ -245,7 +245,7 @@ int flutas_plan_read_timing(flutas_plan *plan, float *ms_out, int n_out, int *st
 double flutas_plan_kernel_bytes(const flutas_plan *plan, int idx);
 
 /* Kernel variants a plan can switch between (never needed for correctness; every value of every option is held to
- * the same parity tests in tests/test_gpu_variants.py).  FLUTAS_ERR_INVALID_ARG for an unknown name or a value the plan
+ * the same parity tests in tests/test_gpu_variants.py and tests/test_gpu_momentum.py).  FLUTAS_ERR_INVALID_ARG for an unknown name or a value the plan
  * cannot take.
  *   "y16" = 0 | 1                 ny = 1024 only: 1 (default) = 16 x 8 x 8 register-resident kernel, 0 = 4-column path.
  *                                 Switching re-orders the eigenvalue tables (synchronises the device).
@@ -253,6 +253,8 @@ double flutas_plan_kernel_bytes(const flutas_plan *plan, int idx);
  *                                 0 = two sweeps through HBM (allocates its c' array, half a spectrum, on first use;
  *                                 plan-owned, outside the workspace)
  *   "thomas_warps" = 1 | 2        solving warps per CTA of the one-pass kernel (default 2)
+ *   "mom_ty16" = 0 | 1            flutas_time_step / flutas_momentum_rhs: tiles of 32 x 16 cells (1, default; used when ny is a
+ *                                 multiple of 16) or of 32 x 8 cells per CTA
  *   "chunk" = n >= 0              planes per launch group of the step (0, default: every kernel covers the grid)
  *   "overlap" = 0 | 1             chunked only: run the three kernels of a group on three internal streams */
 int flutas_plan_set_option(flutas_plan *plan, const char *name, int value);

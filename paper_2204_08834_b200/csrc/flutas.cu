@@ -419,6 +419,7 @@ static int plan_build(flutas_plan *pl, unsigned flags) {
     pl->y_cols = ny >= 1024 ? 4 : 8;
     pl->z_cols = nz >= 1024 ? 4 : 8;
     pl->rhs_kc = 32;
+    pl->mom_ty16 = 1;
     int dev = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&pl->num_sms, cudaDevAttrMultiProcessorCount, dev));

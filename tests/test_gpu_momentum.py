@@ -96,6 +96,28 @@ def test_time_step_matches_oracle_prediction_then_projection(oracle_mod, maker, 
     plan.destroy()
 
 
+def test_momentum_tile_variants_agree(oracle_mod):
+    """option "mom_ty16": tiles of 32 x 16 cells (default when ny is a multiple of 16) and of 32 x 8 give the same M, u', rhs"""
+    W, kappa, m_old = _case(lambda: wl.random_case(64, 32, 40 - 8, PER, 20.0, 107), 13)
+    (us, vs, ws), m_new = _oracle_prediction(oracle_mod, W, kappa, m_old, 1.0)
+    res = []
+    for ty16 in (1, 0):
+        plan = plan_for(W)
+        plan.set_option("mom_ty16", ty16)
+        d = [to_dev(a) for a in W.fields()]
+        dmn = [torch.empty_like(d[0]) for _ in range(3)]
+        out = [torch.empty_like(d[0]) for _ in range(4)]
+        plan.momentum_rhs(d[0], d[1], d[2], d[3], to_dev(kappa), d[4], d[5], [to_dev(a) for a in m_old], dmn, PHYS["mu1"],
+                          PHYS["mu2"], PHYS["sigma"], PHYS["grav"], W.dt, 1.0, *out)
+        torch.cuda.synchronize()
+        for g, want in zip(dmn, m_new):
+            assert rel_l2(g.cpu().numpy(), want) <= 1e-12, ty16
+        res.append([t.cpu().numpy() for t in dmn + out])
+        plan.destroy()
+    for a, b in zip(*res):
+        assert np.array_equal(a, b)                  # the same arithmetic per face, whatever the tile
+
+
 def test_time_step_argument_errors():
     W = wl.random_case(64, 16, 8, 1, 2.0, 106)                                      # a wall-bounded plan
     plan = plan_for(W)
