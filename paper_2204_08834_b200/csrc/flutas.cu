@@ -14,7 +14,7 @@
 #include <vector>
 
 #include "kernels.cuh"
-#include "kernels_momentum.cuh"
+#include "momentum_launch.h"
 #include "kernels_r2r.cuh"
 #include "kernels_rhs.cuh"
 #include "kernels_thomas.cuh"
@@ -1150,28 +1150,14 @@ static int enqueue_momentum(flutas_plan *pl, const double *u, const double *v, c
     g.c_pn = 1.0 + dt_ratio;
     g.c_po = dt_ratio;
     MomentumParams mp{prm[0], prm[1], prm[2], prm[3], prm[4], prm[5], 1.0 + 0.5 * dt_ratio, 0.5 * dt_ratio, kappa ? 1 : 0, p ? 1 : 0};
-    const int kc = pl->nz < 32 ? pl->nz : 32;
-    if (pl->ny % 16 == 0 && pl->mom_ty16) {      // tiles of 32 x 16 cells (one CTA of 736 threads per SM); 32 x 8 when ny is not a multiple of 16
-        using T = MomTile<16>;
-        const dim3 grid(pl->nx / T::TX, pl->ny / T::TY, (pl->nz + kc - 1) / kc);
-        if (set_smem(momentum_rhs_kernel<16>, T::SMEM) != cudaSuccess) return check_launch(cudaGetLastError(), "momentum_rhs attr");
-        momentum_rhs_kernel<16><<<grid, T::NT, T::SMEM, st>>>(g, mp, dt, kc, u, v, w, phi, kappa, p, po, m_old[0], m_old[1], m_old[2],
-                                                              m_new[0], m_new[1], m_new[2], rhs, us, vs, ws);
-    } else {
-        using T = MomTile<8>;
-        const dim3 grid(pl->nx / T::TX, pl->ny / T::TY, (pl->nz + kc - 1) / kc);
-        if (set_smem(momentum_rhs_kernel<8>, T::SMEM) != cudaSuccess) return check_launch(cudaGetLastError(), "momentum_rhs attr");
-        momentum_rhs_kernel<8><<<grid, T::NT, T::SMEM, st>>>(g, mp, dt, kc, u, v, w, phi, kappa, p, po, m_old[0], m_old[1], m_old[2],
-                                                             m_new[0], m_new[1], m_new[2], rhs, us, vs, ws);
-    }
-    return check_launch(cudaGetLastError(), "momentum_rhs");
+    return check_launch(launch_momentum_rhs(g, mp, dt, pl->mom_ty16 != 0, u, v, w, phi, kappa, p, po, m_old, m_new, rhs, us, vs, ws, st), "momentum_rhs");
 }
 
 static int check_momentum_args(const flutas_plan *pl, double mu1, double mu2, double sigma, double gx, double gy, double gz,
                                double dt, double dt_ratio) {
     if (!pl) return fail(FLUTAS_ERR_INVALID_ARG, "NULL plan");
     if (pl->bc[0] != FLUTAS_BC_PERIODIC || pl->bc[1] != FLUTAS_BC_PERIODIC || pl->bc[2] != FLUTAS_BC_PERIODIC ||
-        pl->nx % MomTile<8>::TX != 0 || pl->ny % MomTile<8>::TY != 0)
+        pl->nx % kMomTileX != 0 || pl->ny % kMomTileYMin != 0)
         return fail(FLUTAS_ERR_UNSUPPORTED_SIZE, "the momentum prediction takes triply periodic plans with nx a multiple of 32");
     if (!(dt > 0.0) || !std::isfinite(dt) || !(dt_ratio > 0.0) || !std::isfinite(dt_ratio))
         return fail(FLUTAS_ERR_INVALID_ARG, "dt and dt_ratio must be positive and finite");

@@ -30,15 +30,10 @@
 //   XZ, YZ, ZZ and w' of the level below are carried from the previous step in the other of two slots.
 // Against the first form (every face evaluated on its own from ~45 global loads): 2.1 x fewer instructions per cell.
 #pragma once
-#include "kernels.cuh"
+#include "common.cuh"
+#include "momentum_launch.h"
 
 namespace flutas {
-
-struct MomentumParams {
-    double mu1, mu2, sigma, gx, gy, gz;
-    double f1, f2;            // Adams-Bashforth: 1 + r/2, r/2
-    int with_kappa, with_p;   // surface tension on / off; splitting terms on (fused with the projection) / off (u' = u**)
-};
 
 template <int TY_> struct MomTile {
     static constexpr int TX = 32, TY = TY_;
