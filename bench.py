@@ -390,12 +390,17 @@ def bench_slab(name, args, local_rank, peak_gbs, peak_label, n_ranks=8):
 
 
 def bench_slab_distributed(name, args, rank, local_rank, world):
-    """--slab under torchrun: ONE box decomposed over the N GPUs (strong scaling), one rank per GPU, exchange buffers in
-    torch symmetric memory, an NCCL all-reduce of one element as the barrier between phases.  NOT exercised in this
-    repository's runs (they have one GPU); the kernels and the index maps are the ones the one-device tests check."""
+    """--slab: ONE box decomposed over the N GPUs (strong scaling), one rank per GPU, exchange buffers in torch symmetric
+    memory, an NCCL all-reduce of one element as the barrier between phases.  Exercised in this repository's runs with
+    N = 1 only (they have one GPU); the kernels and the index maps are the ones the one-device tests check."""
     import torch
+    import torch.distributed as dist
     import workloads as wl
     from paper_2204_08834_b200 import replicas, slab
+    if not dist.is_initialized():          # a single process: a group of one rank (the symmetric-memory path needs a group)
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29511")
+        dist.init_process_group("nccl", rank=0, world_size=1)
     W = make_workload(name)
     periodic = W.bc_z == 0
     sr = slab.SlabRank(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2)
@@ -554,7 +559,7 @@ def run_ours(args):
     names = [w for w in args.workloads.split(",") if w]
     if world > 1:       # all-ranks-on-one-device workloads are a one-GPU measurement
         names = [n for n in names if "slab" not in n]
-    if args.slab and world > 1:
+    if args.slab:
         out = bench_slab_distributed(names[0], args, rank, local_rank, world)
         if rank == 0:
             print(json.dumps(out), flush=True)
@@ -613,8 +618,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--no-compare-torch", action="store_true", help="skip the torch/cuFFT statement of the periodic step (comparison only)")
     ap.add_argument("--opt", action="append", help="plan tuning knob name=value (experiments)")
-    ap.add_argument("--slab", action="store_true", help="N > 1 only: decompose ONE box over the N GPUs (z slabs, SURVEY sec. 8(f) "
-                                                        "NEXT-3) instead of running N replicas")
+    ap.add_argument("--slab", action="store_true", help="decompose ONE box over the N GPUs (z slabs, SURVEY sec. 8(f) NEXT-3) instead "
+                                                        "of running N replicas")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

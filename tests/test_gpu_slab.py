@@ -100,3 +100,54 @@ def test_slab_rejects_bad_decompositions():
         assert binding.lib.flutas_slab_workspace_bytes(*args) == 0, args
         with pytest.raises(binding.FlutasError):
             binding.SlabPlan(args[0], args[1], args[2], 1.0, 1.0, 1.0, args[3], 1.0, 2.0, args[4], 0)
+
+
+def _slab_rank_worker(port, q):
+    """one NCCL rank: SlabRank (exchange buffer from torch symmetric memory, all-reduce as the barrier) against flutas_projection_step"""
+    import os
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import paper_2204_08834_b200 as fl
+    import workloads as wl
+    from paper_2204_08834_b200 import slab
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", rank=0, world_size=1)
+    try:
+        W = wl.random_case(128, 16, 32, PER, 10.0, seed=9)
+        plan = fl.Plan(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2)
+        d = [torch.from_numpy(a).cuda() for a in W.fields()]
+        plan.projection_step(*d, W.dt)
+        try:
+            sr = slab.SlabRank(W.nx, W.ny, W.nz, *W.box, W.bc_z, W.rho1, W.rho2)
+        except Exception as e:                                   # symmetric memory not available in this build / on this box
+            q.put(("skip", repr(e)))
+            return
+        loc = [torch.from_numpy(wl.slab_split(a, 1, True)[0]).cuda() for a in W.fields()]
+        sr.step(*loc, W.dt)
+        torch.cuda.synchronize()
+        errs = [float((loc[f][1:-1].reshape(-1) - d[f].reshape(-1)).norm() / d[f].norm()) for f in (0, 1, 2, 4)]
+        q.put(("ok", errs))
+        sr.destroy()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_slab_rank_over_symmetric_memory_one_rank():
+    """the torchrun path of slab.py (SlabRank) with a process group of ONE rank: exercises the symmetric-memory allocation,
+    the rendezvous, the pointer table and the all-reduce barrier; more ranks need more GPUs than this run has"""
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    p = ctx.Process(target=_slab_rank_worker, args=(port, q))
+    p.start()
+    status, payload = q.get(timeout=240)
+    p.join(timeout=60)
+    if status == "skip":
+        pytest.skip("torch symmetric memory unavailable: " + payload)
+    assert max(payload) <= 1e-12, payload
