@@ -38,7 +38,9 @@ def _slab_step(W, n_ranks, p_out_mode="p"):
     ((128, 16, 32), PER, 10.0, 1), ((128, 16, 32), PER, 10.0, 2), ((128, 16, 32), PER, 10.0, 4),
     ((128, 32, 64), PER, 50.0, 8), ((256, 8, 16), PER, 1.0, 8), ((128, 16, 16), PER, 3.0, 16),
     ((128, 16, 32), WALL, 1000.0, 1), ((128, 16, 32), WALL, 1000.0, 2), ((128, 16, 32), WALL, 1000.0, 4),
-    ((256, 32, 64), WALL, 1.2, 8), ((128, 8, 8), WALL, 5.0, 8), ((128, 64, 256), WALL, 20.0, 2)])
+    ((256, 32, 64), WALL, 1.2, 8), ((128, 8, 8), WALL, 5.0, 8), ((128, 64, 256), WALL, 20.0, 2),
+    # lines of 1024 (four-column tiles of the scatter variants): along y, and along z
+    ((128, 1024, 16), WALL, 7.0, 4), ((128, 8, 1024), PER, 2.0, 4), ((1024, 16, 8), PER, 30.0, 2)])
 def test_slab_step_matches_oracle(oracle_mod, shape, bc, ratio, n_ranks):
     nx, ny, nz = shape
     W = wl.random_case(nx, ny, nz, bc, ratio, seed=nx + ny + nz + n_ranks)
