@@ -55,6 +55,21 @@ def test_size_queries_need_no_device():
     binding.lib.flutas_slab_plan_destroy(None)
 
 
+def test_slab_plan_needs_a_device_and_rejects_bad_arguments():
+    import torch
+    lib = binding.lib
+    for args, code in (((128, 16, 32, 1.0, 1.0, 1.0, 0, 1.0, 2.0, 3, 0), 2),      # ranks not a power of two
+                       ((128, 16, 32, 1.0, 1.0, 1.0, 0, 1.0, 2.0, 4, 4), 1),      # rank outside [0, n_ranks)
+                       ((128, 16, 32, 0.0, 1.0, 1.0, 0, 1.0, 2.0, 4, 0), 1),      # box length
+                       ((64, 16, 32, 1.0, 1.0, 1.0, 0, 1.0, 2.0, 2, 0), 2),       # nx below the bulk-copy-fed kernels' minimum
+                       ((128, 16, 600, 1.0, 1.0, 1.0, 1, 1.0, 2.0, 2, 0), 2)):    # wall nz beyond the one-pass elimination
+        assert not lib.flutas_slab_plan_create(*args)
+        assert lib.flutas_last_error_code() == code, (args, lib.flutas_last_error())
+    if not torch.cuda.is_available():
+        assert not lib.flutas_slab_plan_create(128, 16, 32, 1.0, 1.0, 1.0, 0, 1.0, 2.0, 4, 0)
+        assert lib.flutas_last_error_code() == 4 and b"no CPU fallback" in lib.flutas_last_error()
+
+
 def _free_port():
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
