@@ -51,9 +51,9 @@ WORKLOAD_DESC = {
 
 def make_workload(name, ratio=None):
     import workloads as wl          # top-level module: loads neither the CUDA library nor the oracle
-    if name == "cfg5slab8":
+    if name.startswith("cfg5slab"):
         return wl.config5()
-    if name in ("cfg4", "cfg4ts", "cfg4vof", "cfg4slab8"):
+    if name in ("cfg4", "cfg4ts", "cfg4vof") or name.startswith("cfg4slab"):
         return wl.config4(512, 50.0 if ratio is None else ratio)
     if name == "cfg5":
         return wl.config5()
@@ -143,8 +143,8 @@ def bench_workload(name, args, rank, local_rank, world, peak_gbs, peak_label, wi
     import paper_2204_08834_b200 as fl
     from paper_2204_08834_b200 import replicas
 
-    if "slab" in name:
-        return bench_slab(name, args, local_rank, peak_gbs, peak_label)
+    if "slab" in name:      # cfg4slab8 (default list), cfg4slab2, cfg5slab4, ...: the digits are the number of ranks
+        return bench_slab(name, args, local_rank, peak_gbs, peak_label, n_ranks=int(name.split("slab")[1]))
     ratio = replicas.replica_density_ratio(rank) if (name == "cfg4" and world > 1) else None
     t0 = time.time()
     W = make_workload(name, ratio)
@@ -376,7 +376,8 @@ def bench_slab(name, args, local_rank, peak_gbs, peak_label, n_ranks=8):
     return {"metric": METRIC + " (z-slab decomposition, all ranks on one device)", "value": round(W.npts * args.steps / (ms * 1e-3) / 1e6, 1),
             "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(step_ms, 4),
             "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": WORKLOAD_DESC[name], "grid": [W.nx, W.ny, W.nz], "n_ranks": n_ranks, "planes_per_rank": nzl,
+            "config": {"workload": WORKLOAD_DESC.get(name, WORKLOAD_DESC[name.split("slab")[0] + "slab8"]), "grid": [W.nx, W.ny, W.nz],
+                       "n_ranks": n_ranks, "planes_per_rank": nzl,
                        "ky_rows_per_rank": rpp, "input_generation_s": round(gen_s, 1)},
             "clocks": clocks, "gpu_launches": args.steps * n_ranks * (7 if periodic else 8), "finite": finite,
             "phase_ms_all_ranks": [round(x, 4) for x in phase_ms],
