@@ -11,7 +11,9 @@ batch of synthetic input.  Workloads (BASELINE.json `metric` names both):
   cfg4ts the cfg4 fields through flutas_time_step (momentum prediction fused in; NEXT-5)    [under "also"]
   cfg4vof the cfg4 colour function through flutas_vof_step (one MTHINC step; NEXT-4)        [under "also"]
   cfg4slab8 the cfg4 step on a z-slab decomposition over 8 ranks, all on one device (NEXT-3) [under "also"]
-N > 1 (torchrun): N independent replicas, one per GPU, no data-path collective ("replicas only").
+  cfg4slabN / cfg5slabN: the same on N ranks (experiments)
+N > 1 (torchrun): N independent replicas, one per GPU, no data-path collective ("replicas only"); with --slab instead ONE box
+decomposed over the N GPUs (paper_2204_08834_b200/slab.py; exercised with N = 1 only in this repository's runs).
 Prints ONE JSON line on rank 0.  --impl reference times the CPU oracle (tests' ground truth) on the same workload
 (one or two steps of the full 512^3 box); it is a deliberately slow baseline, not a target.
 """
