@@ -193,6 +193,40 @@ int flutas_momentum_rhs(flutas_plan *plan, const double *u, const double *v, con
 int flutas_vof_step(flutas_plan *plan, const double *phi, const double *u, const double *v, const double *w,
                     double *phi_out, double beta, double dt, void *stream);
 
+/* flutas_vof_step for callers that must not allocate device memory (same method, same kernels: eqs. 8-12;
+ * Appendix A; Algorithm 2).
+ *
+ * For whom: a solver embedded in an application whose own memory pool already owns the whole GPU (any further cudaMalloc
+ * fails there), a routine called from inside a latency-critical pipeline (cudaMalloc synchronises the device, so every
+ * stream of the host application would stall on it), or code bound by a "nothing is allocated after start-up" rule.
+ * Such a caller cannot use flutas_vof_step: that one needs a plan, flutas_plan_create allocates the plan's tables, and
+ * the step works in four fields of the plan's workspace.
+ *
+ * This call takes NO plan and allocates NOTHING, neither on the device nor on the host (no cudaMalloc / cudaFree, no
+ * allocating library routine).  The grid is described by its arguments, and the step's four intermediate fields
+ * (the fluxes of one sweep, phi after each of the three sweeps) are kept in one statically sized array inside the library:
+ * 4 x FLUTAS_VOF_NOALLOC_MAX_CELLS doubles = 64 MiB, which every GPU that loads this part of the library holds until the
+ * process exits.  The price of "no allocation" is therefore a size limit:
+ *   nx * ny * nz <= FLUTAS_VOF_NOALLOC_MAX_CELLS (2^21, e.g. 128^3), else FLUTAS_ERR_UNSUPPORTED_SIZE and nothing is
+ *   launched;  nx, ny, nz >= 3, any value (not only powers of two);  triply periodic;  lx, ly, lz, beta, dt > 0.
+ *   phi, u, v, w, phi_out: caller-owned DEVICE arrays of nx*ny*nz doubles on the current device, layout and alignment as
+ *   for flutas_vof_step; inputs are not modified; phi_out may be phi itself, any other overlap is FLUTAS_ERR_ALIAS.
+ * Enqueues seven kernels on `stream` and returns without synchronising; results agree with flutas_vof_step on the same
+ * grid to round-off.
+ *
+ * First call on a device: the entry point looks up, once per device and with that device current, the address its
+ * static array has on that GPU (cudaGetSymbolAddress; this is also when the driver places the array in that GPU's
+ * memory).  Make that first call during start-up, before any stream capture begins.
+ * Shared scratch: there is ONE array per GPU for the whole process, and it keeps what the last call left in it.  A call
+ * needs none of it cleared (every element it reads it has written itself first), but two calls whose kernels can
+ * overlap on the same GPU -- different streams without an ordering between them, or several host threads -- overwrite
+ * each other's intermediate fields and give wrong results: keep all calls on one GPU ordered one after the other. */
+#define FLUTAS_VOF_NOALLOC_MAX_CELLS 2097152
+int flutas_vof_step_noalloc(int nx, int ny, int nz, double lx, double ly, double lz, const double *phi, const double *u,
+                            const double *v, const double *w, double *phi_out, double beta, double dt, void *stream);
+/* FLUTAS_VOF_NOALLOC_MAX_CELLS as the loaded library was built with (no device needed). */
+size_t flutas_vof_step_noalloc_max_cells(void);
+
 /* NULL is a no-op.  Frees every device and host resource of the plan (synchronises the device). */
 void flutas_plan_destroy(flutas_plan *plan);
 

@@ -5,4 +5,5 @@
 fallback.  The seeded synthetic inputs live in the top-level module `workloads` (they also feed the
 tests' CPU checker, so they are not part of this package).
 """
-from .binding import BC_Z_PERIODIC, BC_Z_WALL, FlutasError, Plan, lib  # noqa: F401
+from .binding import (BC_Z_PERIODIC, BC_Z_WALL, FlutasError, Plan, lib,  # noqa: F401
+                      vof_noalloc_max_cells, vof_step_noalloc)

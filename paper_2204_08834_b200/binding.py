@@ -34,6 +34,10 @@ lib.flutas_momentum_rhs.argtypes = [_vp] * 14 + [_cd] * 8 + [_vp] * 5
 lib.flutas_momentum_rhs.restype = _ci
 lib.flutas_vof_step.argtypes = [_vp] * 6 + [_cd, _cd, _vp]
 lib.flutas_vof_step.restype = _ci
+lib.flutas_vof_step_noalloc.argtypes = [_ci] * 3 + [_cd] * 3 + [_vp] * 5 + [_cd, _cd, _vp]
+lib.flutas_vof_step_noalloc.restype = _ci
+lib.flutas_vof_step_noalloc_max_cells.argtypes = []
+lib.flutas_vof_step_noalloc_max_cells.restype = ctypes.c_size_t
 lib.flutas_plan_destroy.argtypes = [_vp]
 lib.flutas_plan_destroy.restype = None
 lib.flutas_projection_step.argtypes = [_vp] * 7 + [_cd, _vp]
@@ -87,7 +91,8 @@ EXPORTS = [
     "flutas_plan_set_timing", "flutas_plan_read_timing", "flutas_plan_kernel_bytes", "flutas_plan_set_option",
     "flutas_projection_step_ex", "flutas_splitting_rhs_ex",
     "flutas_plan_create_ex", "flutas_workspace_bytes", "flutas_plan_set_workspace", "flutas_plan_kernel_symbol",
-    "flutas_time_step", "flutas_momentum_rhs", "flutas_vof_step",
+    "flutas_time_step", "flutas_momentum_rhs", "flutas_vof_step", "flutas_vof_step_noalloc",
+    "flutas_vof_step_noalloc_max_cells",
     "flutas_slab_plan_create", "flutas_slab_workspace_bytes", "flutas_slab_exchange_bytes", "flutas_slab_plan_attach",
     "flutas_slab_step_phase", "flutas_slab_plan_destroy",
 ]
@@ -124,6 +129,20 @@ def _stream():
 def workspace_bytes(nx, ny, nz, bc_z, bc_x=BC_PERIODIC, bc_y=BC_PERIODIC):
     """flutas_workspace_bytes: what a plan for this grid needs (0 = unsupported grid); no device needed"""
     return lib.flutas_workspace_bytes(int(nx), int(ny), int(nz), int(bc_x), int(bc_y), int(bc_z))
+
+
+def vof_step_noalloc(shape, box, phi, u, v, w, phi_out, beta, dt, stream=None):
+    """flutas_vof_step_noalloc: one MTHINC step without a plan and without any allocation by the library (for callers that
+    may not call cudaMalloc; the scratch is a static array in the library, hence shape = (nx, ny, nz) with
+    nx*ny*nz <= vof_noalloc_max_cells()).  One array per GPU is shared by all calls: keep them ordered on the device."""
+    nx, ny, nz = (int(n) for n in shape)
+    ptrs = [_dev_ptr(t, nx * ny * nz) for t in (phi, u, v, w, phi_out)]
+    _check(lib.flutas_vof_step_noalloc(nx, ny, nz, float(box[0]), float(box[1]), float(box[2]), *ptrs, float(beta), float(dt),
+                                       _stream() if stream is None else stream))
+
+
+def vof_noalloc_max_cells():
+    return lib.flutas_vof_step_noalloc_max_cells()
 
 
 class Plan:

@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libflutas_b200.so")
-SOURCES = [os.path.join(CSRC, "flutas.cu"), os.path.join(CSRC, "momentum.cu")]
+SOURCES = [os.path.join(CSRC, "flutas.cu"), os.path.join(CSRC, "momentum.cu"), os.path.join(CSRC, "vof_noalloc.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, h) for h in sorted(os.listdir(CSRC)) if h.endswith((".cuh", ".inl", ".h"))] + [
     os.path.join(ROOT, "include", "flutas.h")]
 # -split-compile 0: the optimiser and ptxas work on the kernels of the one translation unit in parallel (same code, 3x faster)

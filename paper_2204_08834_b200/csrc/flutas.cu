@@ -20,6 +20,7 @@
 #include "kernels_thomas.cuh"
 #include "kernels_tma.cuh"
 #include "kernels_vof.cuh"
+#include "vof_launch.h"
 #include "kernels_x.cuh"
 #include "kernels_y16.cuh"
 
@@ -44,6 +45,9 @@ static int fail(int code, const char *fmt, ...) {
             return fail(e_ == cudaErrorMemoryAllocation ? FLUTAS_ERR_ALLOC : FLUTAS_ERR_CUDA,  \
                         "%s: %s", #expr, cudaGetErrorString(e_));                              \
     } while (0)
+
+// the library's other translation units (vof_noalloc.cu) record their failures in the same thread-local slot (vof_launch.h)
+int flutas::report_error(int code, const char *msg) { return fail(code, "%s", msg); }
 
 extern "C" const char *flutas_last_error(void) { return g_err; }
 extern "C" int flutas_last_error_code(void) { return g_err_code; }
@@ -1245,6 +1249,23 @@ extern "C" int flutas_vof_step(flutas_plan *pl, const double *phi, const double 
     vof_update_kernel<2><<<nb, 256, 0, st>>>(g, dt, py, w, flux, pz);
     vof_final_kernel<<<nb, 256, 0, st>>>(g, dt, px, py, pz, u, v, w, phi_out);
     return check_launch(cudaGetLastError(), "vof_step");
+}
+
+// The launch sequence of flutas_vof_step on caller-given intermediate fields, for vof_noalloc.cu (vof_launch.h): the VoF
+// kernels read only the sizes and spacings of g.
+cudaError_t flutas::launch_vof_step(const GridParams &g, double beta, double dt, const double *phi, const double *u, const double *v,
+                                    const double *w, double *flux, double *px, double *py, double *pz, double *phi_out,
+                                    cudaStream_t st) {
+    const long long npts = (long long)g.nx * g.ny * g.nz;
+    const unsigned nb = (unsigned)((npts + 255) / 256), nbf = (unsigned)((npts + VofTile::CELLS - 1) / VofTile::CELLS);
+    vof_flux_kernel<0><<<nbf, VofTile::NT, 0, st>>>(g, beta, dt, phi, u, flux);
+    vof_update_kernel<0><<<nb, 256, 0, st>>>(g, dt, phi, u, flux, px);
+    vof_flux_kernel<1><<<nbf, VofTile::NT, 0, st>>>(g, beta, dt, px, v, flux);
+    vof_update_kernel<1><<<nb, 256, 0, st>>>(g, dt, px, v, flux, py);
+    vof_flux_kernel<2><<<nbf, VofTile::NT, 0, st>>>(g, beta, dt, py, w, flux);
+    vof_update_kernel<2><<<nb, 256, 0, st>>>(g, dt, py, w, flux, pz);
+    vof_final_kernel<<<nb, 256, 0, st>>>(g, dt, px, py, pz, u, v, w, phi_out);
+    return cudaGetLastError();
 }
 
 extern "C" int flutas_projection_step(flutas_plan *pl, double *u, double *v, double *w, const double *phi, double *p,
