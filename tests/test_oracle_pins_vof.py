@@ -9,6 +9,13 @@ PAPER.md:104-132, Appendix A).  The paper prints no worked numbers for one step,
       each direction: pins upwinding, signs, the swept interval and which velocity component drives which sweep
   V5  a drop in a uniform diagonal flow: 0 <= phi <= 1, volume conserved, centroid moves by u t (consistency)
   V6  a uniform phi stays uniform in a solenoidal flow; donor-cell fluxes for pure cells
+  V7  the Youngs stencil itself (A.6: "derivatives at the cell corners ... each corner-value is averaged") on a
+      NON-linear field: averaging the eight corner gradients is the 27-point stencil 1/2 (central difference) x 1/4 (1,2,1)
+      x 1/4 (1,2,1), written here with numpy.roll -- a plain central difference (or any other consistent stencil) fails
+  V8  a partial-CFL flux (A.26-A.27): uniform velocity along one axis, CFL +-0.37, one step; then
+      phi' = phi - (F_+ - F_-)/dl with F the integral of the DONOR cell's H^ over [1 - c, 1] (u >= 0) or [0, |c|] (u < 0),
+      evaluated with an independent 64-point Gauss-Legendre rule from the oracle's own (n, d) -- the wrong end of the cell,
+      the wrong donor or the wrong sign fails
 """
 import numpy as np
 import pytest
@@ -135,3 +142,81 @@ def test_v6_uniform_and_pure_states(oracle_mod):
     for val in (0.3, 0.0, 1.0):
         out = oracle_mod.vof_step(np.full(shape, val), u, v, w, box, BETA, dt)
         assert np.abs(out - val).max() < 1e-13
+
+
+def _bumpy_field(shape, seed):
+    """a drop with a smooth random perturbation: curved level sets, 0 < phi < 1, nothing linear about it"""
+    rng = np.random.default_rng(seed)
+    nz, ny, nx = shape
+    z, y, x = np.meshgrid(np.arange(nz) + 0.5, np.arange(ny) + 0.5, np.arange(nx) + 0.5, indexing="ij")
+    bump = sum(a * np.sin(2 * np.pi * (kx * x / nx + ky * y / ny + kz * z / nz) + ph)
+               for a, kx, ky, kz, ph in zip(rng.uniform(0.2, 0.6, 4), rng.integers(1, 3, 4), rng.integers(1, 3, 4),
+                                            rng.integers(1, 3, 4), rng.uniform(0, 6.28, 4)))
+    r = _drop(shape, (nx * 0.45, ny * 0.55, nz * 0.5), 0.3 * min(shape), 1.1)
+    return np.clip(r + 0.08 * bump * r * (1.0 - r) * 4.0, 0.0, 1.0)
+
+
+def _youngs_by_roll(phi):
+    """m = (m_x, m_y, m_z) in cell units: central difference along the component's axis, weights (1, 2, 1) / 4 along the other two"""
+    sm = lambda f, ax: 0.25 * (np.roll(f, 1, axis=ax) + 2.0 * f + np.roll(f, -1, axis=ax))
+    cd = lambda f, ax: 0.5 * (np.roll(f, -1, axis=ax) - np.roll(f, 1, axis=ax))
+    return np.stack([sm(sm(cd(phi, 2), 1), 0), sm(sm(cd(phi, 1), 2), 0), sm(sm(cd(phi, 0), 2), 1)], axis=-1)
+
+
+def test_v7_youngs_stencil_on_a_curved_field(oracle_mod):
+    shape = (10, 12, 14)
+    phi = _bumpy_field(shape, 21)
+    n, d, flat = oracle_mod.vof_reconstruct(phi, BETA)
+    m = _youngs_by_roll(phi)
+    mag = np.linalg.norm(m, axis=-1)
+    band = (phi > 1e-8) & (phi < 1.0 - 1e-8)
+    want_flat = ~band | ~(mag > 1e-12)
+    assert np.array_equal(flat == 1, want_flat) and (~want_flat).sum() > 300
+    want = m[~want_flat] / mag[~want_flat][:, None]
+    assert np.abs(n[~want_flat] - want).max() < 1e-13
+    # the field is curved enough for the stencil to matter: plain central differences give a visibly different normal
+    cd = np.stack([0.5 * (np.roll(phi, -1, axis=a) - np.roll(phi, 1, axis=a)) for a in (2, 1, 0)], axis=-1)[~want_flat]
+    cd /= np.linalg.norm(cd, axis=-1)[:, None]
+    assert np.abs(cd - want).max() > 1e-2
+
+
+def _slice_volume(nn, dd, axis_c, a, b, xs, ws):
+    """int_a^b along component axis_c, 2 x 2 Gauss points across it, of 1/2 [1 + tanh(beta (n . x~ + d))] (cell coordinates)"""
+    g2 = (0.5 - 0.5 / np.sqrt(3.0), 0.5 + 0.5 / np.sqrt(3.0))
+    t1, t2 = (axis_c + 1) % 3, (axis_c + 2) % 3
+    x = a + (b - a) * xs
+    tot = 0.0
+    for p in g2:
+        for q in g2:
+            tot += 0.25 * (b - a) * np.sum(ws * 0.5 * (1.0 + np.tanh(BETA * (nn[axis_c] * x + nn[t1] * p + nn[t2] * q + dd))))
+    return tot
+
+
+@pytest.mark.parametrize("comp", [0, 1, 2])
+@pytest.mark.parametrize("cfl", [0.37, -0.37])
+def test_v8_partial_cfl_flux_integrates_the_donor_cell_over_the_swept_interval(oracle_mod, comp, cfl):
+    shape, box = (8, 9, 10), (1.0, 1.35, 1.6)
+    phi = _bumpy_field(shape, 22 + comp)
+    axis = 2 - comp                                               # numpy axis of the component (x is the last axis)
+    dl = ops.spacings(shape, box)[comp]
+    speed, dt = 0.8, abs(cfl) * dl / 0.8
+    vel = [np.zeros(shape) for _ in range(3)]
+    vel[comp][:] = np.sign(cfl) * speed
+    out = oracle_mod.vof_step(phi, vel[0], vel[1], vel[2], box, BETA, dt)
+    n, d, flat = oracle_mod.vof_reconstruct(phi, BETA)
+    xs, ws = np.polynomial.legendre.leggauss(64)
+    xs, ws = 0.5 * (xs + 1.0), 0.5 * ws
+    c = abs(cfl)
+    a, b = (1.0 - c, 1.0) if cfl > 0 else (0.0, c)                # (A.26): the last c of the donor, or its first |c|
+    vol = np.empty(shape)                                         # what every cell gives away
+    for idx in np.ndindex(*shape):
+        vol[idx] = (b - a) * phi[idx] if flat[idx] else _slice_volume(n[idx], d[idx], comp, a, b, xs, ws)
+    # u > 0: a cell loses its own slice and receives that of the cell before it; u < 0: ... of the cell after it
+    want = phi - vol + np.roll(vol, 1 if cfl > 0 else -1, axis=axis)
+    assert np.abs(out - want).max() < 1e-12
+    assert np.abs(out - phi).max() > 1e-2 and (flat == 0).sum() > 100
+    # the other end of the donor cell is a different number: the pin can tell them apart
+    wrong = np.array([_slice_volume(n[idx], d[idx], comp, 1.0 - b, 1.0 - a, xs, ws) for idx in np.argwhere(flat == 0)[:50].tolist()
+                      for idx in [tuple(idx)]])
+    right = np.array([vol[tuple(idx)] for idx in np.argwhere(flat == 0)[:50]])
+    assert np.abs(wrong - right).max() > 1e-3
