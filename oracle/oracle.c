@@ -216,7 +216,7 @@ int oracle_rhs_bc(int nx, int ny, int nz, double lx, double ly, double lz, int b
     grid_t g;
     if (bc_x == ORACLE_BC_DIRICHLET || bc_y == ORACLE_BC_DIRICHLET || bc_z == ORACLE_BC_DIRICHLET) return 1;
     if (grid_init_bc(&g, nx, ny, nz, lx, ly, lz, bc_x, bc_y, bc_z, rho1, rho2, dt)) return 1;
-    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0) || !(dt_ratio > 0.0)) return 1;
+    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0) || !(dt_ratio >= 0.0)) return 1;
     g.r = dt_ratio;
     set_threads(nthreads);
 #pragma omp parallel for collapse(2) schedule(static)
@@ -586,7 +586,7 @@ int oracle_projection_step_bc(int nx, int ny, int nz, double lx, double ly, doub
     grid_t g;
     if (bc_x == ORACLE_BC_DIRICHLET || bc_y == ORACLE_BC_DIRICHLET || bc_z == ORACLE_BC_DIRICHLET) return 1;
     if (grid_init_bc(&g, nx, ny, nz, lx, ly, lz, bc_x, bc_y, bc_z, rho1, rho2, dt)) return 1;
-    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0) || !(dt_ratio > 0.0)) return 1;
+    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(dt > 0.0) || !(dt_ratio >= 0.0)) return 1;
     g.r = dt_ratio;
     const size_t n = (size_t)nx * ny * nz;
     double *rhs = (double *)malloc(sizeof(double) * n), *p_new = (double *)malloc(sizeof(double) * n);
@@ -693,7 +693,7 @@ int oracle_momentum_prediction(int nx, int ny, int nz, double lx, double ly, dou
                                double *mnew_u, double *mnew_v, double *mnew_w, int nthreads) {
     grid_t g;
     if (grid_init(&g, nx, ny, nz, lx, ly, lz, ORACLE_BC_Z_PERIODIC, rho1, rho2, dt)) return 1;
-    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(mu1 >= 0.0) || !(mu2 >= 0.0) || !(dt > 0.0) || !(dt_ratio > 0.0)) return 1;
+    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(mu1 >= 0.0) || !(mu2 >= 0.0) || !(dt > 0.0) || !(dt_ratio >= 0.0)) return 1;
     const double f1 = 1.0 + 0.5 * dt_ratio, f2 = 0.5 * dt_ratio;
     const double dx = g.dx, dy = g.dy, dz = g.dz;
     set_threads(nthreads);

@@ -68,8 +68,10 @@ int oracle_projection_step(int nx, int ny, int nz, double lx, double ly, double 
                            double *p, const double *p_old, double *rhs_out, int nthreads);
 
 /* The same two calls for a variable time step:
- *   p_hat = (1 + r) p^n - r p^(n-1),  r = dt_ratio = dt^(n+1) / dt^n > 0;  dt = dt^(n+1).
- * dt_ratio = 1 is the constant-dt step above, bit for bit. */
+ *   p_hat = (1 + r) p^n - r p^(n-1),  r = dt_ratio = dt^(n+1) / dt^n >= 0;  dt = dt^(n+1).
+ * dt_ratio = 1 is the constant-dt step above, bit for bit.  dt_ratio = 0 (the same formulas, no special case) is the
+ * start-up step when no level n-1 exists: p_hat = p^n, and in the momentum prediction f1 = 1, f2 = 0, explicit Euler
+ * (PAPER.md:140, 161 give the coefficients as functions of r; the paper does not describe its first step: DESIGN.md R29). */
 int oracle_rhs_vdt(int nx, int ny, int nz, double lx, double ly, double lz, int bc_z,
                    double rho1, double rho2, double dt, double dt_ratio,
                    const double *u, const double *v, const double *w, const double *phi,

@@ -140,3 +140,27 @@ def test_m6_time_update_and_sources(oracle_mod):
     us, _ = _mp(oracle_mod, u, v, w, phi, box, m_old=m_new, rho=rho, mu=mu, grav=grav, dt=dt, r=1.0)
     for d, (a, a0, m) in enumerate(zip(us, (u, v, w), m_new)):
         assert ops.rel_l2(a, a0 + dt * (m + grav[d])) < 1e-13                    # classic AB2: 3/2 - 1/2
+
+
+def test_m7_start_up_step_is_explicit_euler(oracle_mod):
+    """DESIGN.md R29 (PAPER.md:140, 161 with r = 0): f1 = 1, f2 = 0 -- the update is u + dt (M(u) + sources) whatever the
+    history holds, and the projection's extrapolated pressure is p^n itself whatever p^(n-1) holds"""
+    shape, box = (6, 8, 10), (1.3, 0.9, 0.7)
+    (u, v, w), phi = _rand(shape, 8)
+    rng = np.random.default_rng(9)
+    rho, mu, grav, dt = (1.0, 20.0), (0.2, 1.0), (0.3, -0.2, -9.81), 2e-3
+    junk = [1e3 * rng.standard_normal(shape) for _ in range(3)]
+    us, m_new = _mp(oracle_mod, u, v, w, phi, box, m_old=junk, rho=rho, mu=mu, grav=grav, dt=dt, r=0.0)
+    us0, _ = _mp(oracle_mod, u, v, w, phi, box, rho=rho, mu=mu, grav=grav, dt=dt, r=0.0)
+    for d, (a, b, a0, m) in enumerate(zip(us, us0, (u, v, w), m_new)):
+        assert np.array_equal(a, b)
+        assert ops.rel_l2(a, a0 + dt * (m + grav[d])) < 1e-14
+    p, p_old = rng.standard_normal(shape), rng.standard_normal(shape)
+    got = oracle_mod.rhs(u, v, w, phi, p, p_old, box, 0, rho[0], rho[1], dt, dt_ratio=0.0)
+    same = oracle_mod.rhs(u, v, w, phi, p, 7.0 * p_old + 1.0, box, 0, rho[0], rho[1], dt, dt_ratio=0.0)
+    assert np.array_equal(got, same)
+    # with p^(n-1) = p^n every r gives p_hat = p^n: r = 0 must agree with r = 1 up to the rounding of (2 p - p)
+    ref = oracle_mod.rhs(u, v, w, phi, p, p, box, 0, rho[0], rho[1], dt, dt_ratio=1.0)
+    assert ops.rel_l2(got, ref) < 1e-13
+    with pytest.raises(Exception):
+        _mp(oracle_mod, u, v, w, phi, box, r=-0.5)
