@@ -157,8 +157,10 @@ int flutas_projection_step_host(flutas_plan *plan, double *u_host, double *v_hos
  * curvature field; gravity with rho_hat = rho: DESIGN.md R18-R20), then exactly flutas_projection_step_ex on u**.
  * ONE kernel forms u**, the splitting terms and the right-hand side, so u** never travels through HBM.
  *   in : u, v, w = u^n;  phi = phi^(n+1);  kappa = curvature at cell centres, or NULL (no surface tension);
- *        p = p^n, p_old = p^(n-1);  m_old_* = M(u^(n-1)) (zeros and dt_ratio = ... for an Euler start: pass M(u^n) itself,
- *        i.e. call once with any m_old and feed m_new back: f1 - f2 = 1);  mu1, mu2 >= 0, sigma, g: plain numbers.
+ *        p = p^n, p_old = p^(n-1);  m_old_* = M(u^(n-1));  mu1, mu2 >= 0, sigma, g: plain numbers;  dt > 0, dt_ratio >= 0.
+ *        FIRST STEP of a run (no level n-1 yet): pass dt_ratio = 0.  The Adams-Bashforth weights are then 1 and 0 (explicit
+ *        Euler) and p_hat = p^n, so m_old_* and p_old are multiplied by zero: they must be valid arrays of finite numbers
+ *        (e.g. zeros), their values do not matter.  m_new_* = M(u^0) comes back for the second step (R29).
  *   out: u, v, w = u^(n+1) in place;  p_out = p^(n+1) (may be p or p_old, as in flutas_projection_step_ex);
  *        m_new_* = M(u^n) (the caller swaps the two sets for the next step).
  * Triply periodic plans with nx a multiple of 32 only (FLUTAS_ERR_UNSUPPORTED_SIZE otherwise).  All arrays are N doubles on

@@ -1163,8 +1163,9 @@ static int check_momentum_args(const flutas_plan *pl, double mu1, double mu2, do
     if (pl->bc[0] != FLUTAS_BC_PERIODIC || pl->bc[1] != FLUTAS_BC_PERIODIC || pl->bc[2] != FLUTAS_BC_PERIODIC ||
         pl->nx % kMomTileX != 0 || pl->ny % kMomTileYMin != 0)
         return fail(FLUTAS_ERR_UNSUPPORTED_SIZE, "the momentum prediction takes triply periodic plans with nx a multiple of 32");
-    if (!(dt > 0.0) || !std::isfinite(dt) || !(dt_ratio > 0.0) || !std::isfinite(dt_ratio))
-        return fail(FLUTAS_ERR_INVALID_ARG, "dt and dt_ratio must be positive and finite");
+    // dt_ratio = 0: the start-up step (f1 = 1, f2 = 0: explicit Euler; p_hat = p^n), R29
+    if (!(dt > 0.0) || !std::isfinite(dt) || !(dt_ratio >= 0.0) || !std::isfinite(dt_ratio))
+        return fail(FLUTAS_ERR_INVALID_ARG, "dt must be positive, dt_ratio non-negative, both finite");
     if (!(mu1 >= 0.0) || !(mu2 >= 0.0) || !std::isfinite(mu1 + mu2 + sigma + gx + gy + gz))
         return fail(FLUTAS_ERR_INVALID_ARG, "viscosities must be non-negative; sigma and g finite");
     if (!pl->ws_base) return fail(FLUTAS_ERR_INVALID_ARG, "the plan has no workspace (flutas_plan_set_workspace)");

@@ -138,3 +138,35 @@ def test_time_step_argument_errors():
         plan.time_step(d[0], d[1], d[2], d[3], None, d[4], d[5], d[4], m[:3], m[3:], -0.1, 0.1, 0.0, (0, 0, 0), 1e-3)
     assert e.value.code == 1
     plan.destroy()
+
+
+def test_first_step_with_dt_ratio_zero_is_an_euler_step(oracle_mod):
+    """DESIGN.md R29: dt_ratio = 0 is the start-up step (f1 = 1, f2 = 0, p_hat = p^n).  M(u^(n-1)) and p^(n-1) are multiplied
+    by zero: two different (finite) fillings give bit-identical results, equal to the oracle's step with r = 0."""
+    W, kappa, m_old = _case(lambda: wl.random_case(64, 32, 16, PER, 100.0, 108), 17)
+    (us, vs, ws), m_new = _oracle_prediction(oracle_mod, W, kappa, m_old, 0.0)
+    want = oracle_mod.projection_step(us, vs, ws, W.phi, W.p, W.p_old, W.box, PER, W.rho1, W.rho2, W.dt, dt_ratio=0.0)
+    plan = plan_for(W)
+    res = []
+    for fill in (0.0, 1.0e3):
+        d = [to_dev(a) for a in W.fields()]
+        d[5] = torch.full_like(d[5], fill)                                          # p^(n-1): does not exist yet
+        dmo = [torch.full_like(d[0], -fill) for _ in range(3)]                      # M(u^(n-1)): neither
+        dmn = [torch.empty_like(d[0]) for _ in range(3)]
+        p_out = torch.empty_like(d[0])
+        plan.time_step(d[0], d[1], d[2], d[3], to_dev(kappa), d[4], d[5], p_out, dmo, dmn, PHYS["mu1"], PHYS["mu2"], PHYS["sigma"],
+                       PHYS["grav"], W.dt, 0.0)
+        torch.cuda.synchronize()
+        res.append([t.cpu().numpy() for t in (d[0], d[1], d[2], p_out, *dmn)])
+    for a, b in zip(*res):
+        assert np.array_equal(a, b)
+    for n, g, w_ in zip("uvwp", res[0][:4], want):
+        assert rel_l2(g, w_) <= TOL, (n, rel_l2(g, w_))
+    for g, w_ in zip(res[0][4:], m_new):
+        assert rel_l2(g, w_) <= 1e-12
+    with pytest.raises(fl.FlutasError) as e:
+        plan.time_step(*[to_dev(a) for a in W.fields()[:4]], None, *[to_dev(a) for a in (W.p, W.p_old, W.p)],
+                       [to_dev(a) for a in m_old], [torch.empty(W.npts, dtype=torch.float64, device="cuda") for _ in range(3)],
+                       0.1, 0.1, 0.0, (0, 0, 0), W.dt, -1.0)
+    assert e.value.code == 1
+    plan.destroy()
