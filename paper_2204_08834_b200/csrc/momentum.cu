@@ -11,8 +11,17 @@ static cudaError_t launch_ty(const GridParams &g, const MomentumParams &mp, doub
     using T = MomTile<TY>;
     const int kc = g.nz < 32 ? g.nz : 32;
     const dim3 grid(g.nx / T::TX, g.ny / T::TY, (g.nz + kc - 1) / kc);
-    cudaError_t e = cudaFuncSetAttribute(momentum_rhs_kernel<TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM);
+    // the shared-memory attribute is a property of the kernel on a device: set once per device and tile size, not on every
+    // step (a driver call on the host; a second thread that gets here at the same time sets it twice, which is harmless)
+    static bool attr_set[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !attr_set[dev]) {
+        e = cudaFuncSetAttribute(momentum_rhs_kernel<TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) attr_set[dev] = true;
+    }
     momentum_rhs_kernel<TY><<<grid, T::NT, T::SMEM, st>>>(g, mp, dt, kc, u, v, w, phi, kappa, p, po, m_old[0], m_old[1], m_old[2],
                                                           m_new[0], m_new[1], m_new[2], rhs, us, vs, ws);
     return cudaGetLastError();
