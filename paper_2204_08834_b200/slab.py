@@ -5,7 +5,8 @@ stages of the y transform and of the z stage, written straight into the peers' m
   * the partition (which planes / which rows of ky a rank owns) -- `partition`,
   * making every rank's exchange buffer addressable by every other rank -- one process: plain device pointers
     (`SlabGroup`); one process per GPU under torchrun: torch symmetric memory (`SlabRank`),
-  * a stream-ordered barrier between the three phases of a step (`SlabRank`: an NCCL all-reduce of one element).
+  * a stream-ordered barrier between the three phases of a step (`SlabRank`: an NCCL all-reduce of one element),
+  * refreshing the halo planes a step does not produce (plane 0 of w, both halo planes of phi) -- `exchange_halos`.
 No arithmetic of the method happens here.
 """
 import torch
@@ -41,6 +42,49 @@ def backward_destinations(k, j, nz, ny, n_ranks, periodic):
     return out
 
 
+def halo_neighbours(n_ranks, rank, periodic):
+    """(below, above): the ranks that own the plane below / above `rank`'s slab; None beyond a wall"""
+    below = rank - 1 if rank > 0 else (n_ranks - 1 if periodic else None)
+    above = rank + 1 if rank + 1 < n_ranks else (0 if periodic else None)
+    return below, above
+
+
+def exchange_halos(w, phi, nzl, periodic, group=None):
+    """Refresh the halo planes a step reads but does not produce (include/flutas.h, flutas_slab_*: "on entry the halo planes
+    of phi (both) and of w (plane 0) must hold the neighbours' values") -- one rank per process, any backend, the local
+    arrays of (nzl + 2) planes being CPU or CUDA tensors.  A step leaves p^(n+1) with its halos; u, v need none; w and phi
+    are their producers' job, and in a time loop that applies steps back to back this is the producer.
+    Every rank sends its top owned plane of w and of phi upwards and its bottom owned plane of phi downwards (pure data
+    movement; point-to-point, two messages per neighbour pair).  Stream-ordered on NCCL like any collective."""
+    grp = group if group is not None else dist.group.WORLD
+    n_ranks, rank = dist.get_world_size(grp), dist.get_rank(grp)
+    below, above = halo_neighbours(n_ranks, rank, periodic)
+    wv, fv = w.view(nzl + 2, -1), phi.view(nzl + 2, -1)
+    up = torch.stack((wv[nzl], fv[nzl]))                 # to the rank above: its plane 0 of w and of phi
+    down = fv[1].clone()                                 # to the rank below: its plane nzl + 1 of phi
+    if n_ranks == 1:
+        if periodic:
+            wv[0].copy_(up[0]); fv[0].copy_(up[1]); fv[nzl + 1].copy_(down)
+        return
+    from_below, from_above = torch.empty_like(up), torch.empty_like(down)
+    peer = lambda r: dist.get_global_rank(grp, r)
+    ops = []
+    # upward messages first, on both sides, so that two messages between the same pair (n_ranks = 2) match in order
+    if above is not None:
+        ops.append(dist.P2POp(dist.isend, up, peer(above), grp, 0))
+    if below is not None:
+        ops.append(dist.P2POp(dist.irecv, from_below, peer(below), grp, 0))
+        ops.append(dist.P2POp(dist.isend, down, peer(below), grp, 1))
+    if above is not None:
+        ops.append(dist.P2POp(dist.irecv, from_above, peer(above), grp, 1))
+    for req in dist.batch_isend_irecv(ops):
+        req.wait()
+    if below is not None:
+        wv[0].copy_(from_below[0]); fv[0].copy_(from_below[1])
+    if above is not None:
+        fv[nzl + 1].copy_(from_above)
+
+
 class SlabGroup:
     """All n_ranks of a decomposition driven by ONE process on the current device, phase by phase on one stream (what a
     single-GPU box can run: the ranks' kernels never wait for one another, stream order is the barrier)."""
@@ -63,6 +107,19 @@ class SlabGroup:
             for r, pl in enumerate(self.plans):
                 u, v, w, phi, p, po = fields[r]
                 pl.step_phase(phase, u, v, w, phi, p, po, p if p_out is None else p_out[r], dt, dt_ratio)
+
+    def exchange_halos(self, fields, periodic):
+        """exchange_halos (above) for the one-process group: fields[r] = (u, v, w, phi, p, p_old); plane 0 of w and both halo
+        planes of phi of every rank from the neighbours' owned planes, as copies on the current stream"""
+        n, nzl = self.n_ranks, self.nzl
+        for r in range(n):
+            below, above = halo_neighbours(n, r, periodic)
+            w, phi = fields[r][2].view(nzl + 2, -1), fields[r][3].view(nzl + 2, -1)
+            if below is not None:
+                w[0].copy_(fields[below][2].view(nzl + 2, -1)[nzl])
+                phi[0].copy_(fields[below][3].view(nzl + 2, -1)[nzl])
+            if above is not None:
+                phi[nzl + 1].copy_(fields[above][3].view(nzl + 2, -1)[1])
 
     def destroy(self):
         for pl in self.plans:
@@ -99,6 +156,11 @@ class SlabRank:
             self.plan.step_phase(phase, u, v, w, phi, p, p_old, p if p_out is None else p_out, dt, dt_ratio)
             if phase < 2:
                 self.barrier_on_stream()
+
+    def exchange_halos(self, w, phi):
+        """refresh plane 0 of w and both halo planes of phi from the neighbours (see exchange_halos above); call between two
+        steps of a loop that feeds a step's velocity back in"""
+        exchange_halos(w, phi, self.nzl, self.plan.bc_z == 0, self.group)
 
     def destroy(self):
         self.plan.destroy()

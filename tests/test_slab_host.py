@@ -132,3 +132,55 @@ def test_maps_are_the_two_transposes_gloo():
         p.join(timeout=60)
         assert p.exitcode == 0
     assert out == [(0, True, True), (1, True, True)]
+
+
+def test_halo_neighbours():
+    assert slab.halo_neighbours(4, 0, True) == (3, 1) and slab.halo_neighbours(4, 3, True) == (2, 0)
+    assert slab.halo_neighbours(4, 0, False) == (None, 1) and slab.halo_neighbours(4, 3, False) == (2, None)
+    assert slab.halo_neighbours(1, 0, True) == (0, 0) and slab.halo_neighbours(1, 0, False) == (None, None)
+
+
+def _halo_worker(rank, world, port, q):
+    os.environ.update(WORLD_SIZE=str(world), RANK=str(rank), LOCAL_RANK=str(rank), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    import torch
+    import torch.distributed as dist
+    import workloads as wl
+    dist.init_process_group(backend="gloo", rank=rank, world_size=world)
+    nz, ny, nx = 8, 3, 5
+    nzl = nz // world
+    rng = np.random.default_rng(3)
+    w_full, phi_full = rng.standard_normal((nz, ny, nx)), rng.standard_normal((nz, ny, nx))     # the same on every rank
+    ok = []
+    for periodic in (True, False):
+        want_w, want_phi = (wl.slab_split(a, world, periodic)[rank] for a in (w_full, phi_full))
+        w, phi = want_w.copy(), want_phi.copy()
+        w[0] = w[nzl + 1] = phi[0] = phi[nzl + 1] = -7.0                                        # stale halos
+        tw, tp = torch.from_numpy(w), torch.from_numpy(phi)
+        slab.exchange_halos(tw, tp, nzl, periodic)
+        below, above = slab.halo_neighbours(world, rank, periodic)
+        # what a step reads: plane 0 of w, both halo planes of phi; planes beyond a wall stay as they were (never read)
+        good = np.array_equal(w[1:nzl + 1], want_w[1:nzl + 1]) and np.array_equal(phi[1:nzl + 1], want_phi[1:nzl + 1])
+        good &= np.array_equal(w[0], want_w[0]) and np.array_equal(phi[0], want_phi[0]) if below is not None else bool(np.all(w[0] == -7.0))
+        good &= np.array_equal(phi[nzl + 1], want_phi[nzl + 1]) if above is not None else bool(np.all(phi[nzl + 1] == -7.0))
+        good &= bool(np.all(w[nzl + 1] == -7.0))                                                # the upper halo of w is never needed
+        ok.append(bool(good))
+    q.put((rank, *ok))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 4])
+def test_halo_exchange_gloo(world):
+    """exchange_halos between processes: with two ranks both messages of a rank go to the same peer (order matters), with
+    four every rank has two distinct neighbours; periodic and wall-bounded"""
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_halo_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    out = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert out == [(r, True, True) for r in range(world)]
