@@ -2,7 +2,7 @@
 
 Every stored entry of u, v, w and p after one flutas_projection_step is compared with oracle.projection_step (the plain
 definition: literal stencils, naive O(n^2) DFT per line, textbook Thomas) on the same seeded inputs, relative
-L2 <= 1e-10 per field -- north_star's bar, SURVEY.md sec. 8(c) "Parity metric".  The oracle needs about 40 s
+L2 <= 1e-10 per field -- north_star's bar, SURVEY.md sec. 8(c) "Parity metric" -- and max |difference| <= 1e-9 max |field|.  The oracle needs about 40 s
 (512^3) and 4 minutes (1024 x 1024 x 512, ~45 GB of host memory) on the GPU box's 16 host cores.
 Beside the element-wise comparison, what is unique about the result is checked through independent operators:
 the right-hand side element by element (oracle.rhs, <= 1e-13), the residual || L p - (rhs - mean rhs) || / || rhs ||,
@@ -50,6 +50,7 @@ def _check_full_size(oracle, W):
     del rhs_gpu
     errs = {n: rel_l2(g, w_) for n, g, w_ in zip("uvwp", got, want)}
     mx = {n: float(np.max(np.abs(g - w_))) for n, g, w_ in zip("uvwp", got, want)}
+    top = {n: float(np.max(np.abs(w_))) for n, w_ in zip("uvwp", want)}
     del want
     u, v, w, p = got
     rn = np.linalg.norm(rhs)
@@ -63,6 +64,9 @@ def _check_full_size(oracle, W):
     assert e_rhs <= 1e-13
     for n, e in errs.items():
         assert e <= TOL, (W.name, n, e)
+        # ... and no single entry hides behind the norm (SURVEY.md:471-474): at 1.3e8 points a relative L2 of 1e-10 alone
+        # would tolerate entries that are off by 1e-6 of the rms
+        assert mx[n] <= 1e-9 * top[n], (W.name, n, mx[n], top[n])
     assert res <= 1e-11 and mean_p <= 1e-10 and dn <= 1e-11
     if wall:
         assert np.array_equal(w[-1], W.w[-1])
