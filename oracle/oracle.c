@@ -814,8 +814,20 @@ static double ln_cosh(double x) {
 /* int_a^b 1/2 [1 + tanh(beta (alpha x + gamma))] dx */
 static double tanh_integral(double a, double b, double alpha, double gamma, double beta) {
     if (fabs(alpha) < 1e-12) return (b - a) * 0.5 * (1.0 + tanh(beta * gamma));
-    return 0.5 * ((b - a) + (ln_cosh(beta * (alpha * b + gamma)) - ln_cosh(beta * (alpha * a + gamma))) / (beta * alpha));
+    /* the antiderivative of tanh is ln cosh: int = 1/2 [(b - a) + (ln cosh z_b - ln cosh z_a) / (beta alpha)], z = beta (alpha x + gamma).
+     * When the increment delta = z_b - z_a is small (a normal almost perpendicular to the direction of integration, or a
+     * small swept interval) the two logarithms agree in their leading digits and their difference, divided by beta alpha,
+     * would lose them: |alpha| = 1e-9 leaves 7 digits.  The same difference without cancellation:
+     *   ln cosh z_b - ln cosh z_a = ln(cosh delta + tanh z_a sinh delta) = log1p(2 sinh^2(delta/2) + tanh z_a sinh delta) */
+    double za = beta * (alpha * a + gamma), delta = beta * alpha * (b - a);
+    if (fabs(delta) < 0.1) {
+        double sh = sinh(0.5 * delta);
+        return 0.5 * ((b - a) + log1p(2.0 * sh * sh + tanh(za) * sinh(delta)) / (beta * alpha));
+    }
+    return 0.5 * ((b - a) + (ln_cosh(beta * (alpha * b + gamma)) - ln_cosh(za)) / (beta * alpha));
 }
+/* the function above, for the pins (tests/test_oracle_pins_vof.py V9) */
+double oracle_tanh_integral(double a, double b, double alpha, double gamma, double beta) { return tanh_integral(a, b, alpha, gamma, beta); }
 static const double GAUSS2[2] = {0.5 - 0.28867513459481288225457439025098, 0.5 + 0.28867513459481288225457439025098};
 
 /* mean of H^ over x~_dir in [a, b] and the full unit square across: exact along dir, 2 x 2 Gauss across (n: normal, d: offset) */

@@ -172,6 +172,10 @@ int oracle_vof_step(int nx, int ny, int nz, double lx, double ly, double lz, dou
 int oracle_vof_reconstruct(int nx, int ny, int nz, double beta, const double *phi, double *n_out, double *d_out,
                            int *flat_out, int nthreads);
 
+/* int_a^b 1/2 [1 + tanh(beta (alpha x + gamma))] dx, the one-dimensional integral every volume and flux of the MTHINC
+ * reconstruction is made of (eq. 10 integrated along one direction; A.9-A.13, A.27): exposed for the pins. */
+double oracle_tanh_integral(double a, double b, double alpha, double gamma, double beta);
+
 /* number of OpenMP threads a call with this nthreads argument would use */
 int oracle_threads(int nthreads);
 

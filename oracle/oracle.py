@@ -47,6 +47,8 @@ _lib.oracle_vof_step.argtypes = [_ci, _ci, _ci, _cd, _cd, _cd, _cd, _cd] + [_dp]
 _lib.oracle_vof_step.restype = _ci
 _lib.oracle_vof_reconstruct.argtypes = [_ci, _ci, _ci, _cd, _dp, _dp, _dp, ctypes.POINTER(_ci), _ci]
 _lib.oracle_vof_reconstruct.restype = _ci
+_lib.oracle_tanh_integral.argtypes = [_cd] * 5
+_lib.oracle_tanh_integral.restype = _cd
 _lib.oracle_threads.argtypes = [_ci]
 for _f in ("oracle_rhs_vdt", "oracle_projection_step_vdt", "oracle_rhs", "oracle_poisson", "oracle_projection_step", "oracle_projection_step_paper",
            "oracle_dft_axis", "oracle_divergence", "oracle_laplacian", "oracle_threads"):
@@ -277,6 +279,11 @@ def vof_step(phi, u, v, w, box, beta, dt, nthreads=0):
     _check(_lib.oracle_vof_step(nx, ny, nz, float(box[0]), float(box[1]), float(box[2]), float(beta), float(dt),
                                 _p(phi), _p(u), _p(v), _p(w), _p(out), nthreads), "oracle_vof_step")
     return out
+
+
+def tanh_integral(a, b, alpha, gamma, beta):
+    """int_a^b 1/2 [1 + tanh(beta (alpha x + gamma))] dx"""
+    return _lib.oracle_tanh_integral(float(a), float(b), float(alpha), float(gamma), float(beta))
 
 
 def vof_reconstruct(phi, beta, nthreads=0):

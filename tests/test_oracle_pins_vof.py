@@ -16,6 +16,9 @@ PAPER.md:104-132, Appendix A).  The paper prints no worked numbers for one step,
       phi' = phi - (F_+ - F_-)/dl with F the integral of the DONOR cell's H^ over [1 - c, 1] (u >= 0) or [0, |c|] (u < 0),
       evaluated with an independent 64-point Gauss-Legendre rule from the oracle's own (n, d) -- the wrong end of the cell,
       the wrong donor or the wrong sign fails
+  V9  the one-dimensional integral of the tanh profile, which every volume and flux is made of, against 50-digit values
+      (mpmath) -- in particular for normals almost perpendicular to the direction of integration (|alpha| = 1e-11 ... 1e-3),
+      where the textbook difference of two ln cosh loses up to nine digits
 """
 import numpy as np
 import pytest
@@ -220,3 +223,20 @@ def test_v8_partial_cfl_flux_integrates_the_donor_cell_over_the_swept_interval(o
                       for idx in [tuple(idx)]])
     right = np.array([vol[tuple(idx)] for idx in np.argwhere(flat == 0)[:50]])
     assert np.abs(wrong - right).max() > 1e-3
+
+
+@pytest.mark.parametrize("beta", [2.0, 3.0])
+def test_v9_tanh_integral_against_high_precision_values(oracle_mod, beta):
+    mpmath = pytest.importorskip("mpmath")
+    mpmath.mp.dps = 50
+    worst = 0.0
+    for alpha in (1e-11, -1e-11, 1e-9, -1e-9, 1e-6, 1e-3, -0.02, 0.3, -0.7, 1.0):
+        for gamma in (-1.3, -0.2, 0.0, 0.05, 0.9):
+            for a, b in ((0.0, 1.0), (0.63, 1.0), (0.0, 0.37), (0.999, 1.0)):
+                got = oracle_mod.tanh_integral(a, b, alpha, gamma, beta)
+                al, ga, be, aa, bb = (mpmath.mpf(x) for x in (alpha, gamma, beta, a, b))
+                want = ((bb - aa) + (mpmath.log(mpmath.cosh(be * (al * bb + ga))) - mpmath.log(mpmath.cosh(be * (al * aa + ga)))) / (be * al)) / 2
+                # the integral is a volume fraction of the slice times its length: what matters (it is added to phi = O(1)) is
+                # the error relative to (b - a); where the slice is almost empty the relative error of the value itself is larger
+                worst = max(worst, abs(float((mpmath.mpf(got) - want) / (bb - aa))))
+    assert worst < 1e-15, worst
