@@ -156,11 +156,27 @@ __device__ __forceinline__ double vof_slice(const VofRecon &r, double a, double 
     const double G2 = r.E[T1][1] * r.E[T2][0] * r.D, G3 = r.E[T1][1] * r.E[T2][1] * r.D;
     if (fabs(alpha) < 1e-12)      // 1/2 (1 + tanh z) = e^{2z} / (1 + e^{2z})
         return (b - a) * 0.25 * (G0 * rcp_normal(1.0 + G0) + G1 * rcp_normal(1.0 + G1) + G2 * rcp_normal(1.0 + G2) + G3 * rcp_normal(1.0 + G3));
-    const double Ea = a == 0.0 ? 1.0 : exp(tb * alpha * a);
-    const double Eb = b == 1.0 ? r.E[DIR][0] * r.E[DIR][1] : exp(tb * alpha * b);
-    const double num = fma(Eb, G0, 1.0) * fma(Eb, G1, 1.0) * (fma(Eb, G2, 1.0) * fma(Eb, G3, 1.0));
-    const double den = fma(Ea, G0, 1.0) * fma(Ea, G1, 1.0) * (fma(Ea, G2, 1.0) * fma(Ea, G3, 1.0));
-    return log(num * rcp_normal(den)) * rcp_normal(4.0 * tb * alpha);
+    // mean over the four Gauss points of int_a^b = ln[ prod_i (1 + E_b G_i) / prod_i (1 + E_a G_i) ] / (4 * 2 beta alpha), E_x = e^{2 beta alpha x}.
+    // The quotient is 1 + O(2 beta alpha (b - a)): for a normal almost perpendicular to the sweep, or a thin slice, its
+    // logarithm would lose the leading digits of that increment (|alpha| = 1e-9 leaves 7).  So the quotient is never formed:
+    // with "lo" the end of [a, b] with the smaller exponent and e = e^{|2 beta alpha (b - a)|} - 1 >= 0, every factor at the
+    // other end is the factor at lo plus e h_i (h_i = E_lo G_i), the difference of the two products is e times a polynomial
+    // in e with positive coefficients -- no subtraction anywhere -- and the result is +- log1p(e poly / prod_lo), accurate for
+    // every alpha.  One expm1 and one log1p per face (before: one exp and one log); E_lo follows from the known end
+    // (E_0 = 1, E_1 = the cell's table) without another exponential.
+    const double dl = tb * alpha * (b - a);
+    const bool up = dl >= 0.0;                                   // lo = a (up) or b
+    const double e = expm1(fabs(dl)), E1 = r.E[DIR][0] * r.E[DIR][1];
+    const double Elo = up ? (a == 0.0 ? 1.0 : (b == 1.0 ? E1 * rcp_normal(1.0 + e) : exp(tb * alpha * a)))
+                          : (b == 1.0 ? E1 : (a == 0.0 ? rcp_normal(1.0 + e) : exp(tb * alpha * b)));
+    const double h0 = Elo * G0, h1 = Elo * G1, h2 = Elo * G2, h3 = Elo * G3;
+    const double d0 = 1.0 + h0, d1 = 1.0 + h1, d2 = 1.0 + h2, d3 = 1.0 + h3;
+    const double A0 = d0 * d1, A1 = fma(d0, h1, h0 * d1), A2 = h0 * h1;      // (d0 + e h0)(d1 + e h1) = A0 + e A1 + e^2 A2
+    const double B0 = d2 * d3, B1 = fma(d2, h3, h2 * d3), B2 = h2 * h3;
+    const double c1 = fma(A0, B1, A1 * B0), c2 = fma(A0, B2, fma(A1, B1, A2 * B0)), c3 = fma(A1, B2, A2 * B1), c4 = A2 * B2;
+    const double x = e * fma(e, fma(e, fma(e, c4, c3), c2), c1) * rcp_normal(A0 * B0);
+    const double L = log1p(x);
+    return (up ? L : -L) * rcp_normal(4.0 * tb * alpha);
 }
 
 // A block owns VofTile::CELLS consecutive cells.  Pass 1: every cell finds out which of its faces it is the donor of (its +

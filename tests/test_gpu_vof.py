@@ -88,3 +88,27 @@ def test_vof_argument_errors():
         plan.vof_step(*d, d[0], -2.0, 1e-3)
     assert e.value.code == 1
     plan.destroy()
+
+
+def test_vof_step_with_nearly_grid_aligned_interfaces(oracle_mod):
+    """two sheets normal to z whose height varies by 1e-10 ... 1e-6 of a cell along x and y: the normals have x, y components
+    of 1e-11 ... 1e-7, so the sweeps along x and y integrate with |alpha| tiny but above the flat-normal cut-off -- the
+    range where a difference of logarithms divided by alpha loses its digits (both sides now use cancellation-free forms,
+    each its own; oracle pin V9)"""
+    nx, ny, nz = 64, 32, 32
+    W = wl.random_case(nx, ny, nz, PER, 1.0, 114)
+    z, y, x = np.meshgrid(np.arange(nz) + 0.5, np.arange(ny) + 0.5, np.arange(nx) + 0.5, indexing="ij")
+    amp = 10.0 ** (-10.0 + 4.0 * (y // 8) / 3.0)                       # 1e-10, 2e-9, 5e-8, 1e-6 in four bands of y
+    ripple = amp * (np.sin(2 * np.pi * x / nx) + 0.5 * np.cos(2 * np.pi * 3 * y / ny))
+    W.phi = 0.5 * (np.tanh((z - 9.3 + ripple) / 1.2) - np.tanh((z - 22.6 - ripple) / 1.2))
+    dt = _cfl_dt(W, 0.4)
+    n, _, flat = oracle_mod.vof_reconstruct(W.phi, 2.0)
+    small = (flat == 0) & (np.abs(n[..., 0]) > 1e-12) & (np.abs(n[..., 0]) < 1e-6)
+    assert small.sum() > 1000                                           # the case does exercise that range
+    want = oracle_mod.vof_step(W.phi, W.u, W.v, W.w, W.box, 2.0, dt)
+    plan = plan_for(W)
+    got = _gpu_vof(plan, W.phi, W, 2.0, dt)
+    err = rel_l2(got, want)
+    print(f"nearly aligned: rel L2 {err:.2e}, max abs {np.abs(got - want).max():.2e}, cells with 1e-12 < |n_x| < 1e-6: {small.sum()}")
+    assert err <= 1e-12 and np.abs(got - want).max() <= 1e-11
+    plan.destroy()
